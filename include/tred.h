@@ -1,0 +1,209 @@
+/*
+ * tred.h -- C ABI of the B200-native TRED hot path (arxiv 2602.12052).
+ *
+ * "Segments in, per-pixel current waveforms out" (Fig. 1):
+ *
+ *   tred_drift            R/A/D of Fig. 1: attachment, drift, diffusion width
+ *   tred_blockbin         block-sparse binned tensor: occupied-block list
+ *   tred_effq             effective charge, Eq. (9)-(10)
+ *   tred_convolve         interlaced FFT convolution, Eq. (12)/(14)
+ *   tred_gather_waveforms overlap-add of block outputs on unique pixels
+ *
+ * Conventions
+ *   - Every pointer named d_* is DEVICE memory, h_* is HOST memory.  All device buffers,
+ *     workspaces included, are allocated by the caller and only borrowed; the library
+ *     never allocates device memory and never synchronises the host inside a call.
+ *     Calls are enqueued on `stream` (a cudaStream_t passed as void*).
+ *   - Results of data-dependent size use "capacity + device-side count": the count is
+ *     written to device memory; entries beyond the capacity are not written.  The caller
+ *     reads the count (its own synchronisation), re-allocates and calls again if needed.
+ *   - Return value: TRED_OK or a negative tred_status.  TRED_ECUDA reports the CUDA error
+ *     seen when the kernels were enqueued; asynchronous faults surface on the caller's
+ *     next synchronisation.
+ *   - Units: mm, microseconds, electrons.  Fine grid G: point (i,j,k)
+ *     is the CENTRE of cuboid (i,j,k): x = origin_x + (i+1/2) h, h = pitch/sub,
+ *     t = t_origin + (k+1/2) tick.  Pixel P = i div sub, sub-pixel phase j = i mod sub.
+ *   - Block key (int64): (bt*NBx + bx)*NBy + by, time slab major; keys are sorted
+ *     ascending.  Tile / slab-pixel key: (tb*npix_x + px)*npix_y + py.
+ *   - Charge outside the grid and current outside the pixel plane / readout window are
+ *     dropped (reading G13).
+ *   - There is no CPU fallback: without a CUDA device every compute call fails.
+ */
+#ifndef TRED_H
+#define TRED_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum tred_status {
+  TRED_OK = 0,
+  TRED_EINVAL = -1,        /* bad argument or configuration                    */
+  TRED_ECAP = -2,          /* caller-provided capacity / workspace too small   */
+  TRED_ECUDA = -3,         /* CUDA runtime error (see tred_last_cuda_error)    */
+  TRED_EUNSUPPORTED = -4   /* configuration outside what the kernels support   */
+} tred_status;
+
+/* Plain-data configuration, host memory, copied by tred_create. */
+typedef struct tred_config {
+  int32_t npix_x, npix_y;        /* pixel plane                                           */
+  int32_t sub;                   /* S: sub-pixel factor (10)               */
+  int32_t nticks;                /* readout window in ticks                               */
+  double  pitch_mm, tick_us;
+  double  origin_x_mm, origin_y_mm, t_origin_us;
+  double  v_mm_us;               /* drift velocity                                        */
+  double  lifetime_us;           /* electron lifetime tau                                 */
+  double  DL_mm2_us, DT_mm2_us;  /* longitudinal / transverse diffusion coefficients      */
+  double  sigma_min_xy_mm, sigma_min_t_us;   /* minimum diffusion scale   */
+  double  nsigma;                /* half-width of the charge box in sigmas (reading G9)   */
+  double  point_thresh;          /* point/line switch, PAPER.md:L148 (0.1)                */
+  int32_t gl_n;                  /* Gauss-Legendre points per axis, 1..4                  */
+  int32_t block[3];              /* Bx, By (fine-grid points), Bt (ticks): powers of two  */
+  int32_t resp_half;             /* H: response covers (2H+1)^2 pixels                    */
+  int32_t resp_nticks;           /* Tr: response length in ticks                          */
+} tred_config;
+
+/* Sizes derived from a configuration (host-side helper, no device work). */
+typedef struct tred_dims {
+  int64_t NG[3];          /* fine-grid points (x, y, t)                                   */
+  int64_t NB[3];          /* blocks per axis = ceil(NG/B)                                 */
+  int32_t fft_len;        /* L: power of two >= Bt + Tr - 1               */
+  int32_t out_len;        /* Bt + Tr - 1: ticks of one block's output                     */
+  int32_t n_over;         /* ceil(out_len / Bt): tiles (Tt = Bt) one output spans         */
+  int32_t out_px, out_py; /* pixels per axis of one block's output footprint              */
+  int32_t n_class;        /* sub-pixel alignment classes of a block origin                */
+  int64_t rhat_floats;    /* floats of the response spectrum: L * S*S*(2H+1)^2            */
+  int64_t block_floats;   /* Bx*By*Bt                                                     */
+} tred_dims;
+
+typedef struct tred_ctx tred_ctx;   /* opaque, host memory */
+
+int  tred_get_dims(const tred_config* cfg, tred_dims* out);
+int  tred_create(const tred_config* cfg, tred_ctx** out);
+void tred_destroy(tred_ctx* ctx);
+const char* tred_strerror(int status);
+const char* tred_last_cuda_error(void);
+int  tred_abi_version(void);
+
+/* Number of floats / int32 per segment in the augmented SoA record (see tred_drift). */
+#define TRED_AUG_NF 10
+#define TRED_AUG_NI 8
+
+/*
+ * tred_drift -- PAPER.md:L41,L57 (A, D of Fig. 1); readings G6-G11, G14 in DESIGN.md.
+ *   d_seg    [8][nseg] float32 SoA rows x0,y0,z0,x1,y1,z1,q,t0 (row stride = nseg);
+ *            z = drift distance to the anode, q = electrons after recombination.
+ *   d_augf   [TRED_AUG_NF][nseg] float32 out: p0x,p0y,p0t,p1x,p1y,p1t (segment ends in
+ *            grid units relative to the bbox corner `lo`), sx,sy,st (sigma in grid units),
+ *            Q' = q exp(-t_m/tau).
+ *   d_augi   [TRED_AUG_NI][nseg] int32 out: lox,loy,lot,hix,hiy,hit (inclusive cuboid
+ *            bounding box, may lie partly outside the grid), flag (1 = point-like),
+ *            npair (number of blocks the clipped grid-point footprint meets).
+ *   d_npairs int64 out: sum of npair (zeroed by the call).
+ *   The integer outputs are computed in fp64, round-to-nearest, without FMA
+ *   contraction, in the operation order DESIGN.md states: they are bit-exact.
+ */
+int tred_drift(tred_ctx* ctx, int64_t nseg, const float* d_seg,
+               float* d_augf, int32_t* d_augi, int64_t* d_npairs, void* stream);
+
+/*
+ * tred_blockbin -- block-sparse binned tensor (readings G15,G16):
+ * expands every segment into (block key, segment) pairs, radix-sorts them by key
+ * (stable), run-length compacts the keys.  The payload [nblocks][Bx][By][Bt] is laid out
+ * by this list and filled by tred_effq.
+ *   cap_pairs   capacity of d_pair_seg (>= *d_npairs of tred_drift)
+ *   d_keys      [cap_blocks] int64 out: sorted unique keys of the occupied blocks
+ *   d_blk_off   [cap_blocks+1] int32 out: CSR offsets into d_pair_seg
+ *   d_pair_seg  [cap_pairs] int32 out: segment ids grouped by block, ascending in a block
+ *   d_slab_off  [NBt+1] int32 out: first block index of every time slab
+ *   d_nblocks   int64 out: number of occupied blocks (may exceed cap_blocks: TRED_ECAP
+ *               semantics, nothing beyond the capacity is written)
+ *   d_work      workspace of at least tred_blockbin_work_bytes(nseg, cap_pairs) bytes
+ */
+size_t tred_blockbin_work_bytes(const tred_ctx* ctx, int64_t nseg, int64_t cap_pairs);
+int tred_blockbin(tred_ctx* ctx, int64_t nseg, const int32_t* d_augi,
+                  int64_t cap_pairs, int64_t cap_blocks,
+                  int64_t* d_keys, int32_t* d_blk_off, int32_t* d_pair_seg,
+                  int32_t* d_slab_off, int64_t* d_nblocks,
+                  void* d_work, size_t work_bytes, void* stream);
+
+/*
+ * tred_effq -- effective charge, Eq. (9) with Eq. (10) / the point-like branch
+ * (readings G1, G4, G5, G10).  One CTA per block tile; the
+ * block's segments are evaluated on dual cells (the cell between 8 neighbouring grid
+ * points) so that every Gauss-Legendre node is evaluated once per tile and scattered to
+ * its 8 corner grid points in shared memory without atomics.
+ *   d_payload [nblocks][Bx][By][Bt] float32 out (fully overwritten).
+ */
+int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
+              const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
+              const float* d_augf, const int32_t* d_augi,
+              float* d_payload, void* stream);
+
+/*
+ * tred_prepare_response -- FFT(R^j) of Eq. (14), computed once.
+ *   d_resp [S][S][2H+1][2H+1][Tr] float32: R[jx][jy][kx+H][ky+H][tau] = current at tick
+ *          tau on the pixel displaced by (kx,ky) from the pixel holding a unit charge at
+ *          sub-pixel phase (jx,jy) (readings G3, G12).
+ *   d_rhat [rhat_floats] float32 out: spectrum, layout [L/2][S][S][2H+1][2H+1] complex
+ *          (DC and Nyquist packed in slot 0).
+ */
+int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* d_rhat, void* stream);
+
+/*
+ * tred_convolve_plan -- output footprint (O6): the (time slab, pixel) pairs
+ * met by the output of any occupied block, and the (tile, pixel) list they overlap-add to.
+ *   d_sp_keys   [cap_sp] int64 out: sorted keys (bt*npix_x + px)*npix_y + py
+ *   d_sp_off    [NBt+1] int32 out: first slab-pixel index of every slab
+ *   d_nsp       int64 out
+ *   d_tile_keys [cap_tiles] int64 out: sorted keys (tb*npix_x + px)*npix_y + py
+ *   d_ntiles    int64 out
+ *   d_work      at least tred_plan_work_bytes() bytes; its content (the slab-pixel index
+ *               map) is read again by tred_convolve and tred_gather_waveforms.
+ */
+size_t tred_plan_work_bytes(const tred_ctx* ctx);
+int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
+                       int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
+                       int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
+                       void* d_plan_work, size_t plan_work_bytes, void* stream);
+
+/*
+ * tred_convolve -- Eq. (12) evaluated as Eq. (14) per block:
+ * real FFT along time of every fine column of a block, multiply-accumulate with the
+ * response spectrum of the column's sub-pixel phase onto the (2H+1)^2 neighbouring
+ * pixels, sum over all blocks of a time slab in the frequency domain, one inverse FFT
+ * per (slab, pixel).  Processes the slabs in groups that fit the workspace.
+ *   h_slab_off [NBt+1] host copy of tred_blockbin's d_slab_off
+ *   h_sp_off   [NBt+1] host copy of tred_convolve_plan's d_sp_off
+ *   d_sp_data  [nsp][n_over*Bt] float32 out: current of (slab bt, pixel) from tick Bt*bt
+ *   d_work     at least tred_convolve_work_bytes(max blocks of a slab, max slab-pixels of
+ *              a slab) bytes; more lets several slabs share one launch.
+ */
+size_t tred_convolve_work_bytes(const tred_ctx* ctx, int64_t nblocks_chunk, int64_t nsp_chunk);
+int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
+                  const int32_t* h_slab_off, const float* d_payload, const float* d_rhat,
+                  int64_t nsp, const int64_t* d_sp_keys, const int32_t* h_sp_off,
+                  const void* d_plan_work, float* d_sp_data,
+                  void* d_work, size_t work_bytes, void* stream);
+
+/*
+ * tred_gather_waveforms -- overlap-add: every tile
+ * (pixel, Tt = Bt ticks) is the sum, in ascending slab order, of the slab outputs that
+ * cover it; optionally also writes dense rows for requested pixels.
+ *   d_tile_keys [ntiles] from tred_convolve_plan; d_tile_data [ntiles][Bt] float32 out
+ *   d_pix_ids   [npix_req] int32 flat pixel ids px*npix_y+py (may be NULL if npix_req=0)
+ *   d_dense     [npix_req][nticks] float32 out (may be NULL)
+ */
+int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_sp_data,
+                          const void* d_plan_work,
+                          int64_t ntiles, const int64_t* d_tile_keys, float* d_tile_data,
+                          int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
+                          void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRED_H */

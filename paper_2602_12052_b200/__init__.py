@@ -1,0 +1,305 @@
+"""paper_2602_12052_b200 -- thin Python binding of libtred (include/tred.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of
+`csrc/`.  PyTorch provides device memory and streams.  There is no CPU fallback: if the
+library cannot be built/loaded, or no CUDA device is present, the calls raise.
+
+    from paper_2602_12052_b200 import Tred
+    sim = Tred(cfg)                       # cfg: object/dict with the tred_config fields
+    rhat = sim.prepare_response(resp)     # resp: float32 CUDA tensor [S][S][2H+1][2H+1][Tr]
+    out = sim.simulate(seg, rhat)         # seg: float32 CUDA tensor [8][nseg]
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS"]
+
+_c_i64 = C.c_int64
+_c_p = C.c_void_p
+
+
+class TredConfig(C.Structure):
+    """Mirror of `tred_config` (include/tred.h)."""
+    _fields_ = [("npix_x", C.c_int32), ("npix_y", C.c_int32), ("sub", C.c_int32), ("nticks", C.c_int32),
+                ("pitch_mm", C.c_double), ("tick_us", C.c_double),
+                ("origin_x_mm", C.c_double), ("origin_y_mm", C.c_double), ("t_origin_us", C.c_double),
+                ("v_mm_us", C.c_double), ("lifetime_us", C.c_double),
+                ("DL_mm2_us", C.c_double), ("DT_mm2_us", C.c_double),
+                ("sigma_min_xy_mm", C.c_double), ("sigma_min_t_us", C.c_double),
+                ("nsigma", C.c_double), ("point_thresh", C.c_double),
+                ("gl_n", C.c_int32), ("block", C.c_int32 * 3),
+                ("resp_half", C.c_int32), ("resp_nticks", C.c_int32)]
+
+
+class TredDims(C.Structure):
+    """Mirror of `tred_dims` (include/tred.h)."""
+    _fields_ = [("NG", _c_i64 * 3), ("NB", _c_i64 * 3),
+                ("fft_len", C.c_int32), ("out_len", C.c_int32), ("n_over", C.c_int32),
+                ("out_px", C.c_int32), ("out_py", C.c_int32), ("n_class", C.c_int32),
+                ("rhat_floats", _c_i64), ("block_floats", _c_i64)]
+
+
+# name -> (restype, argtypes); every symbol include/tred.h declares
+EXPORTS = {
+    "tred_get_dims": (C.c_int, [C.POINTER(TredConfig), C.POINTER(TredDims)]),
+    "tred_create": (C.c_int, [C.POINTER(TredConfig), C.POINTER(_c_p)]),
+    "tred_destroy": (None, [_c_p]),
+    "tred_strerror": (C.c_char_p, [C.c_int]),
+    "tred_last_cuda_error": (C.c_char_p, []),
+    "tred_abi_version": (C.c_int, []),
+    "tred_drift": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p]),
+    "tred_blockbin_work_bytes": (C.c_size_t, [_c_p, _c_i64, _c_i64]),
+    "tred_blockbin": (C.c_int, [_c_p, _c_i64, _c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p,
+                                _c_p, C.c_size_t, _c_p]),
+    "tred_effq": (C.c_int, [_c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p]),
+    "tred_prepare_response": (C.c_int, [_c_p, _c_p, _c_p, _c_p]),
+    "tred_plan_work_bytes": (C.c_size_t, [_c_p]),
+    "tred_convolve_plan": (C.c_int, [_c_p, _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_i64, _c_p, _c_p,
+                                     _c_p, C.c_size_t, _c_p]),
+    "tred_convolve_work_bytes": (C.c_size_t, [_c_p, _c_i64, _c_i64]),
+    "tred_convolve": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
+                                _c_p, C.c_size_t, _c_p]),
+    "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p,
+                                        _c_p]),
+}
+
+_LIB = None
+
+
+class TredError(RuntimeError):
+    pass
+
+
+def lib() -> C.CDLL:
+    """Builds (if stale) and loads libtred.so; raises if that is impossible."""
+    global _LIB
+    if _LIB is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        for name, (res, args) in EXPORTS.items():
+            fn = getattr(L, name)          # AttributeError if a declared symbol is missing
+            fn.restype = res
+            fn.argtypes = args
+        _LIB = L
+    return _LIB
+
+
+_CFG_FIELDS = [f[0] for f in TredConfig._fields_]
+
+
+def make_config(cfg) -> TredConfig:
+    get = (lambda k: cfg[k]) if isinstance(cfg, dict) else (lambda k: getattr(cfg, k))
+    c = TredConfig()
+    for k in _CFG_FIELDS:
+        v = get(k)
+        if k == "block":
+            c.block[0], c.block[1], c.block[2] = (int(x) for x in v)
+        else:
+            setattr(c, k, v)
+    return c
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        L = lib()
+        msg = L.tred_strerror(rc).decode()
+        if rc == -3:
+            msg += ": " + L.tred_last_cuda_error().decode()
+        raise TredError(f"{what} failed ({rc}): {msg}")
+
+
+def get_dims(cfg) -> TredDims:
+    d = TredDims()
+    c = make_config(cfg)
+    _check(lib().tred_get_dims(C.byref(c), C.byref(d)), "tred_get_dims")
+    return d
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+class Tred:
+    """One configuration on one CUDA device.  Methods mirror the C calls one to one; the
+    tensors they return are ordinary torch CUDA tensors owned by the caller."""
+
+    def __init__(self, cfg, device="cuda:0", conv_work_bytes: int | None = None):
+        import torch
+        if not torch.cuda.is_available():
+            raise TredError("no CUDA device: the TRED path has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.L = lib()
+        self.cfg = make_config(cfg)
+        self.dims = TredDims()
+        _check(self.L.tred_get_dims(C.byref(self.cfg), C.byref(self.dims)), "tred_get_dims")
+        h = _c_p()
+        _check(self.L.tred_create(C.byref(self.cfg), C.byref(h)), "tred_create")
+        self.h = h
+        self.conv_work_bytes = conv_work_bytes
+        self._work = {}
+
+    def __del__(self):
+        try:
+            if getattr(self, "h", None):
+                self.L.tred_destroy(self.h)
+                self.h = None
+        except Exception:
+            pass
+
+    # -- helpers ------------------------------------------------------------------
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def _empty(self, shape, dtype):
+        return self.torch.empty(shape, dtype=dtype, device=self.device)
+
+    def _workbuf(self, name, nbytes):
+        """Grow-only cached byte buffer."""
+        b = self._work.get(name)
+        if b is None or b.numel() < nbytes:
+            b = None
+            self._work.pop(name, None)
+            b = self._empty((max(int(nbytes), 256),), self.torch.uint8)
+            self._work[name] = b
+        return b
+
+    # -- the calls ----------------------------------------------------------------
+    def prepare_response(self, resp):
+        t = self.torch
+        K = 2 * self.cfg.resp_half + 1
+        S = self.cfg.sub
+        assert resp.is_cuda and resp.dtype == t.float32 and resp.is_contiguous()
+        assert tuple(resp.shape) == (S, S, K, K, self.cfg.resp_nticks), resp.shape
+        rhat = self._empty((self.dims.rhat_floats,), t.float32)
+        _check(self.L.tred_prepare_response(self.h, _ptr(resp), _ptr(rhat), self._stream()),
+               "tred_prepare_response")
+        return rhat
+
+    def drift(self, seg):
+        t = self.torch
+        assert seg.is_cuda and seg.dtype == t.float32 and seg.is_contiguous() and seg.shape[0] == 8
+        nseg = seg.shape[1]
+        augf = self._empty((10, nseg), t.float32)
+        augi = self._empty((8, nseg), t.int32)
+        npairs = self._empty((1,), t.int64)
+        _check(self.L.tred_drift(self.h, nseg, _ptr(seg), _ptr(augf), _ptr(augi), _ptr(npairs),
+                                 self._stream()), "tred_drift")
+        return augf, augi, npairs
+
+    def blockbin(self, augi, cap_pairs: int, cap_blocks: int | None = None):
+        t = self.torch
+        nseg = augi.shape[1]
+        cap_blocks = cap_pairs if cap_blocks is None else cap_blocks
+        NBt = int(self.dims.NB[2])
+        keys = self._empty((max(cap_blocks, 1),), t.int64)
+        blk_off = self._empty((max(cap_blocks, 1) + 1,), t.int32)
+        pair_seg = self._empty((max(cap_pairs, 1),), t.int32)
+        slab_off = self._empty((NBt + 1,), t.int32)
+        nblocks = self._empty((1,), t.int64)
+        wb = self.L.tred_blockbin_work_bytes(self.h, nseg, cap_pairs)
+        work = self._workbuf("bin", wb)
+        _check(self.L.tred_blockbin(self.h, nseg, _ptr(augi), cap_pairs, cap_blocks, _ptr(keys),
+                                    _ptr(blk_off), _ptr(pair_seg), _ptr(slab_off), _ptr(nblocks),
+                                    _ptr(work), work.numel(), self._stream()), "tred_blockbin")
+        return keys, blk_off, pair_seg, slab_off, nblocks
+
+    def effq(self, nblocks: int, keys, blk_off, pair_seg, augf, augi, payload=None):
+        t = self.torch
+        nseg = augf.shape[1]
+        if payload is None:
+            payload = self._empty((max(nblocks, 1), self.cfg.block[0], self.cfg.block[1], self.cfg.block[2]),
+                                  t.float32)
+        _check(self.L.tred_effq(self.h, nseg, nblocks, _ptr(keys), _ptr(blk_off), _ptr(pair_seg),
+                                _ptr(augf), _ptr(augi), _ptr(payload), self._stream()), "tred_effq")
+        return payload
+
+    def convolve_plan(self, nblocks: int, keys, cap_sp: int, cap_tiles: int):
+        t = self.torch
+        NBt = int(self.dims.NB[2])
+        sp_keys = self._empty((max(cap_sp, 1),), t.int64)
+        sp_off = self._empty((NBt + 1,), t.int32)
+        nsp = self._empty((1,), t.int64)
+        tile_keys = self._empty((max(cap_tiles, 1),), t.int64)
+        ntiles = self._empty((1,), t.int64)
+        pw = self.L.tred_plan_work_bytes(self.h)
+        plan = self._empty((pw,), t.uint8)
+        _check(self.L.tred_convolve_plan(self.h, nblocks, _ptr(keys), cap_sp, _ptr(sp_keys), _ptr(sp_off),
+                                         _ptr(nsp), cap_tiles, _ptr(tile_keys), _ptr(ntiles),
+                                         _ptr(plan), plan.numel(), self._stream()), "tred_convolve_plan")
+        return sp_keys, sp_off, nsp, tile_keys, ntiles, plan
+
+    def convolve(self, nblocks: int, keys, slab_off_host, payload, rhat, nsp: int, sp_keys, sp_off_host,
+                 plan, sp_data=None, work_bytes: int | None = None):
+        t = self.torch
+        import numpy as np
+        row = self.dims.n_over * self.cfg.block[2]
+        if sp_data is None:
+            sp_data = self._empty((max(nsp, 1), row), t.float32)
+        so = np.ascontiguousarray(slab_off_host, dtype=np.int32)
+        po = np.ascontiguousarray(sp_off_host, dtype=np.int32)
+        nb_max = int(np.diff(so).max()) if len(so) > 1 else 0
+        ns_max = int(np.diff(po).max()) if len(po) > 1 else 0
+        need = self.L.tred_convolve_work_bytes(self.h, nb_max, ns_max)
+        if work_bytes is None:
+            work_bytes = self.conv_work_bytes
+        if work_bytes is None:
+            work_bytes = min(self.L.tred_convolve_work_bytes(self.h, nblocks, nsp), 8 << 30)
+        work_bytes = max(int(work_bytes), int(need))
+        work = self._workbuf("conv", work_bytes)
+        _check(self.L.tred_convolve(self.h, nblocks, _ptr(keys), so.ctypes.data_as(_c_p), _ptr(payload),
+                                    _ptr(rhat), nsp, _ptr(sp_keys), po.ctypes.data_as(_c_p), _ptr(plan),
+                                    _ptr(sp_data), _ptr(work), work.numel(), self._stream()),
+               "tred_convolve")
+        return sp_data
+
+    def gather_waveforms(self, nsp: int, sp_data, plan, ntiles: int, tile_keys, pix_ids=None):
+        t = self.torch
+        Bt = self.cfg.block[2]
+        tile_data = self._empty((max(ntiles, 1), Bt), t.float32)
+        dense = None
+        npix = 0
+        if pix_ids is not None and pix_ids.numel() > 0:
+            assert pix_ids.dtype == t.int32 and pix_ids.is_cuda
+            npix = pix_ids.numel()
+            dense = self._empty((npix, self.cfg.nticks), t.float32)
+        _check(self.L.tred_gather_waveforms(self.h, nsp, _ptr(sp_data), _ptr(plan), ntiles, _ptr(tile_keys),
+                                            _ptr(tile_data), npix, _ptr(pix_ids), _ptr(dense),
+                                            self._stream()), "tred_gather_waveforms")
+        return tile_data, dense
+
+    # -- whole path -----------------------------------------------------------------
+    def simulate(self, seg, rhat, pix_ids=None, keep=False):
+        """Segments in, per-pixel current waveforms out.  Reads three
+        device-side counts back to size the buffers (the only host synchronisations)."""
+        t = self.torch
+        nseg = seg.shape[1]
+        augf, augi, npairs = self.drift(seg)
+        cap_pairs = int(npairs.item())
+        keys, blk_off, pair_seg, slab_off, nblocks_d = self.blockbin(augi, cap_pairs)
+        nblocks = int(nblocks_d.item())
+        payload = self.effq(nblocks, keys, blk_off, pair_seg, augf, augi)
+        npixtot = self.cfg.npix_x * self.cfg.npix_y
+        NBt = int(self.dims.NB[2])
+        outp = self.dims.out_px * self.dims.out_py
+        cap_sp = min(nblocks * outp, NBt * npixtot)
+        cap_tiles = min(cap_sp * self.dims.n_over, NBt * npixtot)
+        sp_keys, sp_off, nsp_d, tile_keys, ntiles_d, plan = self.convolve_plan(nblocks, keys, cap_sp, cap_tiles)
+        counts = t.cat([nsp_d, ntiles_d]).cpu()
+        nsp, ntiles = int(counts[0]), int(counts[1])
+        so = slab_off.cpu().numpy()
+        po = sp_off.cpu().numpy()
+        sp_data = self.convolve(nblocks, keys, so, payload, rhat, nsp, sp_keys, po, plan)
+        tile_data, dense = self.gather_waveforms(nsp, sp_data, plan, ntiles, tile_keys, pix_ids)
+        out = dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, nsp=nsp, ntiles=ntiles,
+                   tile_keys=tile_keys[:ntiles], tile_data=tile_data[:ntiles], dense=dense)
+        if keep:
+            out.update(augf=augf, augi=augi, keys=keys[:nblocks], blk_off=blk_off[:nblocks + 1],
+                       pair_seg=pair_seg[:cap_pairs], slab_off=slab_off, payload=payload[:nblocks],
+                       sp_keys=sp_keys[:nsp], sp_data=sp_data[:nsp], sp_off=sp_off)
+        return out

@@ -1,0 +1,69 @@
+// Internal definitions shared by the translation units of libtred (CUDA path only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "../../include/tred.h"
+
+struct tred_ctx {
+  tred_config cfg;
+  tred_dims   dims;
+  int         num_sms;
+  int         smem_optin;     // max dynamic shared memory per block (bytes)
+};
+
+// Grid constants passed by value to kernels.
+struct TredGrid {
+  int NGx, NGy, NGt;
+  int Bx, By, Bt;
+  int NBx, NBy, NBt;
+  int S, H, Tr;
+  int npx, npy, nticks;
+  int L;            // fft length
+  int outx, outy;   // output footprint pixels of one block
+  int nover;        // tiles per output
+  int gl_n;
+};
+
+static inline TredGrid make_grid(const tred_ctx* c) {
+  TredGrid g;
+  g.NGx = (int)c->dims.NG[0]; g.NGy = (int)c->dims.NG[1]; g.NGt = (int)c->dims.NG[2];
+  g.Bx = c->cfg.block[0]; g.By = c->cfg.block[1]; g.Bt = c->cfg.block[2];
+  g.NBx = (int)c->dims.NB[0]; g.NBy = (int)c->dims.NB[1]; g.NBt = (int)c->dims.NB[2];
+  g.S = c->cfg.sub; g.H = c->cfg.resp_half; g.Tr = c->cfg.resp_nticks;
+  g.npx = c->cfg.npix_x; g.npy = c->cfg.npix_y; g.nticks = c->cfg.nticks;
+  g.L = c->dims.fft_len; g.outx = c->dims.out_px; g.outy = c->dims.out_py;
+  g.nover = c->dims.n_over; g.gl_n = c->cfg.gl_n;
+  return g;
+}
+
+void tred_set_cuda_error(cudaError_t e, const char* where);
+
+#define TRED_CUDA(call)                                                    \
+  do {                                                                     \
+    cudaError_t _e = (call);                                               \
+    if (_e != cudaSuccess) { tred_set_cuda_error(_e, #call); return TRED_ECUDA; } \
+  } while (0)
+
+#define TRED_LAUNCH_CHECK(name)                                            \
+  do {                                                                     \
+    cudaError_t _e = cudaGetLastError();                                   \
+    if (_e != cudaSuccess) { tred_set_cuda_error(_e, name); return TRED_ECUDA; } \
+  } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ---- device-wide primitives (tred_scan_sort.cu) ----------------------------------
+// Exclusive scan of int32 (n elements) into out (may alias in); writes the total to
+// d_total (int64) if non-null.  work: at least tred_scan_work_bytes(n).
+size_t tred_scan_work_bytes(int64_t n);
+int tred_exclusive_scan_i32(const int32_t* d_in, int32_t* d_out, int64_t n, int64_t* d_total,
+                            void* d_work, cudaStream_t st);
+// Stable LSD radix sort of (uint32 key, int32 value) pairs on `bits` low key bits.
+// n is read on the host (capacity); the count actually sorted is *d_n (device) if
+// d_n is non-null (elements beyond it are ignored).  Result ends in keys_out/vals_out.
+size_t tred_sort_work_bytes(int64_t n);
+int tred_radix_sort_pairs(uint32_t* d_keys_a, int32_t* d_vals_a, uint32_t* d_keys_b, int32_t* d_vals_b,
+                          int64_t n_cap, const int64_t* d_n, int bits, void* d_work, cudaStream_t st,
+                          uint32_t** keys_out, int32_t** vals_out);

@@ -1,0 +1,308 @@
+"""Parity of the CUDA path (through the C ABI of include/tred.h) with the fp64 oracle,
+element by element on the same seeded inputs.  Needs a CUDA device.
+
+Tolerances:
+  integers (bbox, flags, block keys, CSR lists, slab/tile keys): bit-exact;
+  effective charge (fp32 vs fp64): max|d| <= 2e-5 max|Qeff|, total within 1e-5;
+  waveforms: max|d| <= 1e-4 max|signal| (north_star);
+  per-pixel integrated charge: |dQ_p| <= 1e-5 max(|Q_p|, 1e-3 max_p|Q_p|) (north_star, G17).
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle as o
+
+pytestmark = pytest.mark.gpu
+
+TOL_QEFF = 2e-5
+TOL_WAVE = 1e-4
+TOL_QPIX = 1e-5
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _sim(cfg, **kw):
+    from paper_2602_12052_b200 import Tred
+    return Tred(cfg, **kw)
+
+
+def _seg_tensor(segs):
+    torch = _torch()
+    a = np.stack([segs[k] for k in gen.SEG_FIELDS]).astype(np.float32)
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _small(cfg_id):
+    """Workloads the oracle finishes in seconds, same recipe as BASELINE configs."""
+    if cfg_id == 1:
+        return gen.make_segments(1)
+    if cfg_id == 2:
+        cfg, segs = gen.make_segments(2)
+        return cfg, {k: v[:1500] for k, v in segs.items()}
+    cfg, segs = gen.make_segments(3, n_vertices=1)
+    return cfg, {k: v[:1200] for k, v in segs.items()}
+
+
+# ------------------------------------------------------------------ S1
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_drift_bit_exact(cfg_id):
+    cfg, segs = gen.make_segments(cfg_id) if cfg_id < 3 else gen.make_segments(3, n_vertices=3)
+    aug = o.drift(cfg, segs)
+    sim = _sim(cfg)
+    augf, augi, npairs = sim.drift(_seg_tensor(segs))
+    augi = augi.cpu().numpy()
+    augf = augf.cpu().numpy().astype(np.float64)
+    np.testing.assert_array_equal(augi[0:3].T, aug["lo"])
+    np.testing.assert_array_equal(augi[3:6].T, aug["hi"])
+    np.testing.assert_array_equal(augi[6], aug["flag"])
+    _, _, cnt = o.block_pairs(cfg, aug)
+    np.testing.assert_array_equal(augi[7], cnt)
+    assert int(npairs.item()) == int(cnt.sum())
+    g = o.grid_of(cfg)
+    org, h = np.array(g.org), np.array(g.h)
+    p0 = (aug["p0"] - org) / h - aug["lo"]
+    p1 = (aug["p1"] - org) / h - aug["lo"]
+    np.testing.assert_allclose(augf[0:3].T, p0, atol=4e-6)
+    np.testing.assert_allclose(augf[3:6].T, p1, atol=4e-6)
+    np.testing.assert_allclose(augf[6:9].T, aug["sig"] / h, rtol=1e-6)
+    np.testing.assert_allclose(augf[9], aug["Qp"], rtol=1e-6)
+
+
+# ------------------------------------------------------------------ S3
+def _oracle_csr(cfg, aug):
+    seg, keys, _ = o.block_pairs(cfg, aug)
+    order = np.argsort(keys, kind="stable")
+    ks, ss = keys[order], seg[order]
+    uk, first = np.unique(ks, return_index=True)
+    off = np.concatenate([first, [len(ks)]])
+    return uk, off, ss
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_blockbin_bit_exact(cfg_id):
+    cfg, segs = gen.make_segments(cfg_id) if cfg_id < 3 else gen.make_segments(3, n_vertices=4)
+    aug = o.drift(cfg, segs)
+    uk, off, ss = _oracle_csr(cfg, aug)
+    sim = _sim(cfg)
+    augf, augi, npairs = sim.drift(_seg_tensor(segs))
+    cap = int(npairs.item())
+    keys, blk_off, pair_seg, slab_off, nblocks = sim.blockbin(augi, cap)
+    nb = int(nblocks.item())
+    assert nb == len(uk)
+    np.testing.assert_array_equal(keys[:nb].cpu().numpy(), uk)
+    np.testing.assert_array_equal(blk_off[:nb + 1].cpu().numpy(), off)
+    np.testing.assert_array_equal(pair_seg[:cap].cpu().numpy(), ss)
+    g = o.grid_of(cfg)
+    bt = uk // (g.NB[0] * g.NB[1])
+    ref_slab = np.searchsorted(bt, np.arange(g.NB[2] + 1), side="left")
+    np.testing.assert_array_equal(slab_off.cpu().numpy(), ref_slab)
+    np.testing.assert_array_equal(keys[:nb].cpu().numpy(), o.blocks(cfg, aug))
+
+
+def test_blockbin_capacity_semantics_and_empty():
+    cfg, segs = gen.make_segments(1)
+    sim = _sim(cfg)
+    augf, augi, npairs = sim.drift(_seg_tensor(segs))
+    cap = int(npairs.item())
+    keys, blk_off, pair_seg, slab_off, nblocks = sim.blockbin(augi, cap, cap_blocks=10)
+    full = o.blocks(cfg, o.drift(cfg, segs))
+    assert int(nblocks.item()) == len(full)               # required count still reported
+    np.testing.assert_array_equal(keys[:10].cpu().numpy(), full[:10])
+    # empty input
+    torch = _torch()
+    empty = torch.empty((8, 0), dtype=torch.float32, device="cuda")
+    augf, augi, npairs = sim.drift(empty)
+    assert int(npairs.item()) == 0
+    keys, blk_off, pair_seg, slab_off, nblocks = sim.blockbin(augi, 0)
+    assert int(nblocks.item()) == 0 and int(slab_off.abs().sum().item()) == 0
+    out = sim.simulate(empty, sim.prepare_response(torch.zeros(
+        (cfg.sub, cfg.sub, 11, 11, cfg.resp_nticks), dtype=torch.float32, device="cuda")))
+    assert out["ntiles"] == 0 and out["nblocks"] == 0
+
+
+# ------------------------------------------------------------------ S2
+def _effq_both(cfg, segs):
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    ref = o.effq(cfg, aug, keys)
+    sim = _sim(cfg)
+    augf, augi, npairs = sim.drift(_seg_tensor(segs))
+    k, blk_off, pair_seg, slab_off, nblocks = sim.blockbin(augi, int(npairs.item()))
+    nb = int(nblocks.item())
+    assert nb == len(keys)
+    got = sim.effq(nb, k, blk_off, pair_seg, augf, augi)[:nb].cpu().numpy().astype(np.float64)
+    return aug, keys, ref, got
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_effq_parity(cfg_id):
+    cfg, segs = _small(cfg_id)
+    aug, keys, ref, got = _effq_both(cfg, segs)
+    scale = np.abs(ref).max()
+    assert scale > 0
+    assert np.abs(got - ref).max() <= TOL_QEFF * scale
+    assert abs(got.sum() - ref.sum()) <= 1e-5 * abs(ref.sum())
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4])
+@pytest.mark.parametrize("block", [(4, 4, 32), (8, 8, 64), (16, 16, 128), (32, 32, 256)])
+def test_effq_parity_sweep(n, block):
+    """Config 5's representation sweep on a small sample of config-3 inputs."""
+    cfg, segs = gen.make_segments(3, n_vertices=1)
+    cfg = cfg.with_(gl_n=n, block=block)
+    segs = {k: v[:150] for k, v in segs.items()}
+    aug, keys, ref, got = _effq_both(cfg, segs)
+    assert np.abs(got - ref).max() <= TOL_QEFF * np.abs(ref).max()
+
+
+def test_effq_point_like_and_clipped_segments():
+    """Degenerate cases: a point-like stub, a segment straddling the grid edge, one
+    wholly outside the grid (no blocks), one at z -> 0 (minimum diffusion scale)."""
+    cfg = gen.make_config(1, t_origin_us=0.0)
+    rows = [
+        (70.0, 70.0, 40.0, 70.01, 70.005, 40.01, 50.0, 0.0),       # point-like
+        (-0.3, 30.0, 50.0, 0.6, 30.4, 50.3, 6000.0, 0.0),          # straddles x = 0
+        (70.0, 140.5, 60.0, 70.5, 141.2, 60.2, 6000.0, 0.0),       # straddles y max
+        (500.0, 500.0, 50.0, 501.0, 500.0, 50.0, 6000.0, 0.0),     # outside: dropped
+        (30.0, 30.0, 0.0, 30.5, 30.5, 0.4, 6000.0, 1.0),           # z -> 0, starts at window edge
+        (60.0, 60.0, 163.0, 60.5, 60.2, 164.5, 6000.0, 0.0),       # straddles the last tick
+    ]
+    segs = {k: np.array([r[i] for r in rows], np.float32) for i, k in enumerate(gen.SEG_FIELDS)}
+    aug, keys, ref, got = _effq_both(cfg, segs)
+    assert aug["flag"][0] == 1 and aug["flag"][1] == 0
+    assert np.abs(got - ref).max() <= TOL_QEFF * np.abs(ref).max()
+
+
+# ------------------------------------------------------------------ S4 + S5
+def _wave_checks(got, ref):
+    scale = np.abs(ref).max()
+    assert scale > 0
+    assert np.abs(got - ref).max() <= TOL_WAVE * scale
+    qg, qr = got.sum(1), ref.sum(1)
+    floor = 1e-3 * np.abs(qr).max()
+    assert (np.abs(qg - qr) <= TOL_QPIX * np.maximum(np.abs(qr), floor)).all()
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_plan_tiles_bit_exact(cfg_id):
+    torch = _torch()
+    cfg, segs = _small(cfg_id)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    sim = _sim(cfg)
+    k = torch.from_numpy(keys).cuda()
+    npix = cfg.npix_x * cfg.npix_y
+    NBt = int(sim.dims.NB[2])
+    sp_keys, sp_off, nsp, tile_keys, ntiles, plan = sim.convolve_plan(len(keys), k, NBt * npix, NBt * npix)
+    ref = o.out_tiles(cfg, keys)
+    assert int(ntiles.item()) == len(ref)
+    np.testing.assert_array_equal(tile_keys[:len(ref)].cpu().numpy(), ref)
+    # slab-pixel list = the same footprint without the time spread
+    spk = sp_keys[:int(nsp.item())].cpu().numpy()
+    assert (np.diff(spk) > 0).all()
+    g = o.grid_of(cfg)
+    bt = keys // (g.NB[0] * g.NB[1])
+    assert set(np.unique(spk // npix)) == set(np.unique(bt))
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_convolve_parity_from_oracle_charge(cfg_id):
+    """S4+S5 alone: the GPU convolves the ORACLE's effective charge (cast to fp32)."""
+    torch = _torch()
+    cfg, segs = _small(cfg_id)
+    R = gen.make_response(cfg, 2000 + cfg_id)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    payload32 = o.effq(cfg, aug, keys).astype(np.float32)
+    rng = np.random.default_rng(cfg_id)
+    tiles = o.out_tiles(cfg, keys)
+    act = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
+    pix = np.sort(rng.choice(act, min(48, len(act)), replace=False))
+    ref = o.conv_fft(cfg, keys, payload32.astype(np.float64), R, pix)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    k = torch.from_numpy(keys).cuda()
+    npix = cfg.npix_x * cfg.npix_y
+    NBt = int(sim.dims.NB[2])
+    sp_keys, sp_off, nsp, tile_keys, ntiles, plan = sim.convolve_plan(len(keys), k, NBt * npix, NBt * npix)
+    g = o.grid_of(cfg)
+    bt = keys // (g.NB[0] * g.NB[1])
+    slab_off = np.searchsorted(bt, np.arange(g.NB[2] + 1), side="left").astype(np.int32)
+    nsp, ntiles = int(nsp.item()), int(ntiles.item())
+    sp_data = sim.convolve(len(keys), k, slab_off, torch.from_numpy(payload32).cuda(), rhat, nsp, sp_keys,
+                           sp_off.cpu().numpy(), plan)
+    tile_data, dense = sim.gather_waveforms(nsp, sp_data, plan, ntiles, tile_keys,
+                                            torch.from_numpy(pix.astype(np.int32)).cuda())
+    _wave_checks(dense.cpu().numpy().astype(np.float64), ref)
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_end_to_end_parity(cfg_id):
+    """Whole path, segments in -> waveforms out, against the oracle's direct sum."""
+    torch = _torch()
+    cfg, segs = _small(cfg_id)
+    R = gen.make_response(cfg, 2000 + cfg_id)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    payload = o.effq(cfg, aug, keys)
+    tiles = o.out_tiles(cfg, keys)
+    act = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
+    rng = np.random.default_rng(10 + cfg_id)
+    pix = np.sort(rng.choice(act, min(32, len(act)), replace=False))
+    ref = o.conv_direct(cfg, keys, payload, R, pix)
+    sim = _sim(cfg)
+    out = sim.simulate(_seg_tensor(segs), sim.prepare_response(torch.from_numpy(R).cuda()),
+                       torch.from_numpy(pix.astype(np.int32)).cuda())
+    assert out["nblocks"] == len(keys) and out["ntiles"] == len(tiles)
+    np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
+    got = out["dense"].cpu().numpy().astype(np.float64)
+    _wave_checks(got, ref)
+    # the sparse tiles hold the same numbers as the dense rows
+    tk = out["tile_keys"].cpu().numpy()
+    td = out["tile_data"].cpu().numpy()
+    npix = cfg.npix_x * cfg.npix_y
+    Bt = cfg.block[2]
+    for r, p in enumerate(pix[:8]):
+        for i in np.flatnonzero(tk % npix == p):
+            tb = tk[i] // npix
+            n = min(Bt, cfg.nticks - tb * Bt)
+            np.testing.assert_array_equal(td[i, :n], out["dense"][r, tb * Bt: tb * Bt + n].cpu().numpy())
+
+
+def test_convolve_asymmetric_response_and_chunking():
+    """An unstructured response pins index order / sign on the GPU too; a small
+    workspace forces the slab-group loop, which must give identical bits."""
+    torch = _torch()
+    cfg, segs = _small(1)
+    R = gen.make_random_response(cfg, 77)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    payload = o.effq(cfg, aug, keys)
+    pix = np.arange(0, cfg.npix_x * cfg.npix_y, 13)
+    ref = o.conv_fft(cfg, keys, payload, R, pix)
+    outs = []
+    for wb in (None, 1):          # 1 byte -> raised to the per-slab minimum
+        sim = _sim(cfg, conv_work_bytes=wb)
+        out = sim.simulate(_seg_tensor(segs), sim.prepare_response(torch.from_numpy(R).cuda()),
+                           torch.from_numpy(pix.astype(np.int32)).cuda())
+        outs.append(out["dense"].cpu().numpy())
+    np.testing.assert_array_equal(outs[0], outs[1])
+    got = outs[0].astype(np.float64)
+    assert np.abs(got - ref).max() <= TOL_WAVE * np.abs(ref).max()
+
+
+def test_deterministic_bits():
+    """No unordered float atomics anywhere: two runs give identical bits."""
+    torch = _torch()
+    cfg, segs = _small(2)
+    R = gen.make_response(cfg, 2002)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    a = sim.simulate(_seg_tensor(segs), rhat, keep=True)
+    b = sim.simulate(_seg_tensor(segs), rhat, keep=True)
+    assert torch.equal(a["payload"], b["payload"])
+    assert torch.equal(a["tile_data"], b["tile_data"])
