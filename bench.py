@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the driver.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+A "step" is one pass of the whole hot path (tred_drift, tred_blockbin, tred_effq,
+tred_convolve_plan, tred_convolve, tred_gather_waveforms) over one synthetic event.
+N = 1 workload: BASELINE.json configs[1] (one neutrino-like event, ~14k 1-mm segments,
+128x128 pixels x 4096 ticks, 3-point Gauss-Legendre, blocks 8x8x64, response 11x11 x 100
+phases x 400 ticks).  N > 1: every rank simulates its own event of the same recipe (seed
+1002 + rank): the path shards over independent events with no collective ("weak").
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import gen  # noqa: E402
+
+METRIC = "segments_per_s"
+UNIT = "segments/s"
+FMA_LANES_PER_SM = 128          # fp32 FMA lanes per SM (4 SMSPs x 32), B300_MICROARCH.md
+
+
+def _env_int(k, d):
+    try:
+        return int(os.environ.get(k, d))
+    except ValueError:
+        return d
+
+
+def workload(cfg_id: int, rank: int):
+    cfg, segs = gen.make_segments(cfg_id, seed=1000 + cfg_id + rank)
+    R = gen.make_response(cfg, 2000 + cfg_id)
+    seg = np.ascontiguousarray(np.stack([segs[k] for k in gen.SEG_FIELDS]).astype(np.float32))
+    return cfg, segs, seg, R
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi sampled during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(self.index)],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.p = None
+
+    def _read(self):
+        for line in self.p.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=2)
+        except Exception:
+            self.p.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- oracle legs
+def oracle_sample(cfg, segs, R, n_sample: int):
+    """The oracle as it stands on the first n_sample segments: whole path, every pixel of
+    its output footprint.  Returns (segments, seconds, threads)."""
+    import oracle as o
+    sub = {k: v[:n_sample] for k, v in segs.items()}
+    t0 = time.perf_counter()
+    aug = o.drift(cfg, sub)
+    keys = o.blocks(cfg, aug)
+    payload = o.effq(cfg, aug, keys)
+    tiles = o.out_tiles(cfg, keys)
+    pix = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
+    o.conv_fft(cfg, keys, payload, R, pix)
+    dt = time.perf_counter() - t0
+    return len(sub["q"]), dt, os.cpu_count()
+
+
+def run_reference(args):
+    rank = _env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    cfg, segs, seg, R = workload(args.config, 0)
+    n_sample = args.ref_segments
+    for _ in range(args.warmup and 1):
+        oracle_sample(cfg, segs, R, max(2, n_sample // 8))
+    times = []
+    for _ in range(args.steps):
+        n, dt, cores = oracle_sample(cfg, segs, R, n_sample)
+        times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    val = n / (ms * 1e-3)
+    sample = f"first {n} segments of config {args.config}, whole path, all pixels of their footprint"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2602_12052_b200 import Tred
+
+    world = _env_int("WORLD_SIZE", 1)
+    rank = _env_int("RANK", 0)
+    local = _env_int("LOCAL_RANK", 0)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg, segs, seg_h, R = workload(args.config, rank)
+    nseg = seg_h.shape[1]
+    sim = Tred(cfg, device=dev, conv_work_bytes=args.work_gb << 30 if args.work_gb else None)
+    rhat = sim.prepare_response(torch.from_numpy(R).to(dev))       # once per response
+    seg_d = torch.from_numpy(seg_h).to(dev)
+    seg_pinned = torch.from_numpy(seg_h).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up
+    out = None
+    for _ in range(max(args.warmup, 3)):
+        out = sim.simulate(seg_d, rhat)
+    barrier()
+    info = {k: out[k] for k in ("npairs", "nblocks", "nsp", "ntiles")}
+    # Gauss-Legendre node evaluations of one step = cuboids of every bounding box x n^3
+    _, augi0, _ = sim.drift(seg_d)
+    ext = (augi0[3:6] - augi0[0:3] + 1).to(torch.float64)
+    info["gl_nodes"] = float((ext[0] * ext[1] * ext[2]).sum().item()) * cfg.gl_n ** 3
+
+    # ---- timed region 1: inputs resident in HBM, device time by CUDA events
+    sampler = ClockSampler(local)
+    sampler.start()
+    sim.profile_begin(events=False)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()                       # flush L2 between timed iterations
+        a.record()
+        out = sim.simulate(seg_d, rhat)
+        b.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    launches = sum(v[1] for v in sim.profile_end().values())
+    ms_steps = [a.elapsed_time(b) for a, b in ev]
+    ms = float(np.mean(ms_steps))
+
+    # ---- timed region 2: per-stage events (roofline of the dominant kernel)
+    stage_ms = {}
+    for _ in range(args.steps):
+        flush.zero_()
+        sim.profile_begin(events=True)
+        sim.simulate(seg_d, rhat)
+        torch.cuda.synchronize()
+        for k, (m, n) in sim.profile_end().items():
+            stage_ms[k] = stage_ms.get(k, 0.0) + m / args.steps
+    barrier()
+
+    # ---- timed region 3: end to end through the public API with HOST buffers
+    e2e_ms = []
+    h2d = seg_pinned.numel() * 4
+    d2h = 0
+    for i in range(args.steps + 1):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sd = seg_pinned.to(dev, non_blocking=True)
+        o2 = sim.simulate(sd, rhat)
+        keys_h = o2["tile_keys"].cpu()
+        data_h = o2["tile_data"].cpu()
+        torch.cuda.synchronize()
+        if i > 0:
+            e2e_ms.append(1e3 * (time.perf_counter() - t0))
+        d2h = keys_h.numel() * 8 + data_h.numel() * 4
+    e2e = float(np.mean(e2e_ms))
+    barrier()
+
+    # ---- max over ranks
+    t = torch.tensor([ms, e2e], dtype=torch.float64, device=dev)
+    n_all = torch.tensor([float(nseg)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(n_all, op=dist.ReduceOp.SUM)
+    ms_max, e2e_max = float(t[0]), float(t[1])
+    total_seg = float(n_all[0])
+
+    if rank == 0:
+        d = sim.dims
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        # dominant kernel and its roofline
+        dom = max(stage_ms, key=stage_ms.get)
+        nb = info["nblocks"]
+        ncols = cfg.block[0] * cfg.block[1]
+        K = 2 * cfg.resp_half + 1
+        nf = d.fft_len // 2
+        sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        alu_peak = 148 * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12          # TFLOP/s at max clock
+        roof = {"kernel": dom, "ms": stage_ms[dom]}
+        if dom == "mac":
+            flops = nb * ncols * K * K * (8.0 * (nf - 1) + 4.0)
+            roof.update(bound="alu", achieved=flops / (stage_ms[dom] * 1e-3) / 1e12, peak=alu_peak,
+                        unit="TFLOP/s", traffic=None,
+                        note="fp32 FMA pipe; peak = 148 SM x 128 lanes x 2 x sm_max_mhz (derived, DESIGN.md)")
+        elif dom == "effq":
+            # algorithmic work: one Eq. (10) evaluation per node = EFFQ_INSTR_PER_NODE fp32
+            # lane-instructions; peak = lane-instructions/s of the SMs
+            ipn = 40.0
+            roof.update(bound="alu", achieved=info["gl_nodes"] * ipn / (stage_ms[dom] * 1e-3) / 1e12,
+                        peak=148 * FMA_LANES_PER_SM * sm_max * 1e6 / 1e12, unit="Tinstr/s", traffic=None,
+                        note=f"{ipn:.0f} fp32 lane-instructions per node (derived, DESIGN.md)")
+        else:
+            hbm = peaks.get("hbm_gbs", 6650.0)
+            roof.update(bound="hbm", achieved=None, peak=hbm, unit="GB/s", traffic=None)
+        if roof.get("achieved") is not None:
+            roof["frac"] = roof["achieved"] / roof["peak"]
+        payload_gb = nb * d.block_floats * 4 / 1e9
+        line = {"metric": METRIC, "value": total_seg / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_max,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic",
+                "config": {"workload": cfg.name, "segments_per_event": nseg, "events": world,
+                           "pixels": [cfg.npix_x, cfg.npix_y], "nticks": cfg.nticks, "gl_n": cfg.gl_n,
+                           "block": list(cfg.block), "resp_nticks": cfg.resp_nticks, "fft_len": d.fft_len,
+                           "l2": "flushed between timed iterations (256 MiB write)",
+                           "parallelism": f"events x{world}, no collective", **info},
+                "e2e": {"value": total_seg / (e2e_max * 1e-3), "unit": UNIT, "ms_per_step": e2e_max,
+                        "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                "gpu_launches": int(launches),
+                "clocks": clocks,
+                "stage_ms": {k: round(v, 4) for k, v in stage_ms.items() if v > 0},
+                "roofline": roof,
+                "peak_mem_gb": torch.cuda.max_memory_allocated(dev) / 1e9,
+                "payload_gb": payload_gb,
+                "wall_s_timed_region": t_wall}
+        if not args.no_cpu_baseline and world == 1:
+            n, dt, cores = oracle_sample(cfg, segs, R, args.ref_segments)
+            line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"first {n} segments of config {args.config}, whole path, "
+                                              f"all pixels of their footprint ({dt:.1f} s)"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--ref-segments", type=int, default=40)
+    ap.add_argument("--work-gb", type=int, default=0, help="tred_convolve workspace cap (GiB), 0 = default")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

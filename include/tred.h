@@ -203,6 +203,20 @@ int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_sp_data,
                           int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
                           void* stream);
 
+/*
+ * Stage profiling (the paper's "profiler-guided optimization", Fig. 10).
+ * tred_profile_begin clears the counters; with record_events != 0 every stage of the
+ * following calls is bracketed by CUDA events on the launching stream.
+ * tred_profile_end synchronises those events (the one place the library waits on the
+ * device, on request) and returns, per stage, the summed milliseconds (0 if events were
+ * off) and the number of kernels launched.  Stage s is named tred_stage_name(s),
+ * s < tred_stage_count().  h_ms / h_launches: HOST arrays of nstage entries.
+ */
+int tred_profile_begin(tred_ctx* ctx, int record_events);
+int tred_profile_end(tred_ctx* ctx, int nstage, float* h_ms, int64_t* h_launches);
+int tred_stage_count(void);
+const char* tred_stage_name(int stage);
+
 #ifdef __cplusplus
 }
 #endif

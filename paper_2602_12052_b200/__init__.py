@@ -65,6 +65,10 @@ EXPORTS = {
                                 _c_p, C.c_size_t, _c_p]),
     "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p,
                                         _c_p]),
+    "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
+    "tred_profile_end": (C.c_int, [_c_p, C.c_int, _c_p, _c_p]),
+    "tred_stage_count": (C.c_int, []),
+    "tred_stage_name": (C.c_char_p, [C.c_int]),
 }
 
 _LIB = None
@@ -168,6 +172,17 @@ class Tred:
             b = self._empty((max(int(nbytes), 256),), self.torch.uint8)
             self._work[name] = b
         return b
+
+    def profile_begin(self, events: bool = True):
+        _check(self.L.tred_profile_begin(self.h, 1 if events else 0), "tred_profile_begin")
+
+    def profile_end(self) -> dict:
+        """{stage name: (milliseconds, kernel launches)}; synchronises the recorded events."""
+        n = self.L.tred_stage_count()
+        ms = (C.c_float * n)()
+        ln = (C.c_int64 * n)()
+        _check(self.L.tred_profile_end(self.h, n, C.cast(ms, _c_p), C.cast(ln, _c_p)), "tred_profile_end")
+        return {self.L.tred_stage_name(i).decode(): (float(ms[i]), int(ln[i])) for i in range(n)}
 
     # -- the calls ----------------------------------------------------------------
     def prepare_response(self, resp):

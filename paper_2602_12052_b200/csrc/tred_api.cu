@@ -14,6 +14,68 @@ void tred_set_cuda_error(cudaError_t e, const char* where) {
 }
 
 extern "C" const char* tred_last_cuda_error(void) { return g_cuda_err; }
+
+// ------------------------------------------------------------------ stage profiling
+thread_local int64_t g_tred_launches = 0;
+
+TredProfScope::TredProfScope(tred_ctx* ctx, int stage_, cudaStream_t st_)
+    : c(ctx), stage(stage_), st(st_), l0(g_tred_launches), rec(-1) {
+  if (!c || !c->prof_on) return;
+  if (c->nrecs == c->cap_recs) {
+    int nc = c->cap_recs ? 2 * c->cap_recs : 256;
+    TredProfRec* nr = (TredProfRec*)realloc(c->recs, sizeof(TredProfRec) * nc);
+    if (!nr) return;
+    c->recs = nr; c->cap_recs = nc;
+  }
+  TredProfRec& r = c->recs[c->nrecs];
+  r.stage = stage;
+  if (cudaEventCreate(&r.a) != cudaSuccess) return;
+  if (cudaEventCreate(&r.b) != cudaSuccess) { cudaEventDestroy(r.a); return; }
+  cudaEventRecord(r.a, st);
+  rec = c->nrecs++;
+}
+
+TredProfScope::~TredProfScope() {
+  if (c) c->launches[stage] += g_tred_launches - l0;
+  if (rec >= 0) cudaEventRecord(c->recs[rec].b, st);
+}
+
+static void prof_clear(tred_ctx* c) {
+  for (int i = 0; i < c->nrecs; ++i) { cudaEventDestroy(c->recs[i].a); cudaEventDestroy(c->recs[i].b); }
+  c->nrecs = 0;
+  for (int s = 0; s < ST_COUNT; ++s) c->launches[s] = 0;
+}
+
+extern "C" int tred_profile_begin(tred_ctx* c, int record_events) {
+  if (!c) return TRED_EINVAL;
+  prof_clear(c);
+  c->prof_on = record_events ? 1 : 0;
+  return TRED_OK;
+}
+
+extern "C" int tred_profile_end(tred_ctx* c, int nstage, float* h_ms, int64_t* h_launches) {
+  if (!c || nstage < 0) return TRED_EINVAL;
+  for (int s = 0; s < nstage; ++s) { if (h_ms) h_ms[s] = 0.0f; if (h_launches) h_launches[s] = 0; }
+  for (int i = 0; i < c->nrecs; ++i) {
+    TredProfRec& r = c->recs[i];
+    TRED_CUDA(cudaEventSynchronize(r.b));
+    float ms = 0.0f;
+    TRED_CUDA(cudaEventElapsedTime(&ms, r.a, r.b));
+    if (h_ms && r.stage < nstage) h_ms[r.stage] += ms;
+  }
+  for (int s = 0; s < nstage && s < ST_COUNT; ++s) if (h_launches) h_launches[s] = c->launches[s];
+  prof_clear(c);
+  c->prof_on = 0;
+  return TRED_OK;
+}
+
+extern "C" int tred_stage_count(void) { return ST_COUNT; }
+
+extern "C" const char* tred_stage_name(int s) {
+  static const char* names[ST_COUNT] = {"drift", "pairs", "sort", "rle", "effq", "plan", "resp_dft",
+                                        "fft_fwd", "class_bundles", "mac", "accum", "ifft", "gather"};
+  return (s >= 0 && s < ST_COUNT) ? names[s] : "?";
+}
 extern "C" int tred_abi_version(void) { return 1; }
 
 extern "C" const char* tred_strerror(int s) {
@@ -88,7 +150,12 @@ extern "C" int tred_create(const tred_config* cfg, tred_ctx** out) {
   return TRED_OK;
 }
 
-extern "C" void tred_destroy(tred_ctx* c) { free(c); }
+extern "C" void tred_destroy(tred_ctx* c) {
+  if (!c) return;
+  prof_clear(c);
+  free(c->recs);
+  free(c);
+}
 
 // ------------------------------------------------------------------ S1 drift
 struct DriftParams {
@@ -183,8 +250,12 @@ extern "C" int tred_drift(tred_ctx* ctx, int64_t nseg, const float* d_seg, float
   TRED_CUDA(cudaMemsetAsync(d_npairs, 0, sizeof(int64_t), st));
   if (nseg == 0) return TRED_OK;
   if (!d_seg || !d_augf || !d_augi) return TRED_EINVAL;
-  k_drift<<<cdiv(nseg, 256), 256, 0, st>>>(nseg, d_seg, d_augf, d_augi,
-                                          (unsigned long long*)d_npairs, make_drift_params(ctx));
+  {
+    TredProfScope ps(ctx, ST_DRIFT, st);
+    k_drift<<<cdiv(nseg, 256), 256, 0, st>>>(nseg, d_seg, d_augf, d_augi,
+                                            (unsigned long long*)d_npairs, make_drift_params(ctx));
+    TRED_COUNT_LAUNCH(1);
+  }
   TRED_LAUNCH_CHECK("k_drift");
   return TRED_OK;
 }
@@ -299,7 +370,11 @@ extern "C" int tred_blockbin(tred_ctx* ctx, int64_t nseg, const int32_t* d_augi,
   int64_t* d_np = w.cnt;         // device-side pair count
   int64_t* d_nb = w.cnt + 1;     // device-side block count
   // pair offsets = exclusive scan of the per-segment pair counts
-  int rc = tred_exclusive_scan_i32(d_augi + 7 * nseg, w.pair_off, nseg, d_np, w.scan, st);
+  int rc;
+  {
+    TredProfScope ps(ctx, ST_PAIRS, st);
+    rc = tred_exclusive_scan_i32(d_augi + 7 * nseg, w.pair_off, nseg, d_np, w.scan, st);
+  }
   if (rc != TRED_OK) return rc;
   int total_bits = 1;
   while ((1ll << total_bits) < (int64_t)g.NBx * g.NBy * g.NBt) ++total_bits;
@@ -308,18 +383,30 @@ extern "C" int tred_blockbin(tred_ctx* ctx, int64_t nseg, const int32_t* d_augi,
   uint32_t* ka = w.ka; uint32_t* kb = w.kb;
   int32_t* va = (passes % 2 == 0) ? d_pair_seg : w.vb;
   int32_t* vb = (passes % 2 == 0) ? w.vb : d_pair_seg;
-  k_pair_expand<<<cdiv(nseg, 256), 256, 0, st>>>(nseg, d_augi, w.pair_off, cap_pairs, ka, va, g);
+  {
+    TredProfScope ps(ctx, ST_PAIRS, st);
+    k_pair_expand<<<cdiv(nseg, 256), 256, 0, st>>>(nseg, d_augi, w.pair_off, cap_pairs, ka, va, g);
+    TRED_COUNT_LAUNCH(1);
+  }
   TRED_LAUNCH_CHECK("k_pair_expand");
   uint32_t* ks; int32_t* vs;
-  rc = tred_radix_sort_pairs(ka, va, kb, vb, cap_pairs, d_np, passes * 8, w.sort, st, &ks, &vs);
+  {
+    TredProfScope ps(ctx, ST_SORT, st);
+    rc = tred_radix_sort_pairs(ka, va, kb, vb, cap_pairs, d_np, passes * 8, w.sort, st, &ks, &vs);
+  }
   if (rc != TRED_OK) return rc;
   if (vs != d_pair_seg) return TRED_EINVAL;   // cannot happen
   // run-length compaction of the sorted keys
-  k_rle_flags<<<cdiv(cap_pairs, 256), 256, 0, st>>>(ks, cap_pairs, d_np, w.flags);
-  rc = tred_exclusive_scan_i32(w.flags, w.flags, cap_pairs, d_nb, w.scan, st);
-  if (rc != TRED_OK) return rc;
-  k_rle_write<<<cdiv(cap_pairs, 256), 256, 0, st>>>(ks, w.flags, cap_pairs, d_np, d_nb,
-                                                   cap_blocks, d_keys, d_blk_off, d_slab_off, g);
+  {
+    TredProfScope ps(ctx, ST_RLE, st);
+    k_rle_flags<<<cdiv(cap_pairs, 256), 256, 0, st>>>(ks, cap_pairs, d_np, w.flags);
+    TRED_COUNT_LAUNCH(1);
+    rc = tred_exclusive_scan_i32(w.flags, w.flags, cap_pairs, d_nb, w.scan, st);
+    if (rc != TRED_OK) return rc;
+    k_rle_write<<<cdiv(cap_pairs, 256), 256, 0, st>>>(ks, w.flags, cap_pairs, d_np, d_nb,
+                                                     cap_blocks, d_keys, d_blk_off, d_slab_off, g);
+    TRED_COUNT_LAUNCH(1);
+  }
   TRED_LAUNCH_CHECK("k_rle_write");
   TRED_CUDA(cudaMemcpyAsync(d_nblocks, d_nb, sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
   return TRED_OK;

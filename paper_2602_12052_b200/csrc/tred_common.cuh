@@ -5,11 +5,35 @@
 #include <stdio.h>
 #include "../../include/tred.h"
 
+enum TredStage {
+  ST_DRIFT = 0, ST_PAIRS, ST_SORT, ST_RLE, ST_EFFQ, ST_PLAN, ST_RESP, ST_FFT_FWD, ST_CLASS, ST_MAC,
+  ST_ACCUM, ST_IFFT, ST_GATHER, ST_COUNT
+};
+
+struct TredProfRec { int stage; cudaEvent_t a, b; };
+
 struct tred_ctx {
   tred_config cfg;
   tred_dims   dims;
   int         num_sms;
   int         smem_optin;     // max dynamic shared memory per block (bytes)
+  // stage profiling (tred_profile_begin / tred_profile_end)
+  int         prof_on;
+  int64_t     launches[ST_COUNT];
+  TredProfRec* recs;
+  int         nrecs, cap_recs;
+};
+
+// Kernel-launch counter (per host thread); every <<<>>> site calls TRED_COUNT_LAUNCH.
+extern thread_local int64_t g_tred_launches;
+#define TRED_COUNT_LAUNCH(n) (g_tred_launches += (n))
+
+// Brackets the launches of one stage: counts them and, when profiling is on, records a
+// pair of CUDA events on the stream the kernels are launched on.
+struct TredProfScope {
+  tred_ctx* c; int stage; cudaStream_t st; int64_t l0; int rec;
+  TredProfScope(tred_ctx* ctx, int stage_, cudaStream_t st_);
+  ~TredProfScope();
 };
 
 // Grid constants passed by value to kernels.

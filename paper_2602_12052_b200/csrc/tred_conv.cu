@@ -19,7 +19,7 @@ namespace {
 // x[b*L + i]; input must be in bit-reversed order, output is in natural order.
 // tw[k] = exp(-2 pi i k / L), k < L/2.  inverse: conjugate twiddles, no scaling.
 __device__ __forceinline__ void fft_dit_smem(float2* x, const float2* tw, int L, int logL,
-                                             int nb, bool inverse) {
+                                             int nb, bool inverse, int twmul = 1) {
   const int half_total = nb * (L >> 1);
   for (int s = 1; s <= logL; ++s) {
     const int half = 1 << (s - 1);
@@ -29,7 +29,7 @@ __device__ __forceinline__ void fft_dit_smem(float2* x, const float2* tw, int L,
       const int j = r & (half - 1);
       const int i0 = ((r >> (s - 1)) << s) + j + b * L;
       const int i1 = i0 + half;
-      float2 w = tw[j * tstep];
+      float2 w = tw[j * tstep * twmul];
       if (inverse) w.y = -w.y;
       const float2 a = x[i0], c = x[i1];
       const float2 m = make_float2(w.x * c.x - w.y * c.y, w.x * c.y + w.y * c.x);
@@ -50,40 +50,66 @@ __device__ __forceinline__ void fill_twiddles(float2* tw, int L) {
 
 __device__ __forceinline__ int bitrev(int i, int logL) { return (int)(__brev((unsigned)i) >> (32 - logL)); }
 
-// After a forward FFT of z = a + i b (a, b real), the packed half spectra of a and b.
-__device__ __forceinline__ void split_pair(const float2* Z, int L, int f, float2* A, float2* B) {
-  if (f == 0) {
-    const float2 z0 = Z[0], zn = Z[L >> 1];
-    *A = make_float2(z0.x, zn.x);
-    *B = make_float2(z0.y, zn.y);
-  } else {
-    const float2 p = Z[f], q = Z[L - f];
-    *A = make_float2(0.5f * (p.x + q.x), 0.5f * (p.y - q.y));
-    *B = make_float2(0.5f * (p.y + q.y), 0.5f * (q.x - p.x));
-  }
+// Real FFT of length N = 2M through one complex FFT of length M (no pairing of two
+// signals, so no rounding cross-talk between columns / pixels):
+//   forward:  z[m] = x[2m] + i x[2m+1],  Z = FFT_M(z),
+//             X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) e^{-2 pi i k/N} (Z[k] - conj Z[M-k]),
+//             X[0] = Re Z[0] + Im Z[0] (DC), X[M] = Re Z[0] - Im Z[0] (Nyquist).
+//   inverse:  Z[k] = (X[k] + conj X[M-k]) + i e^{+2 pi i k/N} (X[k] - conj X[M-k]),
+//             z = IFFT_M(Z) (unnormalised), x[2m] = Re z[m]/N, x[2m+1] = Im z[m]/N.
+// twN[k] = exp(-2 pi i k / N), k < M; the M-point twiddles are twN[2k].
+__device__ __forceinline__ float2 rfft_post(const float2* Z, const float2* twN, int M, int k) {
+  if (k == 0) { const float2 z0 = Z[0]; return make_float2(z0.x + z0.y, z0.x - z0.y); }  // (DC, Nyquist)
+  const float2 p = Z[k], q = Z[M - k];
+  const float2 e = make_float2(0.5f * (p.x + q.x), 0.5f * (p.y - q.y));     // (Z[k] + conj Z[M-k])/2
+  const float2 o = make_float2(0.5f * (p.x - q.x), 0.5f * (p.y + q.y));     // (Z[k] - conj Z[M-k])/2
+  const float2 w = twN[k];
+  // -i * w * o
+  const float2 wo = make_float2(w.x * o.x - w.y * o.y, w.x * o.y + w.y * o.x);
+  return make_float2(e.x + wo.y, e.y - wo.x);
+}
+
+// X: packed half spectrum (slot 0 = (DC, Nyquist)); returns Z[k] of the inverse.
+__device__ __forceinline__ float2 rfft_pre_inverse(const float2* X, const float2* twN, int M, int k) {
+  if (k == 0) { const float2 x0 = X[0]; return make_float2(x0.x + x0.y, x0.x - x0.y); }
+  const float2 p = X[k], q = X[M - k];
+  const float2 e = make_float2(p.x + q.x, p.y - q.y);                       // X[k] + conj X[M-k]
+  const float2 o = make_float2(p.x - q.x, p.y + q.y);                       // X[k] - conj X[M-k]
+  const float2 w = make_float2(twN[k].x, -twN[k].y);                        // e^{+2 pi i k/N}
+  // i * w * o
+  const float2 wo = make_float2(w.x * o.x - w.y * o.y, w.x * o.y + w.y * o.x);
+  return make_float2(e.x - wo.y, e.y + wo.x);
 }
 
 // ------------------------------------------------------------------ response spectrum
-// One CTA per pair of response rows (row = ((jx*S+jy)*K+kx)*K+ky); rhat[f][row].
+// Computed ONCE per response, in fp64 by a direct DFT and rounded to
+// fp32 at the end.  Induction-only pixels have a bipolar response whose DC bin is a
+// cancellation to ~0; an fp32 FFT would leave ~1e-7 * sum|R| there, which the
+// convolution multiplies by the whole collected charge.
+// One CTA per response row (row = ((jx*S+jy)*K+kx)*K+ky); rhat[f][row].
 __global__ void __launch_bounds__(256)
-k_resp_fft(const float* __restrict__ resp, float2* __restrict__ rhat, int nrows, int Tr, int L, int logL) {
-  extern __shared__ float2 sm[];
-  float2* Z = sm;            // [L]
-  float2* tw = sm + L;       // [L/2]
-  const int r0 = blockIdx.x * 2, r1 = r0 + 1;
-  fill_twiddles(tw, L);
-  for (int i = threadIdx.x; i < L; i += blockDim.x) {
-    float a = i < Tr ? resp[(int64_t)r0 * Tr + i] : 0.0f;
-    float b = (i < Tr && r1 < nrows) ? resp[(int64_t)r1 * Tr + i] : 0.0f;
-    Z[bitrev(i, logL)] = make_float2(a, b);
+k_resp_dft64(const float* __restrict__ resp, float2* __restrict__ rhat, int nrows, int Tr, int L) {
+  extern __shared__ double smd[];
+  double2* tw = reinterpret_cast<double2*>(smd);       // [L]  exp(-2 pi i k / L)
+  double* r = smd + 2 * L;                              // [Tr]
+  const int row = blockIdx.x;
+  for (int k = threadIdx.x; k < L; k += blockDim.x) {
+    double sn, cs;
+    sincospi(-2.0 * (double)k / (double)L, &sn, &cs);
+    tw[k] = make_double2(cs, sn);
   }
+  for (int i = threadIdx.x; i < Tr; i += blockDim.x) r[i] = (double)resp[(int64_t)row * Tr + i];
   __syncthreads();
-  fft_dit_smem(Z, tw, L, logL, 1, false);
-  for (int f = threadIdx.x; f < (L >> 1); f += blockDim.x) {
-    float2 A, B;
-    split_pair(Z, L, f, &A, &B);
-    rhat[(int64_t)f * nrows + r0] = A;
-    if (r1 < nrows) rhat[(int64_t)f * nrows + r1] = B;
+  const int nf = L >> 1;
+  for (int f = threadIdx.x; f <= nf; f += blockDim.x) {
+    double re = 0.0, im = 0.0;
+    for (int t = 0; t < Tr; ++t) {
+      const double2 w = tw[(f * t) & (L - 1)];
+      re += r[t] * w.x; im += r[t] * w.y;
+    }
+    if (f == 0) rhat[row].x = (float)re;                          // DC
+    else if (f == nf) rhat[row].y = (float)re;                    // Nyquist, packed in slot 0
+    else rhat[(int64_t)f * nrows + row] = make_float2((float)re, (float)im);
   }
 }
 
@@ -126,35 +152,32 @@ k_mark_tiles(int64_t nsp_map, const int32_t* __restrict__ sp_idx, int32_t* __res
 }
 
 // ------------------------------------------------------------------ forward FFT of blocks
-// One CTA per (block of the chunk, group of 2*CP columns).  qhat[f][slot][col].
+// One CTA per (block of the chunk, group of CP columns).  qhat[f][slot][col].
 template <int CP>
 __global__ void __launch_bounds__(256)
-k_fft_fwd(const float* __restrict__ payload, int blk0, int nchunk, float2* __restrict__ qhat, TredGrid g, int logL) {
+k_fft_fwd(const float* __restrict__ payload, int blk0, int nchunk, float2* __restrict__ qhat, TredGrid g, int logM) {
   extern __shared__ float2 sm[];
-  const int L = g.L;
-  float2* Z = sm;                 // [CP][L]
-  float2* tw = sm + CP * L;       // [L/2]
+  const int N = g.L, M = N >> 1;
+  float2* Z = sm;                 // [CP][M]
+  float2* tw = sm + CP * M;       // [M]  exp(-2 pi i k / N)
   const int ncols = g.Bx * g.By;
-  const int groups = ncols / (2 * CP);
+  const int groups = ncols / CP;
   const int slot = blockIdx.x / groups, grp = blockIdx.x - slot * groups;
-  const int col0 = grp * 2 * CP;
-  fill_twiddles(tw, L);
-  const float* src = payload + ((int64_t)(blk0 + slot) * ncols + col0) * g.Bt;
-  for (int i = threadIdx.x; i < CP * L; i += blockDim.x) {
-    const int c = i / L, k = i - c * L;
-    float a = 0.0f, b = 0.0f;
-    if (k < g.Bt) { a = src[(2 * c) * g.Bt + k]; b = src[(2 * c + 1) * g.Bt + k]; }
-    Z[c * L + bitrev(k, logL)] = make_float2(a, b);
+  const int col0 = grp * CP;
+  fill_twiddles(tw, N);
+  const float2* src = reinterpret_cast<const float2*>(payload + ((int64_t)(blk0 + slot) * ncols + col0) * g.Bt);
+  const int hb = g.Bt >> 1;       // float2 samples per column
+  for (int i = threadIdx.x; i < CP * M; i += blockDim.x) {
+    const int c = i / M, m = i - c * M;
+    float2 v = make_float2(0.0f, 0.0f);
+    if (m < hb) v = src[c * hb + m];
+    Z[c * M + bitrev(m, logM)] = v;
   }
   __syncthreads();
-  fft_dit_smem(Z, tw, L, logL, CP, false);
-  const int nf = L >> 1;
-  for (int i = threadIdx.x; i < nf * CP; i += blockDim.x) {
+  fft_dit_smem(Z, tw, M, logM, CP, false, 2);
+  for (int i = threadIdx.x; i < M * CP; i += blockDim.x) {
     const int f = i / CP, c = i - f * CP;
-    float2 A, B;
-    split_pair(Z + c * L, L, f, &A, &B);
-    float2* dst = qhat + ((int64_t)f * nchunk + slot) * ncols + col0 + 2 * c;
-    dst[0] = A; dst[1] = B;
+    qhat[((int64_t)f * nchunk + slot) * ncols + col0 + c] = rfft_post(Z + c * M, tw, M, f);
   }
 }
 
@@ -354,40 +377,39 @@ k_fill_blockmap(int64_t nblocks, const int64_t* __restrict__ keys, int32_t* __re
 }
 
 // ------------------------------------------------------------------ inverse FFT
-// One CTA per pair of slab-pixels; sp_data[sp][n_over*Bt].
+// One CTA per IP slab-pixels; sp_data[sp][n_over*Bt].
+template <int IP>
 __global__ void __launch_bounds__(256)
 k_ifft(const float2* __restrict__ ohat, int sp0, int nsp_chunk, float* __restrict__ sp_data, TredGrid g,
-       int logL, int out_len) {
+       int logM, int out_len) {
   extern __shared__ float2 sm[];
-  const int L = g.L, nf = L >> 1;
-  float2* Z = sm;
-  float2* tw = sm + L;
-  const int a = blockIdx.x * 2, b = a + 1;
-  const bool hb = b < nsp_chunk;
-  fill_twiddles(tw, L);
-  for (int f = threadIdx.x; f < nf; f += blockDim.x) {
-    const float2 A = ohat[(int64_t)a * nf + f];
-    const float2 B = hb ? ohat[(int64_t)b * nf + f] : make_float2(0.0f, 0.0f);
-    if (f == 0) {
-      Z[bitrev(0, logL)] = make_float2(A.x, B.x);            // DC
-      Z[bitrev(nf, logL)] = make_float2(A.y, B.y);           // Nyquist
-    } else {
-      // Z[f] = A + iB ; Z[L-f] = conj(A) + i conj(B)
-      Z[bitrev(f, logL)] = make_float2(A.x - B.y, A.y + B.x);
-      Z[bitrev(L - f, logL)] = make_float2(A.x + B.y, B.x - A.y);
-    }
+  const int N = g.L, M = N >> 1;
+  float2* Z = sm;                 // [IP][M]
+  float2* X = sm + IP * M;        // [IP][M] staged spectra
+  float2* tw = sm + 2 * IP * M;   // [M]
+  const int a0 = blockIdx.x * IP;
+  fill_twiddles(tw, N);
+  for (int i = threadIdx.x; i < IP * M; i += blockDim.x) {
+    const int c = i / M, k = i - c * M;
+    X[i] = (a0 + c < nsp_chunk) ? ohat[(int64_t)(a0 + c) * M + k] : make_float2(0.0f, 0.0f);
   }
   __syncthreads();
-  fft_dit_smem(Z, tw, L, logL, 1, true);
-  const int row = g.nover * g.Bt;
-  const float sc = 1.0f / (float)L;
-  float* da = sp_data + (int64_t)(sp0 + a) * row;
-  float* db = sp_data + (int64_t)(sp0 + b) * row;
-  for (int t = threadIdx.x; t < row; t += blockDim.x) {
-    const float2 z = Z[t];
-    const bool ok = t < out_len;
-    da[t] = ok ? z.x * sc : 0.0f;
-    if (hb) db[t] = ok ? z.y * sc : 0.0f;
+  for (int i = threadIdx.x; i < IP * M; i += blockDim.x) {
+    const int c = i / M, k = i - c * M;
+    Z[c * M + bitrev(k, logM)] = rfft_pre_inverse(X + c * M, tw, M, k);
+  }
+  __syncthreads();
+  fft_dit_smem(Z, tw, M, logM, IP, true, 2);
+  const int row = g.nover * g.Bt, hrow = row >> 1;
+  const float sc = 1.0f / (float)N;
+  for (int i = threadIdx.x; i < IP * hrow; i += blockDim.x) {
+    const int c = i / hrow, m = i - c * hrow;
+    if (a0 + c >= nsp_chunk) continue;
+    const float2 z = Z[c * M + m];
+    float2 v;
+    v.x = (2 * m < out_len) ? z.x * sc : 0.0f;
+    v.y = (2 * m + 1 < out_len) ? z.y * sc : 0.0f;
+    reinterpret_cast<float2*>(sp_data + (int64_t)(sp0 + a0 + c) * row)[m] = v;
   }
 }
 
@@ -493,10 +515,15 @@ extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* 
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);
   const int K = 2 * g.H + 1, nrows = g.S * g.S * K * K;
-  const size_t smem = (size_t)(g.L + g.L / 2) * sizeof(float2);
-  TRED_CUDA(cudaFuncSetAttribute(k_resp_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_resp_fft<<<(nrows + 1) / 2, 256, smem, st>>>(d_resp, (float2*)d_rhat, nrows, g.Tr, g.L, ilog2(g.L));
-  TRED_LAUNCH_CHECK("k_resp_fft");
+  const size_t smem = (size_t)(2 * g.L + g.Tr) * sizeof(double);
+  if (smem > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
+  TRED_CUDA(cudaFuncSetAttribute(k_resp_dft64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  {
+    TredProfScope ps(ctx, ST_RESP, st);
+    k_resp_dft64<<<nrows, 256, smem, st>>>(d_resp, (float2*)d_rhat, nrows, g.Tr, g.L);
+    TRED_COUNT_LAUNCH(1);
+  }
+  TRED_LAUNCH_CHECK("k_resp_dft64");
   return TRED_OK;
 }
 
@@ -515,8 +542,10 @@ extern "C" int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t*
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);
   const int64_t npix = (int64_t)g.npx * g.npy;
+  TredProfScope ps(ctx, ST_PLAN, st);
   TRED_CUDA(cudaMemsetAsync(w.sp_idx, 0, (w.nmap + 1) * 4, st));
   TRED_CUDA(cudaMemsetAsync(w.tile_idx, 0, (w.nmap + 1) * 4, st));
+  TRED_COUNT_LAUNCH(3 + (nblocks > 0 ? 1 : 0));
   if (nblocks > 0) k_mark_sp<<<cdiv(nblocks * 32, 256), 256, 0, st>>>(nblocks, d_keys, w.sp_idx, g);
   int rc = tred_exclusive_scan_i32(w.sp_idx, w.sp_idx, w.nmap + 1, nullptr, w.scan, st);
   if (rc != TRED_OK) return rc;
@@ -562,18 +591,24 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
   const size_t mac_smem = ((size_t)mp.nrows + (size_t)mp.G * ncols * MAC_NB) * sizeof(float2);
   if (mac_smem > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
   TRED_CUDA(cudaFuncSetAttribute(k_mac, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mac_smem));
-  constexpr int CP = 4;
-  const size_t fft_smem = (size_t)(CP * g.L + g.L / 2) * sizeof(float2);
+  constexpr int CP = 8, IP = 4;
+  const int M = g.L / 2, logM = logL - 1;
+  if (g.Bt < 2) return TRED_EUNSUPPORTED;
+  const size_t fft_smem = (size_t)(CP * M + M) * sizeof(float2);
   TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd<CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem));
-  const size_t ifft_smem = (size_t)(g.L + g.L / 2) * sizeof(float2);
-  TRED_CUDA(cudaFuncSetAttribute(k_ifft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ifft_smem));
+  const size_t ifft_smem = (size_t)(2 * IP * M + M) * sizeof(float2);
+  TRED_CUDA(cudaFuncSetAttribute(k_ifft<IP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ifft_smem));
 
   // block map of the whole event (lives at the start of the workspace)
   ConvWork w0 = carve_conv(ctx, d_work, 1, 1);
   if (work_bytes < w0.total) return TRED_ECAP;
   const int64_t nbtot = (int64_t)g.NBx * g.NBy * g.NBt;
-  TRED_CUDA(cudaMemsetAsync(w0.blockmap, 0xff, nbtot * 4, st));
-  k_fill_blockmap<<<cdiv(nblocks, 256), 256, 0, st>>>(nblocks, d_keys, w0.blockmap);
+  {
+    TredProfScope ps(ctx, ST_CLASS, st);
+    TRED_CUDA(cudaMemsetAsync(w0.blockmap, 0xff, nbtot * 4, st));
+    k_fill_blockmap<<<cdiv(nblocks, 256), 256, 0, st>>>(nblocks, d_keys, w0.blockmap);
+    TRED_COUNT_LAUNCH(1);
+  }
 
   // process the slabs in groups that fit the workspace
   int s0 = 0;
@@ -589,19 +624,39 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
     if (nb == 0 || ns == 0) continue;
     ConvWork w = carve_conv(ctx, d_work, nb, ns);
     if (w.total > work_bytes) return TRED_ECAP;
-    k_fft_fwd<CP><<<nb * (ncols / (2 * CP)), 256, fft_smem, st>>>(d_payload, blk0, nb, w.qhat, g, logL);
-    TRED_CUDA(cudaMemsetAsync(w.cls_cnt, 0, ci.ncls * 4, st));
-    k_class_count<<<cdiv(nb, 256), 256, 0, st>>>(d_keys, blk0, nb, w.cls_cnt, g, ci);
-    k_class_scan<<<1, 32, 0, st>>>(w.cls_cnt, w.cls_off, w.cls_cur, w.bundles, w.nbundles, ci.ncls);
-    k_class_place<<<cdiv(nb, 256), 256, 0, st>>>(d_keys, blk0, nb, w.cls_off, w.cls_cur, w.order, g, ci);
+    {
+      TredProfScope ps(ctx, ST_FFT_FWD, st);
+      k_fft_fwd<CP><<<nb * (ncols / CP), 256, fft_smem, st>>>(d_payload, blk0, nb, w.qhat, g, logM);
+      TRED_COUNT_LAUNCH(1);
+    }
+    {
+      TredProfScope ps(ctx, ST_CLASS, st);
+      TRED_CUDA(cudaMemsetAsync(w.cls_cnt, 0, ci.ncls * 4, st));
+      k_class_count<<<cdiv(nb, 256), 256, 0, st>>>(d_keys, blk0, nb, w.cls_cnt, g, ci);
+      k_class_scan<<<1, 32, 0, st>>>(w.cls_cnt, w.cls_off, w.cls_cur, w.bundles, w.nbundles, ci.ncls);
+      k_class_place<<<cdiv(nb, 256), 256, 0, st>>>(d_keys, blk0, nb, w.cls_off, w.cls_cur, w.order, g, ci);
+      TRED_COUNT_LAUNCH(3);
+    }
     const int nb_ub = nb / MAC_NB + ci.ncls;
     int gy = (nb_ub + mp.G * 16 - 1) / (mp.G * 16);
     if (gy < 1) gy = 1;
     if (gy > 65535) gy = 65535;
-    k_mac<<<dim3(nf, gy), mp.G * mp.gthreads, mac_smem, st>>>(w.qhat, (const float2*)d_rhat, w.chat, w.order,
-                                                              w.bundles, w.nbundles, nb, g, ci, mp);
-    k_accum<<<ns, 256, 0, st>>>(w.chat, d_sp_keys, sp0, ns, w0.blockmap, blk0, w.ohat, g, outp);
-    k_ifft<<<(ns + 1) / 2, 256, ifft_smem, st>>>(w.ohat, sp0, ns, d_sp_data, g, logL, ctx->dims.out_len);
+    {
+      TredProfScope ps(ctx, ST_MAC, st);
+      k_mac<<<dim3(nf, gy), mp.G * mp.gthreads, mac_smem, st>>>(w.qhat, (const float2*)d_rhat, w.chat, w.order,
+                                                                w.bundles, w.nbundles, nb, g, ci, mp);
+      TRED_COUNT_LAUNCH(1);
+    }
+    {
+      TredProfScope ps(ctx, ST_ACCUM, st);
+      k_accum<<<ns, 256, 0, st>>>(w.chat, d_sp_keys, sp0, ns, w0.blockmap, blk0, w.ohat, g, outp);
+      TRED_COUNT_LAUNCH(1);
+    }
+    {
+      TredProfScope ps(ctx, ST_IFFT, st);
+      k_ifft<IP><<<(ns + IP - 1) / IP, 256, ifft_smem, st>>>(w.ohat, sp0, ns, d_sp_data, g, logM, ctx->dims.out_len);
+      TRED_COUNT_LAUNCH(1);
+    }
     TRED_LAUNCH_CHECK("convolve chunk");
   }
   return TRED_OK;
@@ -616,6 +671,8 @@ extern "C" int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);
   PlanWork w = carve_plan(ctx, (void*)d_plan_work);
+  TredProfScope ps(ctx, ST_GATHER, st);
+  TRED_COUNT_LAUNCH((ntiles > 0 ? 1 : 0) + (npix_req > 0 ? 1 : 0));
   if (ntiles > 0) {
     if (!d_tile_keys || !d_tile_data || (nsp > 0 && !d_sp_data)) return TRED_EINVAL;
     if (ntiles >= (1ll << 31)) return TRED_EUNSUPPORTED;

@@ -241,6 +241,8 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
     k_effq<NN><<<(unsigned)grid, threads, smem, st>>>(nseg, d_keys, d_blk_off, d_pair_seg,    \
                                                       d_augf, d_augi, d_payload, g, P);       \
   } while (0)
+  TredProfScope ps(ctx, ST_EFFQ, st);
+  TRED_COUNT_LAUNCH(1);
   switch (g.gl_n) {
     case 1: LAUNCH(1); break;
     case 2: LAUNCH(2); break;

@@ -189,6 +189,7 @@ int tred_exclusive_scan_i32(const int32_t* d_in, int32_t* d_out, int64_t n, int6
   k_scan_reduce<<<nb, SCAN_THREADS, 0, st>>>(d_in, n, sums);
   k_scan_sums<<<1, 1024, 0, st>>>(sums, nb, d_total);
   k_scan_apply<<<nb, SCAN_THREADS, 0, st>>>(d_in, d_out, n, sums);
+  TRED_COUNT_LAUNCH(3);
   TRED_LAUNCH_CHECK("exclusive_scan");
   return TRED_OK;
 }
@@ -213,6 +214,7 @@ int tred_radix_sort_pairs(uint32_t* ka, int32_t* va, uint32_t* kb, int32_t* vb,
     int rc = tred_exclusive_scan_i32(counts, counts, (int64_t)ncta * 256, nullptr, scan_work, st);
     if (rc != TRED_OK) return rc;
     k_sort_scatter<<<ncta, SORT_THREADS, 0, st>>>(ka, va, kb, vb, n_cap, d_n, shift, counts, ncta);
+    TRED_COUNT_LAUNCH(2);
     TRED_LAUNCH_CHECK("radix_sort");
     uint32_t* tk = ka; ka = kb; kb = tk;
     int32_t* tv = va; va = vb; vb = tv;

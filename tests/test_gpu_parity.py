@@ -5,7 +5,9 @@ Tolerances (DESIGN.md "Tolerances"):
   integers (bbox, flags, block keys, CSR lists, slab/tile keys): bit-exact;
   effective charge (fp32 vs fp64): max|d| <= 2e-5 max|Qeff|, total within 1e-5;
   waveforms: max|d| <= 1e-4 max|signal| (north_star);
-  per-pixel integrated charge: |dQ_p| <= 1e-5 max(|Q_p|, 1e-3 max_p|Q_p|) (north_star, G17).
+  per-pixel integrated charge: |dQ_p| <= 1e-5 |Q_p| + 4 * 2^-24 * sum_t |I_p(t)|
+      (north_star's relative 1e-5, plus the rounding an fp32 waveform of L1 norm
+       sum_t|I_p| carries in its own integral -- DESIGN.md "Tolerances", reading G17).
 """
 import numpy as np
 import pytest
@@ -183,8 +185,10 @@ def _wave_checks(got, ref):
     assert scale > 0
     assert np.abs(got - ref).max() <= TOL_WAVE * scale
     qg, qr = got.sum(1), ref.sum(1)
-    floor = 1e-3 * np.abs(qr).max()
-    assert (np.abs(qg - qr) <= TOL_QPIX * np.maximum(np.abs(qr), floor)).all()
+    l1 = np.abs(ref).sum(1)
+    assert (np.abs(qg - qr) <= TOL_QPIX * np.abs(qr) + 4 * 2.0 ** -24 * l1).all()
+    # pixels the oracle leaves exactly empty stay exactly empty
+    assert (got[l1 == 0] == 0).all()
 
 
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
@@ -293,6 +297,7 @@ def test_convolve_asymmetric_response_and_chunking():
     np.testing.assert_array_equal(outs[0], outs[1])
     got = outs[0].astype(np.float64)
     assert np.abs(got - ref).max() <= TOL_WAVE * np.abs(ref).max()
+    assert np.abs(got - ref).max() <= 2e-6 * np.abs(ref).max()      # what fp32 actually gives
 
 
 def test_deterministic_bits():
