@@ -40,6 +40,8 @@ class Config:
     nsigma: float = 4.0
     point_thresh: float = 0.1
     drift_mm: float = 500.0         # generator only: depth of the drift volume
+    effq_mode: int = 0              # tred_config.effq_mode (kernel variant, 0 = default)
+    mac_mode: int = 0               # tred_config.mac_mode  (kernel variant, 0 = default)
 
     def with_(self, **kw) -> "Config":
         return replace(self, **kw)

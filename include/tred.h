@@ -64,6 +64,12 @@ typedef struct tred_config {
   int32_t block[3];              /* Bx, By (fine-grid points), Bt (ticks): powers of two  */
   int32_t resp_half;             /* H: response covers (2H+1)^2 pixels                    */
   int32_t resp_nticks;           /* Tr: response length in ticks                          */
+  int32_t effq_mode;             /* how tred_effq evaluates the charge density of Eq. (10):
+                                    0 = factored line integral (default, see tred_effq),
+                                    1 = closed form with erf per Gauss-Legendre node          */
+  int32_t mac_mode;              /* spectrum multiply-accumulate of tred_convolve:
+                                    0 = default (tensor cores, 3xTF32, if supported),
+                                    1 = fp32 FMA pipe, 2 = tensor cores 3xTF32              */
 } tred_config;
 
 /* Sizes derived from a configuration (host-side helper, no device work). */
@@ -132,10 +138,15 @@ int tred_blockbin(tred_ctx* ctx, int64_t nseg, const int32_t* d_augi,
 
 /*
  * tred_effq -- effective charge, Eq. (9) with Eq. (10) / the point-like branch
- * (readings G1, G4, G5, G10).  One CTA per block tile; the
- * block's segments are evaluated on dual cells (the cell between 8 neighbouring grid
- * points) so that every Gauss-Legendre node is evaluated once per tile and scattered to
- * its 8 corner grid points in shared memory without atomics.
+ * (readings G1, G4, G5, G10).  One CTA per block tile, the tile
+ * staged in shared memory, no atomics, fixed summation order.
+ *   effq_mode 0: the charge density at a Gauss-Legendre node is the line integral that
+ *     Eq. (10) is the closed form of, q = Q' int_0^1 prod_a N(r_a - p0_a - s d_a; sigma_a) ds,
+ *     evaluated by an m-point Gauss-Legendre rule in s with m chosen per segment so that
+ *     the relative error is < 1.5e-7 (below fp32 rounding of the result).  Every term is
+ *     separable in (x, y, t), so the sums over the n^3 nodes and the trilinear
+ *     coefficients u of Eq. (9) factor into three 1-D tables per segment.
+ *   effq_mode 1: Eq. (10) in closed form (exp, erf) at every node.
  *   d_payload [nblocks][Bx][By][Bt] float32 out (fully overwritten).
  */
 int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,

@@ -32,7 +32,8 @@ class TredConfig(C.Structure):
                 ("sigma_min_xy_mm", C.c_double), ("sigma_min_t_us", C.c_double),
                 ("nsigma", C.c_double), ("point_thresh", C.c_double),
                 ("gl_n", C.c_int32), ("block", C.c_int32 * 3),
-                ("resp_half", C.c_int32), ("resp_nticks", C.c_int32)]
+                ("resp_half", C.c_int32), ("resp_nticks", C.c_int32),
+                ("effq_mode", C.c_int32), ("mac_mode", C.c_int32)]
 
 
 class TredDims(C.Structure):
@@ -93,12 +94,20 @@ def lib() -> C.CDLL:
 
 
 _CFG_FIELDS = [f[0] for f in TredConfig._fields_]
+_CFG_OPTIONAL = ("effq_mode", "mac_mode")        # 0 = library default
 
 
 def make_config(cfg) -> TredConfig:
     get = (lambda k: cfg[k]) if isinstance(cfg, dict) else (lambda k: getattr(cfg, k))
     c = TredConfig()
     for k in _CFG_FIELDS:
+        if k in _CFG_OPTIONAL:
+            try:
+                v = get(k)
+            except (KeyError, AttributeError):
+                v = 0
+            setattr(c, k, int(v))
+            continue
         v = get(k)
         if k == "block":
             c.block[0], c.block[1], c.block[2] = (int(x) for x in v)

@@ -78,6 +78,14 @@ void tred_set_cuda_error(cudaError_t e, const char* where);
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
+// ---- S2 variants (tred_effq.cu: closed form; tred_effq_fact.cu: factored, dispatch) ---
+int tred_effq_closed_form(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
+                          const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
+                          const float* d_augf, const int32_t* d_augi,
+                          float* d_payload, cudaStream_t st);
+// Uploads the Gauss-Legendre tables of the line quadrature (called by tred_create).
+int tred_effq_init_tables(void);
+
 // ---- device-wide primitives (tred_scan_sort.cu) ----------------------------------
 // Exclusive scan of int32 (n elements) into out (may alias in); writes the total to
 // d_total (int64) if non-null.  work: at least tred_scan_work_bytes(n).

@@ -1,5 +1,7 @@
-// S2 effective charge: Eq. (9) with Eq. (10) / the point-like branch
-// (PAPER.md:L85-148, L197).
+// S2 effective charge, closed-form variant (effq_mode 1): Eq. (9) with Eq. (10) / the
+// point-like branch evaluated with exp and erf at every Gauss-Legendre node
+// (PAPER.md:L85-148, L197).  The default variant is tred_effq_fact.cu; this one is kept as
+// the literal per-node evaluation and as a cross-check of the factored form.
 //
 // Re-bracketing used here (same nodes, weights and coefficients as Eq. (9), only the
 // order of summation differs): the Gauss-Legendre nodes are grouped by DUAL CELL, the
@@ -208,14 +210,10 @@ k_effq(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict
 
 }  // namespace
 
-extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
-                         const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
-                         const float* d_augf, const int32_t* d_augi,
-                         float* d_payload, void* stream) {
-  if (!ctx || nseg < 0 || nblocks < 0) return TRED_EINVAL;
-  if (nblocks == 0) return TRED_OK;
-  if (!d_keys || !d_blk_off || !d_pair_seg || !d_augf || !d_augi || !d_payload) return TRED_EINVAL;
-  cudaStream_t st = (cudaStream_t)stream;
+int tred_effq_closed_form(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
+                          const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
+                          const float* d_augf, const int32_t* d_augi,
+                          float* d_payload, cudaStream_t st) {
   const TredGrid g = make_grid(ctx);
   EffqParams P;
   P.plane = g.Bx * g.By + 1;

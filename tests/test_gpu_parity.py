@@ -127,7 +127,8 @@ def test_blockbin_capacity_semantics_and_empty():
 
 
 # ------------------------------------------------------------------ S2
-def _effq_both(cfg, segs):
+def _effq_both(cfg, segs, effq_mode=0):
+    cfg = cfg.with_(effq_mode=effq_mode)
     aug = o.drift(cfg, segs)
     keys = o.blocks(cfg, aug)
     ref = o.effq(cfg, aug, keys)
@@ -140,28 +141,59 @@ def _effq_both(cfg, segs):
     return aug, keys, ref, got
 
 
+@pytest.mark.parametrize("effq_mode", [0, 1])
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
-def test_effq_parity(cfg_id):
+def test_effq_parity(cfg_id, effq_mode):
+    """effq_mode 0: factored line quadrature (default); 1: closed form Eq. (10) per node."""
     cfg, segs = _small(cfg_id)
-    aug, keys, ref, got = _effq_both(cfg, segs)
+    aug, keys, ref, got = _effq_both(cfg, segs, effq_mode)
     scale = np.abs(ref).max()
     assert scale > 0
     assert np.abs(got - ref).max() <= TOL_QEFF * scale
     assert abs(got.sum() - ref.sum()) <= 1e-5 * abs(ref.sum())
 
 
+@pytest.mark.parametrize("effq_mode", [0, 1])
 @pytest.mark.parametrize("n", [1, 2, 3, 4])
 @pytest.mark.parametrize("block", [(4, 4, 32), (8, 8, 64), (16, 16, 128), (32, 32, 256)])
-def test_effq_parity_sweep(n, block):
+def test_effq_parity_sweep(n, block, effq_mode):
     """Config 5's representation sweep on a small sample of config-3 inputs."""
     cfg, segs = gen.make_segments(3, n_vertices=1)
     cfg = cfg.with_(gl_n=n, block=block)
     segs = {k: v[:150] for k, v in segs.items()}
-    aug, keys, ref, got = _effq_both(cfg, segs)
+    aug, keys, ref, got = _effq_both(cfg, segs, effq_mode)
     assert np.abs(got - ref).max() <= TOL_QEFF * np.abs(ref).max()
 
 
-def test_effq_point_like_and_clipped_segments():
+def test_effq_factored_long_segments_in_sigmas():
+    """The line quadrature picks its order from the segment length in sigmas: 5 mm steps
+     at the minimum diffusion scale are ~60 sigma_t long along the drift and
+    take several quadrature pieces; a short stub takes the smallest rule."""
+    cfg = gen.make_config(1, t_origin_us=0.0, gl_n=3)
+    rows = [
+        (60.0, 60.0, 2.0, 60.3, 60.2, 7.0, 30000.0, 5.0),          # 5 mm along the drift, sigma_min
+        (30.0, 90.0, 1.0, 34.5, 91.0, 1.5, 30000.0, 20.0),         # 4.6 mm across the pixels, sigma_min
+        (80.0, 40.0, 100.0, 82.0, 43.0, 103.5, 25000.0, 0.0),      # 5 mm, diffused
+        (100.0, 100.0, 120.0, 100.02, 100.3, 120.01, 1800.0, 0.0),  # 0.3 mm stub
+    ]
+    segs = {k: np.array([r[i] for r in rows], np.float32) for i, k in enumerate(gen.SEG_FIELDS)}
+    aug, keys, ref, got = _effq_both(cfg, segs, 0)
+    W = np.sqrt((((aug["p1"] - aug["p0"]) / aug["sig"]) ** 2).sum(1))
+    assert W.max() > 40 and W.min() < 1.0
+    assert np.abs(got - ref).max() <= TOL_QEFF * np.abs(ref).max()
+    assert abs(got.sum() - ref.sum()) <= 1e-5 * abs(ref.sum())
+
+
+def test_effq_modes_agree():
+    """The two evaluations of Eq. (10) agree far below the parity tolerance."""
+    cfg, segs = _small(2)
+    _, _, ref, a = _effq_both(cfg, segs, 0)
+    _, _, _, b = _effq_both(cfg, segs, 1)
+    assert np.abs(a - b).max() <= 5e-6 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("effq_mode", [0, 1])
+def test_effq_point_like_and_clipped_segments(effq_mode):
     """Degenerate cases: a point-like stub, a segment straddling the grid edge, one
     wholly outside the grid (no blocks), one at z -> 0 (minimum diffusion scale)."""
     cfg = gen.make_config(1, t_origin_us=0.0)
@@ -174,7 +206,7 @@ def test_effq_point_like_and_clipped_segments():
         (60.0, 60.0, 163.0, 60.5, 60.2, 164.5, 6000.0, 0.0),       # straddles the last tick
     ]
     segs = {k: np.array([r[i] for r in rows], np.float32) for i, k in enumerate(gen.SEG_FIELDS)}
-    aug, keys, ref, got = _effq_both(cfg, segs)
+    aug, keys, ref, got = _effq_both(cfg, segs, effq_mode)
     assert aug["flag"][0] == 1 and aug["flag"][1] == 0
     assert np.abs(got - ref).max() <= TOL_QEFF * np.abs(ref).max()
 
