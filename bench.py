@@ -175,7 +175,7 @@ def run_cuda(args):
     for _ in range(max(args.warmup, 3)):
         out = sim.simulate(seg_d, rhat)
     barrier()
-    info = {k: out[k] for k in ("npairs", "nblocks", "nsp", "ntiles")}
+    info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles")}
     # Gauss-Legendre node evaluations of one step = cuboids of every bounding box x n^3
     _, augi0, _ = sim.drift(seg_d)
     ext = (augi0[3:6] - augi0[0:3] + 1).to(torch.float64)
@@ -251,7 +251,7 @@ def run_cuda(args):
         nb = info["nblocks"]
         ncols = cfg.block[0] * cfg.block[1]
         K = 2 * cfg.resp_half + 1
-        nf = d.fft_len // 2
+        nf = d.n_freq
         sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
         alu_peak = 148 * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12          # TFLOP/s at max clock
         roof = {"kernel": dom, "ms": stage_ms[dom]}

@@ -76,13 +76,19 @@ typedef struct tred_config {
 typedef struct tred_dims {
   int64_t NG[3];          /* fine-grid points (x, y, t)                                   */
   int64_t NB[3];          /* blocks per axis = ceil(NG/B)                                 */
-  int32_t fft_len;        /* L: power of two >= Bt + Tr - 1               */
+  int32_t fft_len;        /* L: smallest 2^a 3^b (a >= 3) >= Bt + Tr - 1 (reading G20;
+                             PAPER.md:L264 pads to a power of two)                        */
   int32_t out_len;        /* Bt + Tr - 1: ticks of one block's output                     */
   int32_t n_over;         /* ceil(out_len / Bt): tiles (Tt = Bt) one output spans         */
-  int32_t out_px, out_py; /* pixels per axis of one block's output footprint              */
-  int32_t n_class;        /* sub-pixel alignment classes of a block origin                */
-  int64_t rhat_floats;    /* floats of the response spectrum: L * S*S*(2H+1)^2            */
+  int32_t n_freq;         /* L/2 complex spectrum slots (slot 0 packs DC and Nyquist)     */
+  int32_t n_phase;        /* S*S sub-pixel phases                                         */
+  int32_t n_off;          /* (2H+1)^2 pixel offsets of the response                       */
+  int32_t n_off_pad;      /* n_off rounded up to a multiple of 8                          */
+  int32_t pix_per_block;  /* max charge pixels met by one block: product over x, y of
+                             floor((S - 1 + B - 1)/S) + 1                                 */
+  int64_t rhat_floats;    /* floats of the response spectrum buffer (all layouts)         */
   int64_t block_floats;   /* Bx*By*Bt                                                     */
+  int64_t conv_row_bytes; /* tred_convolve workspace bytes per charge pixel in flight     */
 } tred_dims;
 
 typedef struct tred_ctx tred_ctx;   /* opaque, host memory */
@@ -159,43 +165,50 @@ int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
  *   d_resp [S][S][2H+1][2H+1][Tr] float32: R[jx][jy][kx+H][ky+H][tau] = current at tick
  *          tau on the pixel displaced by (kx,ky) from the pixel holding a unit charge at
  *          sub-pixel phase (jx,jy) (readings G3, G12).
- *   d_rhat [rhat_floats] float32 out: spectrum, layout [L/2][S][S][2H+1][2H+1] complex
- *          (DC and Nyquist packed in slot 0).
+ *   d_rhat [rhat_floats] float32 out: the spectrum in the layouts the kernels read
+ *          (fp32 [f][phase][offset] complex, and the real-ified matrices
+ *          [f][2*offset+c][2*phase+c'] split into tf32 hi / lo parts for the tensor cores).
  */
 int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* d_rhat, void* stream);
 
 /*
- * tred_convolve_plan -- output footprint (O6): the (time slab, pixel) pairs
- * met by the output of any occupied block, and the (tile, pixel) list they overlap-add to.
- *   d_sp_keys   [cap_sp] int64 out: sorted keys (bt*npix_x + px)*npix_y + py
- *   d_sp_off    [NBt+1] int32 out: first slab-pixel index of every slab
- *   d_nsp       int64 out
- *   d_tile_keys [cap_tiles] int64 out: sorted keys (tb*npix_x + px)*npix_y + py
- *   d_ntiles    int64 out
- *   d_work      at least tred_plan_work_bytes() bytes; its content (the slab-pixel index
- *               map) is read again by tred_convolve and tred_gather_waveforms.
+ * tred_convolve_plan -- footprints (O6).  Charge pixels: the (time slab, pixel)
+ * pairs met by an occupied block; slab pixels: the (time slab, pixel) pairs met by the
+ * output of an occupied block (charge pixels dilated by H); tiles: the (tile, pixel)
+ * list the slab outputs overlap-add to.  All keys are (bt*npix_x + px)*npix_y + py, sorted.
+ *   d_cp_keys   [cap_cp] int64 out, d_cp_off [NBt+1] int32 out (first index per slab), d_ncp
+ *   d_sp_keys   [cap_sp] int64 out, d_sp_off [NBt+1] int32 out, d_nsp
+ *   d_tile_keys [cap_tiles] int64 out, d_ntiles
+ *   d_plan_work at least tred_plan_work_bytes() bytes; its content (the index maps) is
+ *               read again by tred_convolve and tred_gather_waveforms.
  */
 size_t tred_plan_work_bytes(const tred_ctx* ctx);
 int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
+                       int64_t cap_cp, int64_t* d_cp_keys, int32_t* d_cp_off, int64_t* d_ncp,
                        int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
                        int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
                        void* d_plan_work, size_t plan_work_bytes, void* stream);
 
 /*
- * tred_convolve -- Eq. (12) evaluated as Eq. (14) per block:
- * real FFT along time of every fine column of a block, multiply-accumulate with the
- * response spectrum of the column's sub-pixel phase onto the (2H+1)^2 neighbouring
- * pixels, sum over all blocks of a time slab in the frequency domain, one inverse FFT
- * per (slab, pixel).  Processes the slabs in groups that fit the workspace.
- *   h_slab_off [NBt+1] host copy of tred_blockbin's d_slab_off
- *   h_sp_off   [NBt+1] host copy of tred_convolve_plan's d_sp_off
+ * tred_convolve -- Eq. (12) evaluated as Eq. (14), pruned to
+ * the time axis: real FFT along time of the S*S fine columns of every charge pixel
+ * (zero where no block is occupied); per frequency, the product of the [charge pixels x
+ * phases] spectra with the [phases x offsets] response spectrum (one batched complex
+ * GEMM: fp32 FMA, or tensor cores with 3xTF32 split operands, see tred_config.mac_mode);
+ * sum over the (2H+1)^2 offsets onto the output pixels in the frequency domain (sum
+ * before the inverse FFT, Eq. (14)), in a fixed order; one inverse FFT per slab pixel.
+ * Charge pixels are processed in chunks that fit the workspace; results do not depend on
+ * the chunking (bit-identical).
+ *   h_cp_off   [NBt+1] HOST copy of tred_convolve_plan's d_cp_off
+ *   h_sp_off   [NBt+1] HOST copy of d_sp_off
  *   d_sp_data  [nsp][n_over*Bt] float32 out: current of (slab bt, pixel) from tick Bt*bt
- *   d_work     at least tred_convolve_work_bytes(max blocks of a slab, max slab-pixels of
- *              a slab) bytes; more lets several slabs share one launch.
+ *   d_work     at least tred_convolve_work_bytes(min_rows) bytes with min_rows >= 1; more
+ *              rows per chunk make larger launches.
  */
-size_t tred_convolve_work_bytes(const tred_ctx* ctx, int64_t nblocks_chunk, int64_t nsp_chunk);
-int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
-                  const int32_t* h_slab_off, const float* d_payload, const float* d_rhat,
+size_t tred_convolve_work_bytes(const tred_ctx* ctx, int64_t rows_chunk, int64_t nsp_batch);
+int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys, const float* d_payload,
+                  const float* d_rhat,
+                  int64_t ncp, const int64_t* d_cp_keys, const int32_t* h_cp_off,
                   int64_t nsp, const int64_t* d_sp_keys, const int32_t* h_sp_off,
                   const void* d_plan_work, float* d_sp_data,
                   void* d_work, size_t work_bytes, void* stream);

@@ -40,8 +40,9 @@ class TredDims(C.Structure):
     """Mirror of `tred_dims` (include/tred.h)."""
     _fields_ = [("NG", _c_i64 * 3), ("NB", _c_i64 * 3),
                 ("fft_len", C.c_int32), ("out_len", C.c_int32), ("n_over", C.c_int32),
-                ("out_px", C.c_int32), ("out_py", C.c_int32), ("n_class", C.c_int32),
-                ("rhat_floats", _c_i64), ("block_floats", _c_i64)]
+                ("n_freq", C.c_int32), ("n_phase", C.c_int32), ("n_off", C.c_int32),
+                ("n_off_pad", C.c_int32), ("pix_per_block", C.c_int32),
+                ("rhat_floats", _c_i64), ("block_floats", _c_i64), ("conv_row_bytes", _c_i64)]
 
 
 # name -> (restype, argtypes); every symbol include/tred.h declares
@@ -59,11 +60,16 @@ EXPORTS = {
     "tred_effq": (C.c_int, [_c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p]),
     "tred_prepare_response": (C.c_int, [_c_p, _c_p, _c_p, _c_p]),
     "tred_plan_work_bytes": (C.c_size_t, [_c_p]),
-    "tred_convolve_plan": (C.c_int, [_c_p, _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_i64, _c_p, _c_p,
+    "tred_convolve_plan": (C.c_int, [_c_p, _c_i64, _c_p,
+                                     _c_i64, _c_p, _c_p, _c_p,
+                                     _c_i64, _c_p, _c_p, _c_p,
+                                     _c_i64, _c_p, _c_p,
                                      _c_p, C.c_size_t, _c_p]),
     "tred_convolve_work_bytes": (C.c_size_t, [_c_p, _c_i64, _c_i64]),
-    "tred_convolve": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
-                                _c_p, C.c_size_t, _c_p]),
+    "tred_convolve": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p,
+                                _c_i64, _c_p, _c_p,
+                                _c_i64, _c_p, _c_p,
+                                _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p,
                                         _c_p]),
     "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
@@ -243,46 +249,59 @@ class Tred:
                                 _ptr(augf), _ptr(augi), _ptr(payload), self._stream()), "tred_effq")
         return payload
 
-    def convolve_plan(self, nblocks: int, keys, cap_sp: int, cap_tiles: int):
+    def convolve_plan(self, nblocks: int, keys, cap_cp: int | None = None, cap_sp: int | None = None,
+                      cap_tiles: int | None = None) -> dict:
+        """Footprints of the convolution; returns a dict of device tensors (counts are
+        1-element int64 device tensors, read them yourself)."""
         t = self.torch
         NBt = int(self.dims.NB[2])
-        sp_keys = self._empty((max(cap_sp, 1),), t.int64)
-        sp_off = self._empty((NBt + 1,), t.int32)
-        nsp = self._empty((1,), t.int64)
-        tile_keys = self._empty((max(cap_tiles, 1),), t.int64)
-        ntiles = self._empty((1,), t.int64)
+        nmap = NBt * self.cfg.npix_x * self.cfg.npix_y
+        K2 = self.dims.n_off
+        if cap_cp is None:
+            cap_cp = min(nblocks * self.dims.pix_per_block, nmap)
+        if cap_sp is None:
+            cap_sp = min(cap_cp * K2, nmap)
+        if cap_tiles is None:
+            cap_tiles = min(cap_sp * self.dims.n_over, nmap)
+        p = dict(cp_keys=self._empty((max(cap_cp, 1),), t.int64), cp_off=self._empty((NBt + 1,), t.int32),
+                 ncp=self._empty((1,), t.int64),
+                 sp_keys=self._empty((max(cap_sp, 1),), t.int64), sp_off=self._empty((NBt + 1,), t.int32),
+                 nsp=self._empty((1,), t.int64),
+                 tile_keys=self._empty((max(cap_tiles, 1),), t.int64), ntiles=self._empty((1,), t.int64))
         pw = self.L.tred_plan_work_bytes(self.h)
-        plan = self._empty((pw,), t.uint8)
-        _check(self.L.tred_convolve_plan(self.h, nblocks, _ptr(keys), cap_sp, _ptr(sp_keys), _ptr(sp_off),
-                                         _ptr(nsp), cap_tiles, _ptr(tile_keys), _ptr(ntiles),
-                                         _ptr(plan), plan.numel(), self._stream()), "tred_convolve_plan")
-        return sp_keys, sp_off, nsp, tile_keys, ntiles, plan
+        p["work"] = self._empty((pw,), t.uint8)
+        _check(self.L.tred_convolve_plan(self.h, nblocks, _ptr(keys),
+                                         cap_cp, _ptr(p["cp_keys"]), _ptr(p["cp_off"]), _ptr(p["ncp"]),
+                                         cap_sp, _ptr(p["sp_keys"]), _ptr(p["sp_off"]), _ptr(p["nsp"]),
+                                         cap_tiles, _ptr(p["tile_keys"]), _ptr(p["ntiles"]),
+                                         _ptr(p["work"]), p["work"].numel(), self._stream()), "tred_convolve_plan")
+        return p
 
-    def convolve(self, nblocks: int, keys, slab_off_host, payload, rhat, nsp: int, sp_keys, sp_off_host,
-                 plan, sp_data=None, work_bytes: int | None = None):
+    def convolve(self, nblocks: int, keys, payload, rhat, plan: dict, ncp: int, nsp: int,
+                 cp_off_host, sp_off_host, sp_data=None, work_bytes: int | None = None):
         t = self.torch
         import numpy as np
         row = self.dims.n_over * self.cfg.block[2]
         if sp_data is None:
             sp_data = self._empty((max(nsp, 1), row), t.float32)
-        so = np.ascontiguousarray(slab_off_host, dtype=np.int32)
+        co = np.ascontiguousarray(cp_off_host, dtype=np.int32)
         po = np.ascontiguousarray(sp_off_host, dtype=np.int32)
-        nb_max = int(np.diff(so).max()) if len(so) > 1 else 0
         ns_max = int(np.diff(po).max()) if len(po) > 1 else 0
-        need = self.L.tred_convolve_work_bytes(self.h, nb_max, ns_max)
+        need = self.L.tred_convolve_work_bytes(self.h, 128, ns_max)
         if work_bytes is None:
             work_bytes = self.conv_work_bytes
         if work_bytes is None:
-            work_bytes = min(self.L.tred_convolve_work_bytes(self.h, nblocks, nsp), 8 << 30)
+            work_bytes = min(self.L.tred_convolve_work_bytes(self.h, ncp, nsp), 16 << 30)
         work_bytes = max(int(work_bytes), int(need))
         work = self._workbuf("conv", work_bytes)
-        _check(self.L.tred_convolve(self.h, nblocks, _ptr(keys), so.ctypes.data_as(_c_p), _ptr(payload),
-                                    _ptr(rhat), nsp, _ptr(sp_keys), po.ctypes.data_as(_c_p), _ptr(plan),
-                                    _ptr(sp_data), _ptr(work), work.numel(), self._stream()),
+        _check(self.L.tred_convolve(self.h, nblocks, _ptr(keys), _ptr(payload), _ptr(rhat),
+                                    ncp, _ptr(plan["cp_keys"]), co.ctypes.data_as(_c_p),
+                                    nsp, _ptr(plan["sp_keys"]), po.ctypes.data_as(_c_p),
+                                    _ptr(plan["work"]), _ptr(sp_data), _ptr(work), work.numel(), self._stream()),
                "tred_convolve")
         return sp_data
 
-    def gather_waveforms(self, nsp: int, sp_data, plan, ntiles: int, tile_keys, pix_ids=None):
+    def gather_waveforms(self, nsp: int, sp_data, plan: dict, ntiles: int, pix_ids=None):
         t = self.torch
         Bt = self.cfg.block[2]
         tile_data = self._empty((max(ntiles, 1), Bt), t.float32)
@@ -292,9 +311,9 @@ class Tred:
             assert pix_ids.dtype == t.int32 and pix_ids.is_cuda
             npix = pix_ids.numel()
             dense = self._empty((npix, self.cfg.nticks), t.float32)
-        _check(self.L.tred_gather_waveforms(self.h, nsp, _ptr(sp_data), _ptr(plan), ntiles, _ptr(tile_keys),
-                                            _ptr(tile_data), npix, _ptr(pix_ids), _ptr(dense),
-                                            self._stream()), "tred_gather_waveforms")
+        _check(self.L.tred_gather_waveforms(self.h, nsp, _ptr(sp_data), _ptr(plan["work"]), ntiles,
+                                            _ptr(plan["tile_keys"]), _ptr(tile_data), npix, _ptr(pix_ids),
+                                            _ptr(dense), self._stream()), "tred_gather_waveforms")
         return tile_data, dense
 
     # -- whole path -----------------------------------------------------------------
@@ -308,19 +327,16 @@ class Tred:
         keys, blk_off, pair_seg, slab_off, nblocks_d = self.blockbin(augi, cap_pairs)
         nblocks = int(nblocks_d.item())
         payload = self.effq(nblocks, keys, blk_off, pair_seg, augf, augi)
-        npixtot = self.cfg.npix_x * self.cfg.npix_y
+        plan = self.convolve_plan(nblocks, keys)
+        counts = t.cat([plan["ncp"], plan["nsp"], plan["ntiles"], plan["cp_off"].to(t.int64),
+                        plan["sp_off"].to(t.int64)]).cpu().numpy()
+        ncp, nsp, ntiles = int(counts[0]), int(counts[1]), int(counts[2])
         NBt = int(self.dims.NB[2])
-        outp = self.dims.out_px * self.dims.out_py
-        cap_sp = min(nblocks * outp, NBt * npixtot)
-        cap_tiles = min(cap_sp * self.dims.n_over, NBt * npixtot)
-        sp_keys, sp_off, nsp_d, tile_keys, ntiles_d, plan = self.convolve_plan(nblocks, keys, cap_sp, cap_tiles)
-        counts = t.cat([nsp_d, ntiles_d]).cpu()
-        nsp, ntiles = int(counts[0]), int(counts[1])
-        so = slab_off.cpu().numpy()
-        po = sp_off.cpu().numpy()
-        sp_data = self.convolve(nblocks, keys, so, payload, rhat, nsp, sp_keys, po, plan)
-        tile_data, dense = self.gather_waveforms(nsp, sp_data, plan, ntiles, tile_keys, pix_ids)
-        out = dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, nsp=nsp, ntiles=ntiles,
+        co, po = counts[3:3 + NBt + 1], counts[3 + NBt + 1:]
+        sp_data = self.convolve(nblocks, keys, payload, rhat, plan, ncp, nsp, co, po)
+        tile_data, dense = self.gather_waveforms(nsp, sp_data, plan, ntiles, pix_ids)
+        tile_keys, sp_keys, sp_off = plan["tile_keys"], plan["sp_keys"], plan["sp_off"]
+        out = dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ncp=ncp, nsp=nsp, ntiles=ntiles,
                    tile_keys=tile_keys[:ntiles], tile_data=tile_data[:ntiles], dense=dense)
         if keep:
             out.update(augf=augf, augi=augi, keys=keys[:nblocks], blk_off=blk_off[:nblocks + 1],

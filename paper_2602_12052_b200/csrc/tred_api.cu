@@ -73,7 +73,7 @@ extern "C" int tred_stage_count(void) { return ST_COUNT; }
 
 extern "C" const char* tred_stage_name(int s) {
   static const char* names[ST_COUNT] = {"drift", "pairs", "sort", "rle", "effq", "plan", "resp_dft",
-                                        "fft_fwd", "class_bundles", "mac", "accum", "ifft", "gather"};
+                                        "fft_fwd", "conv_misc", "mac", "accum", "ifft", "gather"};
   return (s >= 0 && s < ST_COUNT) ? names[s] : "?";
 }
 extern "C" int tred_abi_version(void) { return 1; }
@@ -91,7 +91,6 @@ extern "C" const char* tred_strerror(int s) {
 
 // ------------------------------------------------------------------ dims / context
 static bool is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
-static int gcd_i(int a, int b) { while (b) { int t = a % b; a = b; b = t; } return a; }
 
 extern "C" int tred_get_dims(const tred_config* c, tred_dims* d) {
   if (!c || !d) return TRED_EINVAL;
@@ -111,20 +110,33 @@ extern "C" int tred_get_dims(const tred_config* c, tred_dims* d) {
   if (d->NB[0] * d->NB[1] * d->NB[2] >= (1ll << 31)) return TRED_EUNSUPPORTED;
   if ((int64_t)c->npix_x * c->npix_y * d->NB[2] >= (1ll << 31)) return TRED_EUNSUPPORTED;
   d->out_len = c->block[2] + c->resp_nticks - 1;
-  int L = 1;
-  while (L < d->out_len) L *= 2;       // power-of-two padding
-  if (L < 64) L = 64;
-  if (L > 4096) return TRED_EUNSUPPORTED;
+  // Padding: any L >= Bt + Tr - 1 gives the linear convolution (PAPER.md:L264 pads to a
+  // power of two; reading G20).  L = smallest 2^a 3^b >= out_len with a >= 3: fewer
+  // frequencies for the spectrum multiply-accumulate, still short radix-{8,4,2,3} FFTs.
+  int L = 0;
+  for (int p3 = 1; p3 <= 8192; p3 *= 3)
+    for (int p2 = 8; p2 * p3 <= 8192; p2 *= 2) {
+      const int cand = p2 * p3;
+      if (cand >= d->out_len && cand >= 64 && (L == 0 || cand < L)) L = cand;
+    }
+  if (L == 0 || L > 4096) return TRED_EUNSUPPORTED;
   d->fft_len = L;
   d->n_over = (d->out_len + c->block[2] - 1) / c->block[2];
-  if (d->n_over * c->block[2] > L) return TRED_EUNSUPPORTED;
-  // pixels spanned by B consecutive fine points starting anywhere in a pixel, plus 2H
-  d->out_px = (c->sub - 1 + c->block[0] - 1) / c->sub + 1 + 2 * c->resp_half;
-  d->out_py = (c->sub - 1 + c->block[1] - 1) / c->sub + 1 + 2 * c->resp_half;
-  d->n_class = (c->sub / gcd_i(c->sub, c->block[0])) * (c->sub / gcd_i(c->sub, c->block[1]));
-  int K = 2 * c->resp_half + 1;
-  d->rhat_floats = (int64_t)L * c->sub * c->sub * K * K;
+  d->n_freq = L / 2;
+  d->n_phase = c->sub * c->sub;
+  const int K = 2 * c->resp_half + 1;
+  d->n_off = K * K;
+  d->n_off_pad = (d->n_off + 7) / 8 * 8;
+  if (d->n_off_pad > 128) return TRED_EUNSUPPORTED;      // MAC tiles hold all offsets
+  // pixels spanned by B consecutive fine points starting anywhere in a pixel
+  d->pix_per_block = ((c->sub - 1 + c->block[0] - 1) / c->sub + 1) *
+                     ((c->sub - 1 + c->block[1] - 1) / c->sub + 1);
+  // response spectrum: fp32 [f][phase][off_pad] complex (2 floats) + tf32 hi and lo
+  // [f][2 off_pad][2 phase] (4 floats each)
+  d->rhat_floats = (int64_t)d->n_freq * d->n_phase * d->n_off_pad * 10;
   d->block_floats = (int64_t)c->block[0] * c->block[1] * c->block[2];
+  // per charge pixel in flight: spectra [f][phase] + products [f][off_pad], complex fp32
+  d->conv_row_bytes = (int64_t)d->n_freq * (d->n_phase + d->n_off_pad) * 8;
   return TRED_OK;
 }
 

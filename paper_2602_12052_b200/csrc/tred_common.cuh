@@ -6,7 +6,7 @@
 #include "../../include/tred.h"
 
 enum TredStage {
-  ST_DRIFT = 0, ST_PAIRS, ST_SORT, ST_RLE, ST_EFFQ, ST_PLAN, ST_RESP, ST_FFT_FWD, ST_CLASS, ST_MAC,
+  ST_DRIFT = 0, ST_PAIRS, ST_SORT, ST_RLE, ST_EFFQ, ST_PLAN, ST_RESP, ST_FFT_FWD, ST_MISC, ST_MAC,
   ST_ACCUM, ST_IFFT, ST_GATHER, ST_COUNT
 };
 
@@ -44,7 +44,9 @@ struct TredGrid {
   int S, H, Tr;
   int npx, npy, nticks;
   int L;            // fft length
-  int outx, outy;   // output footprint pixels of one block
+  int nf;           // L/2 spectrum slots
+  int nph;          // S*S phases
+  int noff, kp;     // (2H+1)^2 offsets, padded to a multiple of 8
   int nover;        // tiles per output
   int gl_n;
 };
@@ -56,7 +58,8 @@ static inline TredGrid make_grid(const tred_ctx* c) {
   g.NBx = (int)c->dims.NB[0]; g.NBy = (int)c->dims.NB[1]; g.NBt = (int)c->dims.NB[2];
   g.S = c->cfg.sub; g.H = c->cfg.resp_half; g.Tr = c->cfg.resp_nticks;
   g.npx = c->cfg.npix_x; g.npy = c->cfg.npix_y; g.nticks = c->cfg.nticks;
-  g.L = c->dims.fft_len; g.outx = c->dims.out_px; g.outy = c->dims.out_py;
+  g.L = c->dims.fft_len; g.nf = c->dims.n_freq; g.nph = c->dims.n_phase;
+  g.noff = c->dims.n_off; g.kp = c->dims.n_off_pad;
   g.nover = c->dims.n_over; g.gl_n = c->cfg.gl_n;
   return g;
 }

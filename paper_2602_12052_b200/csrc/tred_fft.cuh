@@ -1,0 +1,166 @@
+// Shared-memory mixed-radix FFT used by the block convolution (S4, PAPER.md:L223-232
+// Eq. (14); padding rule PAPER.md:L264, reading G20).
+//
+// Batched complex Stockham autosort FFT of length M = 2^a 3^b, radices {8, 4, 2, 3},
+// ping-pong between two shared buffers; every thread does whole radix-R butterflies in
+// registers.  Real transforms of length N = 2M go through one complex FFT of length M
+// (no pairing of two signals, so no rounding cross-talk between columns / pixels):
+//   forward:  z[m] = x[2m] + i x[2m+1],  Z = FFT_M(z),
+//             X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) e^{-2 pi i k/N} (Z[k] - conj Z[M-k]),
+//             X[0] = Re Z[0] + Im Z[0] (DC), X[M] = Re Z[0] - Im Z[0] (Nyquist).
+//   inverse:  Z[k] = (X[k] + conj X[M-k]) + i e^{+2 pi i k/N} (X[k] - conj X[M-k]),
+//             z = IFFT_M(Z) (unnormalised), x[2m] = Re z[m]/N, x[2m+1] = Im z[m]/N.
+// Spectra hold M complex numbers: slot 0 packs (DC, Nyquist), both real.
+#pragma once
+#include <cuda_runtime.h>
+
+struct FftPlan {
+  int M;            // complex length
+  int npass;
+  int radix[12];
+};
+
+static inline bool tred_make_fft_plan(int M, FftPlan* p) {
+  p->M = M; p->npass = 0;
+  int m = M;
+  while (m % 8 == 0) { p->radix[p->npass++] = 8; m /= 8; }
+  while (m % 4 == 0) { p->radix[p->npass++] = 4; m /= 4; }
+  while (m % 2 == 0) { p->radix[p->npass++] = 2; m /= 2; }
+  while (m % 3 == 0) { p->radix[p->npass++] = 3; m /= 3; }
+  return m == 1 && p->npass <= 12;
+}
+
+__device__ __forceinline__ float2 cmulf(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+// multiply by -i (forward) or +i (inverse)
+template <bool INV> __device__ __forceinline__ float2 mul_mi(float2 a) {
+  return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+}
+
+template <bool INV> __device__ __forceinline__ void dft2(float2& a, float2& b) {
+  const float2 t = a;
+  a = make_float2(t.x + b.x, t.y + b.y);
+  b = make_float2(t.x - b.x, t.y - b.y);
+}
+
+template <bool INV> __device__ __forceinline__ void dft4(float2* v) {
+  dft2<INV>(v[0], v[2]);
+  dft2<INV>(v[1], v[3]);
+  v[3] = mul_mi<INV>(v[3]);
+  dft2<INV>(v[0], v[1]);
+  dft2<INV>(v[2], v[3]);
+  const float2 t = v[1]; v[1] = v[2]; v[2] = t;       // bit reversal of 2 bits
+}
+
+template <bool INV> __device__ __forceinline__ void dft8(float2* v) {
+  constexpr float H = 0.70710678118654752f;
+  dft2<INV>(v[0], v[4]); dft2<INV>(v[1], v[5]); dft2<INV>(v[2], v[6]); dft2<INV>(v[3], v[7]);
+  // twiddles w8^1, w8^2, w8^3 on the odd half
+  { const float2 t = v[5]; v[5] = INV ? make_float2(H * (t.x - t.y), H * (t.x + t.y))
+                                      : make_float2(H * (t.x + t.y), H * (t.y - t.x)); }
+  v[6] = mul_mi<INV>(v[6]);
+  { const float2 t = v[7]; v[7] = INV ? make_float2(-H * (t.x + t.y), H * (t.x - t.y))
+                                      : make_float2(H * (t.y - t.x), -H * (t.x + t.y)); }
+  dft2<INV>(v[0], v[2]); dft2<INV>(v[1], v[3]); dft2<INV>(v[4], v[6]); dft2<INV>(v[5], v[7]);
+  v[3] = mul_mi<INV>(v[3]); v[7] = mul_mi<INV>(v[7]);
+  dft2<INV>(v[0], v[1]); dft2<INV>(v[2], v[3]); dft2<INV>(v[4], v[5]); dft2<INV>(v[6], v[7]);
+  // bit reversal of 3 bits: (1,4) (3,6)
+  float2 t = v[1]; v[1] = v[4]; v[4] = t;
+  t = v[3]; v[3] = v[6]; v[6] = t;
+}
+
+template <bool INV> __device__ __forceinline__ void dft3(float2* v) {
+  constexpr float S60 = 0.86602540378443865f;
+  const float2 t = make_float2(v[1].x + v[2].x, v[1].y + v[2].y);
+  const float2 u = make_float2(v[1].x - v[2].x, v[1].y - v[2].y);
+  const float2 m = make_float2(v[0].x - 0.5f * t.x, v[0].y - 0.5f * t.y);
+  // forward: -i sin60 u ; inverse: +i sin60 u
+  const float2 n = INV ? make_float2(-S60 * u.y, S60 * u.x) : make_float2(S60 * u.y, -S60 * u.x);
+  v[0] = make_float2(v[0].x + t.x, v[0].y + t.y);
+  v[1] = make_float2(m.x + n.x, m.y + n.y);
+  v[2] = make_float2(m.x - n.x, m.y - n.y);
+}
+
+// twN[k] = exp(-2 pi i k / N), k < N = 2M.  w_M^e = twN[2e].
+__device__ __forceinline__ void fill_twiddles_N(float2* twN, int N) {
+  for (int k = threadIdx.x; k < N; k += blockDim.x) {
+    float sn, cs;
+    sincospif(-2.0f * (float)k / (float)N, &sn, &cs);
+    twN[k] = make_float2(cs, sn);
+  }
+}
+
+// One Stockham pass of radix R over nb transforms of length M.
+// src/dst: [nb][bs] shared buffers (bs >= M: batch stride, padded against bank conflicts).
+// Ns = product of the radices of earlier passes.
+template <int R, bool INV>
+__device__ __forceinline__ void stockham_pass(const float2* __restrict__ src, float2* __restrict__ dst,
+                                              const float2* __restrict__ twN, int M, int Ns, int nb, int bs) {
+  const int per = M / R;
+  const int tws = (M / (Ns * R)) * 2;       // exponent step in units of twN
+  for (int idx = threadIdx.x; idx < nb * per; idx += blockDim.x) {
+    const int b = idx / per, j = idx - b * per;
+    const int k = j % Ns;
+    float2 v[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) v[t] = src[b * bs + j + t * per];
+    if (Ns > 1) {
+#pragma unroll
+      for (int t = 1; t < R; ++t) {
+        float2 w = twN[k * t * tws];
+        if (INV) w.y = -w.y;
+        v[t] = cmulf(v[t], w);
+      }
+    }
+    if (R == 2) dft2<INV>(v[0], v[1]);
+    else if (R == 3) dft3<INV>(v);
+    else if (R == 4) dft4<INV>(v);
+    else dft8<INV>(v);
+    const int o = b * bs + (j - k) * R + k;
+#pragma unroll
+    for (int t = 0; t < R; ++t) dst[o + t * Ns] = v[t];
+  }
+}
+
+// Runs all passes; data starts in `a`, returns the buffer that holds the result
+// (natural order).  Contains the __syncthreads between passes and one after the last.
+template <bool INV>
+__device__ __forceinline__ float2* fft_stockham(float2* a, float2* b, const float2* twN,
+                                                const FftPlan& pl, int nb, int bs) {
+  int Ns = 1;
+  for (int p = 0; p < pl.npass; ++p) {
+    const int R = pl.radix[p];
+    if (R == 8) stockham_pass<8, INV>(a, b, twN, pl.M, Ns, nb, bs);
+    else if (R == 4) stockham_pass<4, INV>(a, b, twN, pl.M, Ns, nb, bs);
+    else if (R == 2) stockham_pass<2, INV>(a, b, twN, pl.M, Ns, nb, bs);
+    else stockham_pass<3, INV>(a, b, twN, pl.M, Ns, nb, bs);
+    __syncthreads();
+    Ns *= R;
+    float2* t = a; a = b; b = t;
+  }
+  return a;
+}
+
+// Z: complex spectrum of the packed signal (natural order); returns X[k], k < M
+// (slot 0 = (DC, Nyquist)).
+__device__ __forceinline__ float2 rfft_post(const float2* Z, const float2* twN, int M, int k) {
+  if (k == 0) { const float2 z0 = Z[0]; return make_float2(z0.x + z0.y, z0.x - z0.y); }
+  const float2 p = Z[k], q = Z[M - k];
+  const float2 e = make_float2(0.5f * (p.x + q.x), 0.5f * (p.y - q.y));     // (Z[k] + conj Z[M-k])/2
+  const float2 o = make_float2(0.5f * (p.x - q.x), 0.5f * (p.y + q.y));     // (Z[k] - conj Z[M-k])/2
+  const float2 w = twN[k];
+  const float2 wo = cmulf(w, o);
+  return make_float2(e.x + wo.y, e.y - wo.x);                                // e - i w o
+}
+
+// X: packed half spectrum; returns Z[k] of the inverse.
+__device__ __forceinline__ float2 rfft_pre_inverse(const float2* X, const float2* twN, int M, int k) {
+  if (k == 0) { const float2 x0 = X[0]; return make_float2(x0.x + x0.y, x0.x - x0.y); }
+  const float2 p = X[k], q = X[M - k];
+  const float2 e = make_float2(p.x + q.x, p.y - q.y);                       // X[k] + conj X[M-k]
+  const float2 o = make_float2(p.x - q.x, p.y + q.y);                       // X[k] - conj X[M-k]
+  const float2 w = make_float2(twN[k].x, -twN[k].y);                        // e^{+2 pi i k/N}
+  const float2 wo = cmulf(w, o);
+  return make_float2(e.x - wo.y, e.y + wo.x);                                // e + i w o
+}

@@ -35,18 +35,27 @@ def test_five_north_star_calls_are_present():
         assert n in names
 
 
-@pytest.mark.parametrize("cfg_id,L,nover,outp", [(1, 512, 5, 12), (2, 512, 8, 12), (3, 1024, 5, 13)])
-def test_dims_host_logic(cfg_id, L, nover, outp):
-    """fft_len is the power of two >= Bt + Tr - 1 (32 + 2000 - 1 -> 2048)."""
+@pytest.mark.parametrize("cfg_id,L,nover,ppb", [(1, 288, 5, 4), (2, 512, 8, 4), (3, 576, 5, 9)])
+def test_dims_host_logic(cfg_id, L, nover, ppb):
+    """fft_len is the smallest 2^a 3^b (a >= 3) >= Bt + Tr - 1 (reading G20; the paper pads
+    to a power of two, which this rule reproduces for its own block)."""
     import paper_2602_12052_b200 as pkg
     cfg = gen.make_config(cfg_id)
     d = pkg.get_dims(cfg)
     assert d.fft_len == L and d.out_len == cfg.block[2] + cfg.resp_nticks - 1
-    assert d.n_over == nover and d.out_px == outp and d.out_py == outp
+    assert d.fft_len >= d.out_len
+    n = L
+    while n % 2 == 0:
+        n //= 2
+    while n % 3 == 0:
+        n //= 3
+    assert n == 1 and L % 8 == 0
+    assert d.n_over == nover and d.n_freq == L // 2 and d.pix_per_block == ppb
     assert list(d.NG) == [cfg.sub * cfg.npix_x, cfg.sub * cfg.npix_y, cfg.nticks]
     assert list(d.NB) == [-(-d.NG[a] // cfg.block[a]) for a in range(3)]
-    assert d.n_class == 25
-    assert d.rhat_floats == L * 100 * 121
+    assert (d.n_phase, d.n_off, d.n_off_pad) == (100, 121, 128)
+    assert d.rhat_floats == 10 * (L // 2) * 100 * 128
+    assert d.conv_row_bytes == (L // 2) * (100 + 128) * 8
 
 
 def test_paper_block_shape_gives_paper_padding():

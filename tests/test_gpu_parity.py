@@ -223,6 +223,19 @@ def _wave_checks(got, ref):
     assert (got[l1 == 0] == 0).all()
 
 
+def _oracle_charge_pixels(cfg, keys):
+    """(slab, pixel) pairs met by an occupied block (O6), as sorted keys."""
+    g = o.grid_of(cfg)
+    bx, by, bt = o.key_to_bxyz(g, keys)
+    S = cfg.sub
+    out = set()
+    for x, y, t in zip(bx, by, bt):
+        for px in range(g.B[0] * x // S, min((g.B[0] * x + g.B[0] - 1) // S, cfg.npix_x - 1) + 1):
+            for py in range(g.B[1] * y // S, min((g.B[1] * y + g.B[1] - 1) // S, cfg.npix_y - 1) + 1):
+                out.add((int(t) * cfg.npix_x + px) * cfg.npix_y + py)
+    return np.array(sorted(out), dtype=np.int64)
+
+
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
 def test_plan_tiles_bit_exact(cfg_id):
     torch = _torch()
@@ -233,23 +246,46 @@ def test_plan_tiles_bit_exact(cfg_id):
     k = torch.from_numpy(keys).cuda()
     npix = cfg.npix_x * cfg.npix_y
     NBt = int(sim.dims.NB[2])
-    sp_keys, sp_off, nsp, tile_keys, ntiles, plan = sim.convolve_plan(len(keys), k, NBt * npix, NBt * npix)
+    p = sim.convolve_plan(len(keys), k)
     ref = o.out_tiles(cfg, keys)
-    assert int(ntiles.item()) == len(ref)
-    np.testing.assert_array_equal(tile_keys[:len(ref)].cpu().numpy(), ref)
-    # slab-pixel list = the same footprint without the time spread
-    spk = sp_keys[:int(nsp.item())].cpu().numpy()
+    assert int(p["ntiles"].item()) == len(ref)
+    np.testing.assert_array_equal(p["tile_keys"][:len(ref)].cpu().numpy(), ref)
+    # charge pixels
+    cref = _oracle_charge_pixels(cfg, keys)
+    assert int(p["ncp"].item()) == len(cref)
+    np.testing.assert_array_equal(p["cp_keys"][:len(cref)].cpu().numpy(), cref)
+    np.testing.assert_array_equal(p["cp_off"].cpu().numpy(),
+                                  np.searchsorted(cref // npix, np.arange(NBt + 1), side="left"))
+    # slab-pixel list = the output footprint without the time spread
+    spk = p["sp_keys"][:int(p["nsp"].item())].cpu().numpy()
     assert (np.diff(spk) > 0).all()
     g = o.grid_of(cfg)
     bt = keys // (g.NB[0] * g.NB[1])
     assert set(np.unique(spk // npix)) == set(np.unique(bt))
+    np.testing.assert_array_equal(p["sp_off"].cpu().numpy(),
+                                  np.searchsorted(spk // npix, np.arange(NBt + 1), side="left"))
 
 
+def _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix, work_bytes=None):
+    torch = _torch()
+    k = torch.from_numpy(keys).cuda()
+    p = sim.convolve_plan(len(keys), k)
+    ncp, nsp, ntiles = int(p["ncp"].item()), int(p["nsp"].item()), int(p["ntiles"].item())
+    sp_data = sim.convolve(len(keys), k, torch.from_numpy(payload32).cuda(), rhat, p, ncp, nsp,
+                           p["cp_off"].cpu().numpy(), p["sp_off"].cpu().numpy(), work_bytes=work_bytes)
+    tile_data, dense = sim.gather_waveforms(nsp, sp_data, p, ntiles,
+                                            torch.from_numpy(pix.astype(np.int32)).cuda())
+    return dense.cpu().numpy()
+
+
+@pytest.mark.parametrize("mac_mode", [1, 0])
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
-def test_convolve_parity_from_oracle_charge(cfg_id):
-    """S4+S5 alone: the GPU convolves the ORACLE's effective charge (cast to fp32)."""
+def test_convolve_parity_from_oracle_charge(cfg_id, mac_mode):
+    """S4+S5 alone: the GPU convolves the ORACLE's effective charge (cast to fp32).
+    mac_mode 1: fp32 FMA spectrum product; 0: library default (tensor cores if available)."""
     torch = _torch()
     cfg, segs = _small(cfg_id)
+    cfg = cfg.with_(mac_mode=mac_mode)
     R = gen.make_response(cfg, 2000 + cfg_id)
     aug = o.drift(cfg, segs)
     keys = o.blocks(cfg, aug)
@@ -261,19 +297,32 @@ def test_convolve_parity_from_oracle_charge(cfg_id):
     ref = o.conv_fft(cfg, keys, payload32.astype(np.float64), R, pix)
     sim = _sim(cfg)
     rhat = sim.prepare_response(torch.from_numpy(R).cuda())
-    k = torch.from_numpy(keys).cuda()
-    npix = cfg.npix_x * cfg.npix_y
-    NBt = int(sim.dims.NB[2])
-    sp_keys, sp_off, nsp, tile_keys, ntiles, plan = sim.convolve_plan(len(keys), k, NBt * npix, NBt * npix)
-    g = o.grid_of(cfg)
-    bt = keys // (g.NB[0] * g.NB[1])
-    slab_off = np.searchsorted(bt, np.arange(g.NB[2] + 1), side="left").astype(np.int32)
-    nsp, ntiles = int(nsp.item()), int(ntiles.item())
-    sp_data = sim.convolve(len(keys), k, slab_off, torch.from_numpy(payload32).cuda(), rhat, nsp, sp_keys,
-                           sp_off.cpu().numpy(), plan)
-    tile_data, dense = sim.gather_waveforms(nsp, sp_data, plan, ntiles, tile_keys,
-                                            torch.from_numpy(pix.astype(np.int32)).cuda())
-    _wave_checks(dense.cpu().numpy().astype(np.float64), ref)
+    got = _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix)
+    _wave_checks(got.astype(np.float64), ref)
+
+
+@pytest.mark.parametrize("block,tr", [((4, 4, 32), 200), ((8, 8, 64), 137), ((16, 16, 128), 400),
+                                      ((32, 32, 256), 400), ((8, 8, 32), 225)])
+def test_convolve_parity_fft_lengths(block, tr):
+    """Config 5's block shapes and odd response lengths: FFT lengths 2^a 3^b with every
+    radix mix (432 = 16*27, 256, 576 = 64*9, 768 = 256*3, 256)."""
+    torch = _torch()
+    cfg, segs = gen.make_segments(1)
+    cfg = cfg.with_(block=block, resp_nticks=tr, gl_n=2)
+    segs = {k: v[:150] for k, v in segs.items()}
+    R = gen.make_random_response(cfg, 5)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    assert len(keys) > 0
+    payload32 = o.effq(cfg, aug, keys).astype(np.float32)
+    tiles = o.out_tiles(cfg, keys)
+    act = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
+    pix = act[:: max(1, len(act) // 24)]
+    ref = o.conv_fft(cfg, keys, payload32.astype(np.float64), R, pix)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    got = _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix).astype(np.float64)
+    assert np.abs(got - ref).max() <= TOL_WAVE * np.abs(ref).max()
 
 
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
@@ -321,7 +370,7 @@ def test_convolve_asymmetric_response_and_chunking():
     pix = np.arange(0, cfg.npix_x * cfg.npix_y, 13)
     ref = o.conv_fft(cfg, keys, payload, R, pix)
     outs = []
-    for wb in (None, 1):          # 1 byte -> raised to the per-slab minimum
+    for wb in (None, 1):          # 1 byte -> raised to the minimum (128 charge pixels per chunk)
         sim = _sim(cfg, conv_work_bytes=wb)
         out = sim.simulate(_seg_tensor(segs), sim.prepare_response(torch.from_numpy(R).cuda()),
                            torch.from_numpy(pix.astype(np.int32)).cuda())
