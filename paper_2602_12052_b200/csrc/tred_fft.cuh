@@ -2,8 +2,8 @@
 // Eq. (14); padding rule PAPER.md:L264, reading G20).
 //
 // Batched complex Stockham autosort FFT of length M = 2^a 3^b, radices {8, 4, 2, 3},
-// ping-pong between two shared buffers; every thread does whole radix-R butterflies in
-// registers.  Real transforms of length N = 2M go through one complex FFT of length M
+// ping-pong between two shared buffers laid out [element][transform]; every thread does
+// whole radix-R butterflies in registers.  Real transforms of length N = 2M go through one complex FFT of length M
 // (no pairing of two signals, so no rounding cross-talk between columns / pixels):
 //   forward:  z[m] = x[2m] + i x[2m+1],  Z = FFT_M(z),
 //             X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) e^{-2 pi i k/N} (Z[k] - conj Z[M-k]),
@@ -82,29 +82,39 @@ template <bool INV> __device__ __forceinline__ void dft3(float2* v) {
   v[2] = make_float2(m.x - n.x, m.y - n.y);
 }
 
-// twN[k] = exp(-2 pi i k / N), k < N = 2M.  w_M^e = twN[2e].
-__device__ __forceinline__ void fill_twiddles_N(float2* twN, int N) {
-  for (int k = threadIdx.x; k < N; k += blockDim.x) {
-    float sn, cs;
-    sincospif(-2.0f * (float)k / (float)N, &sn, &cs);
-    twN[k] = make_float2(cs, sn);
-  }
+// twN[k] = exp(-2 pi i k / N), k < N = 2M.  w_M^e = twN[2e].  Filled once per call into
+// global memory (k_fill_twiddles in tred_conv.cu), copied to shared memory by each CTA.
+__device__ __forceinline__ float2 twiddle_N(int k, int N) {
+  float sn, cs;
+  sincospif(-2.0f * (float)k / (float)N, &sn, &cs);
+  return make_float2(cs, sn);
+}
+__device__ __forceinline__ void load_twiddles_N(float2* twN, const float2* __restrict__ gtw, int N) {
+  for (int k = threadIdx.x; k < N; k += blockDim.x) twN[k] = gtw[k];
 }
 
 // One Stockham pass of radix R over nb transforms of length M.
-// src/dst: [nb][bs] shared buffers (bs >= M: batch stride, padded against bank conflicts).
-// Ns = product of the radices of earlier passes.
+// src/dst: [M][nb] shared buffers, the batch index fastest: the threads of a warp work on
+// neighbouring transforms at the same butterfly, so every shared-memory access of a warp
+// is a contiguous run (no bank conflicts) and the twiddle loads are broadcasts.
+// Ns = product of the radices of earlier passes.  Elements >= nz of src are taken as zero
+// without being read (zero padding of the first pass).
 template <int R, bool INV>
 __device__ __forceinline__ void stockham_pass(const float2* __restrict__ src, float2* __restrict__ dst,
-                                              const float2* __restrict__ twN, int M, int Ns, int nb, int bs) {
+                                              const float2* __restrict__ twN, int M, int Ns, int nb, int nz) {
   const int per = M / R;
   const int tws = (M / (Ns * R)) * 2;       // exponent step in units of twN
-  for (int idx = threadIdx.x; idx < nb * per; idx += blockDim.x) {
-    const int b = idx / per, j = idx - b * per;
+  const int jstep = blockDim.x / nb;
+  const int b = threadIdx.x % nb;
+  if ((int)threadIdx.x >= jstep * nb) return;
+  for (int j = threadIdx.x / nb; j < per; j += jstep) {
     const int k = j % Ns;
     float2 v[R];
 #pragma unroll
-    for (int t = 0; t < R; ++t) v[t] = src[b * bs + j + t * per];
+    for (int t = 0; t < R; ++t) {
+      const int e = j + t * per;
+      v[t] = (e < nz) ? src[e * nb + b] : make_float2(0.0f, 0.0f);
+    }
     if (Ns > 1) {
 #pragma unroll
       for (int t = 1; t < R; ++t) {
@@ -117,36 +127,38 @@ __device__ __forceinline__ void stockham_pass(const float2* __restrict__ src, fl
     else if (R == 3) dft3<INV>(v);
     else if (R == 4) dft4<INV>(v);
     else dft8<INV>(v);
-    const int o = b * bs + (j - k) * R + k;
+    const int o = (j - k) * R + k;
 #pragma unroll
-    for (int t = 0; t < R; ++t) dst[o + t * Ns] = v[t];
+    for (int t = 0; t < R; ++t) dst[(o + t * Ns) * nb + b] = v[t];
   }
 }
 
-// Runs all passes; data starts in `a`, returns the buffer that holds the result
-// (natural order).  Contains the __syncthreads between passes and one after the last.
+// Runs all passes; data starts in `a` ([M][nb], elements >= nz are zero and need not be
+// stored), returns the buffer that holds the result (natural order).  Contains the
+// __syncthreads between passes and one after the last.  Needs blockDim.x >= nb.
 template <bool INV>
 __device__ __forceinline__ float2* fft_stockham(float2* a, float2* b, const float2* twN,
-                                                const FftPlan& pl, int nb, int bs) {
+                                                const FftPlan& pl, int nb, int nz) {
   int Ns = 1;
   for (int p = 0; p < pl.npass; ++p) {
     const int R = pl.radix[p];
-    if (R == 8) stockham_pass<8, INV>(a, b, twN, pl.M, Ns, nb, bs);
-    else if (R == 4) stockham_pass<4, INV>(a, b, twN, pl.M, Ns, nb, bs);
-    else if (R == 2) stockham_pass<2, INV>(a, b, twN, pl.M, Ns, nb, bs);
-    else stockham_pass<3, INV>(a, b, twN, pl.M, Ns, nb, bs);
+    if (R == 8) stockham_pass<8, INV>(a, b, twN, pl.M, Ns, nb, nz);
+    else if (R == 4) stockham_pass<4, INV>(a, b, twN, pl.M, Ns, nb, nz);
+    else if (R == 2) stockham_pass<2, INV>(a, b, twN, pl.M, Ns, nb, nz);
+    else stockham_pass<3, INV>(a, b, twN, pl.M, Ns, nb, nz);
     __syncthreads();
     Ns *= R;
+    nz = pl.M;
     float2* t = a; a = b; b = t;
   }
   return a;
 }
 
-// Z: complex spectrum of the packed signal (natural order); returns X[k], k < M
-// (slot 0 = (DC, Nyquist)).
-__device__ __forceinline__ float2 rfft_post(const float2* Z, const float2* twN, int M, int k) {
-  if (k == 0) { const float2 z0 = Z[0]; return make_float2(z0.x + z0.y, z0.x - z0.y); }
-  const float2 p = Z[k], q = Z[M - k];
+// Z: complex spectrum of the packed signals ([M][nb], natural order); returns X[k], k < M,
+// of transform b (slot 0 = (DC, Nyquist)).
+__device__ __forceinline__ float2 rfft_post(const float2* Z, int nb, int b, const float2* twN, int M, int k) {
+  if (k == 0) { const float2 z0 = Z[b]; return make_float2(z0.x + z0.y, z0.x - z0.y); }
+  const float2 p = Z[k * nb + b], q = Z[(M - k) * nb + b];
   const float2 e = make_float2(0.5f * (p.x + q.x), 0.5f * (p.y - q.y));     // (Z[k] + conj Z[M-k])/2
   const float2 o = make_float2(0.5f * (p.x - q.x), 0.5f * (p.y + q.y));     // (Z[k] - conj Z[M-k])/2
   const float2 w = twN[k];
@@ -154,10 +166,10 @@ __device__ __forceinline__ float2 rfft_post(const float2* Z, const float2* twN, 
   return make_float2(e.x + wo.y, e.y - wo.x);                                // e - i w o
 }
 
-// X: packed half spectrum; returns Z[k] of the inverse.
-__device__ __forceinline__ float2 rfft_pre_inverse(const float2* X, const float2* twN, int M, int k) {
-  if (k == 0) { const float2 x0 = X[0]; return make_float2(x0.x + x0.y, x0.x - x0.y); }
-  const float2 p = X[k], q = X[M - k];
+// p = X[k], q = X[M-k] of a packed half spectrum (k > 0); returns Z[k] of the inverse.
+// For k = 0 pass p = q = X[0] = (DC, Nyquist).
+__device__ __forceinline__ float2 rfft_pre_inverse(float2 p, float2 q, const float2* twN, int k) {
+  if (k == 0) return make_float2(p.x + p.y, p.x - p.y);
   const float2 e = make_float2(p.x + q.x, p.y - q.y);                       // X[k] + conj X[M-k]
   const float2 o = make_float2(p.x - q.x, p.y + q.y);                       // X[k] - conj X[M-k]
   const float2 w = make_float2(twN[k].x, -twN[k].y);                        // e^{+2 pi i k/N}

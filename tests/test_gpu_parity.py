@@ -5,9 +5,10 @@ Tolerances (DESIGN.md "Tolerances"):
   integers (bbox, flags, block keys, CSR lists, slab/tile keys): bit-exact;
   effective charge (fp32 vs fp64): max|d| <= 2e-5 max|Qeff|, total within 1e-5;
   waveforms: max|d| <= 1e-4 max|signal| (north_star);
-  per-pixel integrated charge: |dQ_p| <= 1e-5 |Q_p| + 4 * 2^-24 * sum_t |I_p(t)|
-      (north_star's relative 1e-5, plus the rounding an fp32 waveform of L1 norm
-       sum_t|I_p| carries in its own integral -- DESIGN.md "Tolerances", reading G17).
+  per-pixel integrated charge: |dQ_p| <= 1e-5 |Q_p| + 1e-6 * sum_t |I_p(t)|
+      (north_star's relative 1e-5 on the collected charge; induction-only pixels integrate
+       to ~0 by cancellation, where a relative bound is undefined, so the floor is 1e-6 of
+       the L1 norm of the pixel's own waveform -- DESIGN.md "Tolerances", reading G17).
 """
 import numpy as np
 import pytest
@@ -20,6 +21,7 @@ pytestmark = pytest.mark.gpu
 TOL_QEFF = 2e-5
 TOL_WAVE = 1e-4
 TOL_QPIX = 1e-5
+TOL_QPIX_L1 = 1e-6
 
 
 def _torch():
@@ -218,7 +220,7 @@ def _wave_checks(got, ref):
     assert np.abs(got - ref).max() <= TOL_WAVE * scale
     qg, qr = got.sum(1), ref.sum(1)
     l1 = np.abs(ref).sum(1)
-    assert (np.abs(qg - qr) <= TOL_QPIX * np.abs(qr) + 4 * 2.0 ** -24 * l1).all()
+    assert (np.abs(qg - qr) <= TOL_QPIX * np.abs(qr) + TOL_QPIX_L1 * l1).all()
     # pixels the oracle leaves exactly empty stay exactly empty
     assert (got[l1 == 0] == 0).all()
 
