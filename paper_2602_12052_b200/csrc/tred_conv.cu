@@ -135,26 +135,33 @@ k_fill_blockmap(int64_t nblocks, const int64_t* __restrict__ keys, int32_t* __re
   if (i < nblocks) blockmap[keys[i]] = (int32_t)i;
 }
 
+// ------------------------------------------------------------------ twiddles
+__global__ void __launch_bounds__(256) k_fill_twiddles(float2* __restrict__ tw, int N) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < N) tw[k] = twiddle_N(k, N);
+}
+
 // ------------------------------------------------------------------ (a) forward FFT
 // One CTA per (charge pixel of the chunk, group of CG = JG*S fine columns).
-// qhat[f][row][phase], plane stride rp rows.
+// Shared buffers are [sample][column] (tred_fft.cuh).  qhat[f][row][phase], plane stride
+// rp rows.
 __global__ void __launch_bounds__(256)
 k_fft_fwd(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
           const int64_t* __restrict__ cp_keys, int r0, int nrows, int rp, int JG,
-          float2* __restrict__ qhat, TredGrid g, FftPlan pl) {
+          float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g, FftPlan pl) {
   extern __shared__ float2 sm[];
-  const int N = g.L, M = N >> 1, MS = M + 1;
+  const int N = g.L, M = N >> 1;
   const int CG = JG * g.S;
-  float2* A = sm;                   // [CG][MS]
-  float2* B = sm + CG * MS;         // [CG][MS]
-  float2* tw = sm + 2 * CG * MS;    // [N]
+  float2* A = sm;                   // [M][CG]
+  float2* B = sm + CG * M;          // [M][CG]
+  float2* tw = sm + 2 * CG * M;     // [N]
   __shared__ long long colbase[64];
   const int ngrp = (g.S + JG - 1) / JG;
   const int row = blockIdx.x / ngrp, grp = blockIdx.x - row * ngrp;
   const int64_t key = cp_keys[r0 + row];
   const int py = (int)(key % g.npy), px = (int)((key / g.npy) % g.npx);
   const int bt = (int)(key / ((int64_t)g.npy * g.npx));
-  fill_twiddles_N(tw, N);
+  load_twiddles_N(tw, gtw, N);
   if (threadIdx.x < CG) {
     const int jx = grp * JG + threadIdx.x / g.S, jy = threadIdx.x % g.S;
     long long base = -1;
@@ -167,21 +174,25 @@ k_fft_fwd(const float* __restrict__ payload, const int32_t* __restrict__ blockma
     colbase[threadIdx.x] = base;
   }
   __syncthreads();
-  const int hb = g.Bt >> 1;         // float2 samples per column
-  for (int i = threadIdx.x; i < CG * M; i += blockDim.x) {
-    const int c = i / M, m = i - c * M;
+  // 4 consecutive lanes read one 32-byte sector of a column; samples >= Bt/2 are the zero
+  // padding, which the first pass does not read
+  const int hb = g.Bt >> 1, hq = (hb + 3) >> 2;
+  for (int i = threadIdx.x; i < CG * hq * 4; i += blockDim.x) {
+    const int m4 = i & 3, rest = i >> 2;
+    const int c = rest % CG, m = (rest / CG) * 4 + m4;
+    if (m >= hb) continue;
     float2 v = make_float2(0.0f, 0.0f);
     const long long base = colbase[c];
-    if (m < hb && base >= 0) v = *reinterpret_cast<const float2*>(payload + base + 2 * m);
-    A[c * MS + m] = v;
+    if (base >= 0) v = *reinterpret_cast<const float2*>(payload + base + 2 * m);
+    A[m * CG + c] = v;
   }
   __syncthreads();
-  const float2* Z = fft_stockham<false>(A, B, tw, pl, CG, MS);
+  const float2* Z = fft_stockham<false>(A, B, tw, pl, CG, hb);
   const int jbase = grp * CG;
   const int ncol = min(CG, g.nph - jbase);
   for (int i = threadIdx.x; i < M * CG; i += blockDim.x) {
     const int f = i / CG, c = i - f * CG;
-    if (c < ncol) qhat[((int64_t)f * rp + row) * g.nph + jbase + c] = rfft_post(Z + c * MS, tw, M, f);
+    if (c < ncol) qhat[((int64_t)f * rp + row) * g.nph + jbase + c] = rfft_post(Z, CG, c, tw, M, f);
   }
 }
 
@@ -320,36 +331,44 @@ k_accum(const float2* __restrict__ T, const int64_t* __restrict__ sp_keys, int s
 }
 
 // ------------------------------------------------------------------ (d) inverse FFT
-// One CTA per IP slab pixels; sp_data[sp][n_over*Bt].
+// One CTA per IP slab pixels ([sample][pixel] in shared memory); sp_data[sp][n_over*Bt].
+// Lanes: pixel fastest, 4 consecutive samples per pixel -> full 32-byte sectors in HBM,
+// contiguous shared-memory rows.
 __global__ void __launch_bounds__(256)
 k_ifft(const float2* __restrict__ ohat, int s0, int ns, int sbase, float* __restrict__ sp_data,
-       TredGrid g, FftPlan pl, int IP, int out_len) {
+       const float2* __restrict__ gtw, TredGrid g, FftPlan pl, int IP, int out_len) {
   extern __shared__ float2 sm[];
-  const int N = g.L, M = N >> 1, MS = M + 1;
-  float2* A = sm;                   // [IP][MS]
-  float2* B = sm + IP * MS;         // [IP][MS]
-  float2* tw = sm + 2 * IP * MS;    // [N]
+  const int N = g.L, M = N >> 1;
+  float2* A = sm;                   // [M][IP]
+  float2* B = sm + IP * M;          // [M][IP]
+  float2* tw = sm + 2 * IP * M;     // [N]
   const int a0 = blockIdx.x * IP;
-  fill_twiddles_N(tw, N);
-  for (int i = threadIdx.x; i < IP * M; i += blockDim.x) {
-    const int c = i / M, k = i - c * M;
-    B[c * MS + k] = (a0 + c < ns) ? ohat[(int64_t)(s0 + a0 + c - sbase) * M + k] : make_float2(0.0f, 0.0f);
+  load_twiddles_N(tw, gtw, N);
+  __syncthreads();
+  const int mq = (M + 3) >> 2;
+  for (int i = threadIdx.x; i < IP * mq * 4; i += blockDim.x) {
+    const int k4 = i & 3, rest = i >> 2;
+    const int c = rest % IP, k = (rest / IP) * 4 + k4;
+    if (k >= M) continue;
+    float2 z = make_float2(0.0f, 0.0f);
+    if (a0 + c < ns) {
+      const float2* X = ohat + (int64_t)(s0 + a0 + c - sbase) * M;
+      const float2 p = X[k], q = X[k ? M - k : 0];
+      z = rfft_pre_inverse(p, q, tw, k);
+    }
+    A[k * IP + c] = z;
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < IP * M; i += blockDim.x) {
-    const int c = i / M, k = i - c * M;
-    A[c * MS + k] = rfft_pre_inverse(B + c * MS, tw, M, k);
-  }
-  __syncthreads();
-  const float2* Z = fft_stockham<true>(A, B, tw, pl, IP, MS);
-  const int row = g.nover * g.Bt, hrow = row >> 1;
+  const float2* Z = fft_stockham<true>(A, B, tw, pl, IP, M);
+  const int row = g.nover * g.Bt, hrow = row >> 1, hq = (hrow + 3) >> 2;
   const float sc = 1.0f / (float)N;
-  for (int i = threadIdx.x; i < IP * hrow; i += blockDim.x) {
-    const int c = i / hrow, m = i - c * hrow;
-    if (a0 + c >= ns) continue;
+  for (int i = threadIdx.x; i < IP * hq * 4; i += blockDim.x) {
+    const int m4 = i & 3, rest = i >> 2;
+    const int c = rest % IP, m = (rest / IP) * 4 + m4;
+    if (m >= hrow || a0 + c >= ns) continue;
     float2 v = make_float2(0.0f, 0.0f);
     if (m < M) {
-      const float2 z = Z[c * MS + m];
+      const float2 z = Z[m * IP + c];
       v.x = (2 * m < out_len) ? z.x * sc : 0.0f;
       v.y = (2 * m + 1 < out_len) ? z.y * sc : 0.0f;
     }
@@ -413,7 +432,7 @@ static PlanWork carve_plan(const tred_ctx* c, void* base) {
 }
 
 struct ConvWork {
-  int32_t* blockmap; float2* ohat; float2* qhat; float2* T;
+  int32_t* blockmap; float2* tw; float2* ohat; float2* qhat; float2* T;
   size_t total;
 };
 
@@ -428,6 +447,7 @@ static ConvWork carve_conv(const tred_ctx* c, void* base, int64_t rows, int64_t 
   if (nsp < 1) nsp = 1;
   const int64_t rp = pad_rows(rows);
   w.blockmap = (int32_t*)take((size_t)(d.NB[0] * d.NB[1] * d.NB[2]) * 4);
+  w.tw = (float2*)take((size_t)d.fft_len * 8);
   w.ohat = (float2*)take((size_t)nsp * d.n_freq * 8);
   w.qhat = (float2*)take((size_t)d.n_freq * rp * d.n_phase * 8);
   w.T = (float2*)take((size_t)d.n_freq * d.n_off_pad * rp * 8);
@@ -526,17 +546,17 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
   const PlanWork pw = carve_plan(ctx, (void*)d_plan_work);
   FftPlan pl;
   if (!tred_make_fft_plan(g.L / 2, &pl)) return TRED_EUNSUPPORTED;
-  const int M = g.L / 2, MS = M + 1;
+  const int M = g.L / 2;
 
   // forward FFT: CG = JG*S columns per CTA, two ping-pong buffers + twiddles
   int JG = g.S;
-  auto fwd_smem = [&](int jg) { return (size_t)(2 * jg * g.S * MS + g.L) * sizeof(float2); };
+  auto fwd_smem = [&](int jg) { return (size_t)(2 * jg * g.S * M + g.L) * sizeof(float2); };
   while (JG > 1 && (fwd_smem(JG) > 100 * 1024 || JG * g.S > 64)) --JG;
   if (fwd_smem(JG) > (size_t)ctx->smem_optin || JG * g.S > 64) return TRED_EUNSUPPORTED;
   const int ngrp = (g.S + JG - 1) / JG;
   TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fwd_smem(JG)));
   int IP = 8;
-  auto inv_smem = [&](int ip) { return (size_t)(2 * ip * MS + g.L) * sizeof(float2); };
+  auto inv_smem = [&](int ip) { return (size_t)(2 * ip * M + g.L) * sizeof(float2); };
   while (IP > 1 && inv_smem(IP) > 64 * 1024) IP /= 2;
   if (inv_smem(IP) > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
   TRED_CUDA(cudaFuncSetAttribute(k_ifft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)inv_smem(IP)));
@@ -552,7 +572,8 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
     TredProfScope ps(ctx, ST_MISC, st);
     TRED_CUDA(cudaMemsetAsync(w0.blockmap, 0xff, nbtot * 4, st));
     k_fill_blockmap<<<cdiv(nblocks, 256), 256, 0, st>>>(nblocks, d_keys, w0.blockmap);
-    TRED_COUNT_LAUNCH(2);
+    k_fill_twiddles<<<cdiv(g.L, 256), 256, 0, st>>>(w0.tw, g.L);
+    TRED_COUNT_LAUNCH(3);
   }
   const float* Wf = d_rhat;
   const int64_t wfl = d.rhat_floats / 10 * 2, bfl = d.rhat_floats / 10 * 4;
@@ -586,7 +607,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         k_fft_fwd<<<(unsigned)(nr * ngrp), 256, fwd_smem(JG), st>>>(d_payload, w.blockmap, d_cp_keys, r0, nr, rp,
-                                                                  JG, w.qhat, g, pl);
+                                                                  JG, w.qhat, w.tw, g, pl);
         TRED_COUNT_LAUNCH(1);
       }
       {
@@ -622,7 +643,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
     }
     {
       TredProfScope ps(ctx, ST_IFFT, st);
-      k_ifft<<<cdiv(nsb, IP), 256, inv_smem(IP), st>>>(w.ohat, sbase, nsb, sbase, d_sp_data, g, pl, IP, d.out_len);
+      k_ifft<<<cdiv(nsb, IP), 256, inv_smem(IP), st>>>(w.ohat, sbase, nsb, sbase, d_sp_data, w.tw, g, pl, IP, d.out_len);
       TRED_COUNT_LAUNCH(1);
     }
     TRED_LAUNCH_CHECK("convolve ifft");
