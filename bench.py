@@ -4,11 +4,14 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
 
 A "step" is one pass of the whole hot path (tred_drift, tred_blockbin, tred_effq,
-tred_convolve_plan, tred_convolve, tred_gather_waveforms) over one synthetic event.
-N = 1 workload: BASELINE.json configs[1] (one neutrino-like event, ~14k 1-mm segments,
-128x128 pixels x 4096 ticks, 3-point Gauss-Legendre, blocks 8x8x64, response 11x11 x 100
-phases x 400 ticks).  N > 1: every rank simulates its own event of the same recipe (seed
-1002 + rank): the path shards over independent events with no collective ("weak").
+tred_convolve_plan, tred_convolve, tred_gather_waveforms) over one synthetic spill.
+N = 1 workload: BASELINE.json's third config, the full beam spill in one module that the
+metric "ms per spill" is quoted on (~0.93 M 1-mm segments, 230x230 pixels x 5000 ticks,
+4-point Gauss-Legendre, blocks 16x16x128, response 11x11 x 100 phases x 400 ticks); it fits
+one GPU (56 GB).  `--config 1|2|4` select the other workloads, `--config 5` the
+representation sweep with the dense-grid comparison.  N > 1: every rank simulates its own
+spill of the same recipe (seed 1003 + rank): the path shards over independent events with
+no collective ("weak").
 `--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample instead.
 """
 from __future__ import annotations
@@ -41,7 +44,8 @@ def _env_int(k, d):
 
 
 def workload(cfg_id: int, rank: int):
-    cfg, segs = gen.make_segments(cfg_id, seed=1000 + cfg_id + rank)
+    from paper_2602_12052_b200.shard import event_seed
+    cfg, segs = gen.make_segments(cfg_id, seed=event_seed(cfg_id, rank))
     R = gen.make_response(cfg, 2000 + cfg_id)
     seg = np.ascontiguousarray(np.stack([segs[k] for k in gen.SEG_FIELDS]).astype(np.float32))
     return cfg, segs, seg, R
@@ -99,6 +103,21 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def _load_traffic(workload_name: str) -> dict:
+    """DRAM bytes per step and stage from the committed ncu --set full capture
+    (profiles/traffic.csv: workload,stage,dram_bytes_per_step); {} if there is none."""
+    out = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                p = [x.strip() for x in line.split(",")]
+                if len(p) >= 3 and p[0] == workload_name:
+                    out[p[1]] = float(p[2])
+    except (OSError, ValueError):
+        pass
+    return out
+
+
 # --------------------------------------------------------------------------- oracle legs
 def oracle_sample(cfg, segs, R, n_sample: int):
     """The oracle as it stands on the first n_sample segments: whole path, every pixel of
@@ -116,12 +135,19 @@ def oracle_sample(cfg, segs, R, n_sample: int):
     return len(sub["q"]), dt, os.cpu_count()
 
 
+REF_SEGMENTS = {1: 60, 2: 40, 3: 8, 4: 8}      # ~20 s of oracle work on 8-16 host cores
+
+
+def _ref_segments(args):
+    return args.ref_segments or REF_SEGMENTS.get(args.config, 8)
+
+
 def run_reference(args):
     rank = _env_int("RANK", 0)
     if rank != 0:
         return 0
     cfg, segs, seg, R = workload(args.config, 0)
-    n_sample = args.ref_segments
+    n_sample = _ref_segments(args)
     for _ in range(args.warmup and 1):
         oracle_sample(cfg, segs, R, max(2, n_sample // 8))
     times = []
@@ -202,12 +228,14 @@ def run_cuda(args):
 
     # ---- timed region 2: per-stage events (roofline of the dominant kernel)
     stage_ms = {}
+    stage_prof_last = {}
     for _ in range(args.steps):
         flush.zero_()
         sim.profile_begin(events=True)
         sim.simulate(seg_d, rhat)
         torch.cuda.synchronize()
-        for k, (m, n) in sim.profile_end().items():
+        stage_prof_last = sim.profile_end()
+        for k, (m, n) in stage_prof_last.items():
             stage_ms[k] = stage_ms.get(k, 0.0) + m / args.steps
     barrier()
 
@@ -230,14 +258,9 @@ def run_cuda(args):
     e2e = float(np.mean(e2e_ms))
     barrier()
 
-    # ---- max over ranks
-    t = torch.tensor([ms, e2e], dtype=torch.float64, device=dev)
-    n_all = torch.tensor([float(nseg)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(n_all, op=dist.ReduceOp.SUM)
-    ms_max, e2e_max = float(t[0]), float(t[1])
-    total_seg = float(n_all[0])
+    # ---- max over ranks of the times, sum of the units (paper_2602_12052_b200/shard.py)
+    from paper_2602_12052_b200.shard import reduce_timing
+    (ms_max, e2e_max), total_seg = reduce_timing([ms, e2e], nseg, device=dev)
 
     if rank == 0:
         d = sim.dims
@@ -246,32 +269,49 @@ def run_cuda(args):
             peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
         except Exception:
             pass
-        # dominant kernel and its roofline
-        dom = max(stage_ms, key=stage_ms.get)
+        # per-stage rooflines: algorithmic work of the METHOD per step
+        # / CUDA-event time of the stage, against the measured peaks
         nb = info["nblocks"]
         ncols = cfg.block[0] * cfg.block[1]
         K = 2 * cfg.resp_half + 1
-        nf = d.n_freq
+        nf, L = d.n_freq, d.fft_len
         sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
-        alu_peak = 148 * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12          # TFLOP/s at max clock
-        roof = {"kernel": dom, "ms": stage_ms[dom]}
-        if dom == "mac":
-            flops = nb * ncols * K * K * (8.0 * (nf - 1) + 4.0)
-            roof.update(bound="alu", achieved=flops / (stage_ms[dom] * 1e-3) / 1e12, peak=alu_peak,
-                        unit="TFLOP/s", traffic=None,
-                        note="fp32 FMA pipe; peak = 148 SM x 128 lanes x 2 x sm_max_mhz (derived, DESIGN.md)")
-        elif dom == "effq":
-            # algorithmic work: one Eq. (10) evaluation per node = EFFQ_INSTR_PER_NODE fp32
-            # lane-instructions; peak = lane-instructions/s of the SMs
-            ipn = 40.0
-            roof.update(bound="alu", achieved=info["gl_nodes"] * ipn / (stage_ms[dom] * 1e-3) / 1e12,
-                        peak=148 * FMA_LANES_PER_SM * sm_max * 1e6 / 1e12, unit="Tinstr/s", traffic=None,
-                        note=f"{ipn:.0f} fp32 lane-instructions per node (derived, DESIGN.md)")
-        else:
-            hbm = peaks.get("hbm_gbs", 6650.0)
-            roof.update(bound="hbm", achieved=None, peak=hbm, unit="GB/s", traffic=None)
-        if roof.get("achieved") is not None:
-            roof["frac"] = roof["achieved"] / roof["peak"]
+        hbm = peaks.get("hbm_gbs", 6650.0)
+        hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650"
+        alu_peak = 148 * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12          # fp32 TFLOP/s at max clock
+        tf32_peak = peaks.get("bf16_tflops", 1590.0) * 0.5                     # guide: tf32 = bf16 / 2 nominal
+        fftf = 2.5 * L * np.log2(L)                                            # flops of one real FFT of length L
+        payload_b = nb * d.block_floats * 4.0
+        spd_b = info["nsp"] * d.n_over * cfg.block[2] * 4.0
+        work = {
+            "effq": ("hbm", payload_b + nseg * 104.0),
+            "fft_fwd": ("alu", nb * ncols * fftf),
+            "mac": ("tensor" if sim.cfg.mac_mode != 1 else "alu", nb * ncols * K * K * (8.0 * (nf - 1) + 4.0)),
+            "accum": ("hbm", info["nsp"] * nf * 8.0),
+            "ifft": ("alu", info["nsp"] * fftf),
+            "gather": ("hbm", spd_b + info["ntiles"] * cfg.block[2] * 4.0),
+        }
+        pk = {"hbm": (hbm, "GB/s", 1e9, hbm_src),
+              "alu": (alu_peak, "TFLOP/s", 1e12, "derived: 148 SM x 128 lanes x 2 x sm_max_mhz (DESIGN.md)"),
+              "tensor": (tf32_peak, "TFLOP/s", 1e12,
+                         "tf32 dense = measured bf16_tflops x 1/2 (nominal ratio); the kernel executes "
+                         "3 tf32 products per algorithmic fp32 product (3xTF32), so 1/3 is its ceiling")}
+        nlaunch = {k: v[1] for k, v in stage_prof_last.items()}
+        traffic = _load_traffic(cfg.name)
+        stage_roof = {}
+        for k, (bound, w) in work.items():
+            if stage_ms.get(k, 0.0) <= 0:
+                continue
+            peak, unit, sc, src = pk[bound]
+            nl = max(nlaunch.get(k, 1), 1)
+            ach = w / (stage_ms[k] * 1e-3) / sc
+            tr = traffic.get(k)
+            stage_roof[k] = {"kernel": k, "bound": bound, "achieved": ach, "peak": peak, "unit": unit,
+                             "frac": ach / peak, "ms_per_launch": stage_ms[k] / nl, "launches_per_step": nl,
+                             "work_per_launch": w / nl, "peak_source": src,
+                             "traffic": (tr / nl) if tr else None}
+        dom = max(stage_roof, key=lambda k: stage_ms[k])
+        roof = dict(stage_roof[dom])
         payload_gb = nb * d.block_floats * 4 / 1e9
         line = {"metric": METRIC, "value": total_seg / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_max,
@@ -288,11 +328,15 @@ def run_cuda(args):
                 "clocks": clocks,
                 "stage_ms": {k: round(v, 4) for k, v in stage_ms.items() if v > 0},
                 "roofline": roof,
+                "stage_roofline": {k: {kk: (round(vv, 6) if isinstance(vv, float) else vv)
+                                       for kk, vv in v.items() if kk in ("bound", "achieved", "peak", "unit", "frac",
+                                                                          "traffic")}
+                                   for k, v in stage_roof.items()},
                 "peak_mem_gb": torch.cuda.max_memory_allocated(dev) / 1e9,
                 "payload_gb": payload_gb,
                 "wall_s_timed_region": t_wall}
         if not args.no_cpu_baseline and world == 1:
-            n, dt, cores = oracle_sample(cfg, segs, R, args.ref_segments)
+            n, dt, cores = oracle_sample(cfg, segs, R, _ref_segments(args))
             line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"first {n} segments of config {args.config}, whole path, "
                                               f"all pixels of their footprint ({dt:.1f} s)"}
@@ -307,9 +351,9 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--ref-segments", type=int, default=40)
+    ap.add_argument("--ref-segments", type=int, default=0, help="oracle sample size (0 = per config)")
     ap.add_argument("--work-gb", type=int, default=0, help="tred_convolve workspace cap (GiB), 0 = default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

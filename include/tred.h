@@ -68,8 +68,11 @@ typedef struct tred_config {
                                     0 = factored line integral (default, see tred_effq),
                                     1 = closed form with erf per Gauss-Legendre node          */
   int32_t mac_mode;              /* spectrum multiply-accumulate of tred_convolve:
-                                    0 = default (tensor cores, 3xTF32, if supported),
-                                    1 = fp32 FMA pipe, 2 = tensor cores 3xTF32              */
+                                    0 = default: tensor cores (3xTF32) over row tiles with
+                                        the sum over the offsets fused into the epilogue,
+                                        if supported, else as 2, else as 1,
+                                    1 = fp32 FMA pipe, products written to memory,
+                                    2 = tensor cores 3xTF32, products written to memory       */
 } tred_config;
 
 /* Sizes derived from a configuration (host-side helper, no device work). */
@@ -179,6 +182,9 @@ int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* d_rhat, voi
  *   d_cp_keys   [cap_cp] int64 out, d_cp_off [NBt+1] int32 out (first index per slab), d_ncp
  *   d_sp_keys   [cap_sp] int64 out, d_sp_off [NBt+1] int32 out, d_nsp
  *   d_tile_keys [cap_tiles] int64 out, d_ntiles
+ *   d_rt_off    [NBt+1] int32 out: first row tile of every slab (row tiles: runs of at most
+ *               128 charge pixels of one slab and one 8-pixel-wide strip, the unit the
+ *               tensor-core spectrum product works on; slot NBt = their number)
  *   d_plan_work at least tred_plan_work_bytes() bytes; its content (the index maps) is
  *               read again by tred_convolve and tred_gather_waveforms.
  */
@@ -187,6 +193,7 @@ int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
                        int64_t cap_cp, int64_t* d_cp_keys, int32_t* d_cp_off, int64_t* d_ncp,
                        int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
                        int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
+                       int32_t* d_rt_off,
                        void* d_plan_work, size_t plan_work_bytes, void* stream);
 
 /*
@@ -201,6 +208,7 @@ int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
  * the chunking (bit-identical).
  *   h_cp_off   [NBt+1] HOST copy of tred_convolve_plan's d_cp_off
  *   h_sp_off   [NBt+1] HOST copy of d_sp_off
+ *   h_rt_off   [NBt+1] HOST copy of d_rt_off
  *   d_sp_data  [nsp][n_over*Bt] float32 out: current of (slab bt, pixel) from tick Bt*bt
  *   d_work     at least tred_convolve_work_bytes(min_rows) bytes with min_rows >= 1; more
  *              rows per chunk make larger launches.
@@ -210,6 +218,7 @@ int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys, const f
                   const float* d_rhat,
                   int64_t ncp, const int64_t* d_cp_keys, const int32_t* h_cp_off,
                   int64_t nsp, const int64_t* d_sp_keys, const int32_t* h_sp_off,
+                  const int32_t* h_rt_off,
                   const void* d_plan_work, float* d_sp_data,
                   void* d_work, size_t work_bytes, void* stream);
 

@@ -64,11 +64,13 @@ EXPORTS = {
                                      _c_i64, _c_p, _c_p, _c_p,
                                      _c_i64, _c_p, _c_p, _c_p,
                                      _c_i64, _c_p, _c_p,
+                                     _c_p,
                                      _c_p, C.c_size_t, _c_p]),
     "tred_convolve_work_bytes": (C.c_size_t, [_c_p, _c_i64, _c_i64]),
     "tred_convolve": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p,
                                 _c_i64, _c_p, _c_p,
                                 _c_i64, _c_p, _c_p,
+                                _c_p,
                                 _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p,
                                         _c_p]),
@@ -267,18 +269,20 @@ class Tred:
                  ncp=self._empty((1,), t.int64),
                  sp_keys=self._empty((max(cap_sp, 1),), t.int64), sp_off=self._empty((NBt + 1,), t.int32),
                  nsp=self._empty((1,), t.int64),
-                 tile_keys=self._empty((max(cap_tiles, 1),), t.int64), ntiles=self._empty((1,), t.int64))
+                 tile_keys=self._empty((max(cap_tiles, 1),), t.int64), ntiles=self._empty((1,), t.int64),
+                 rt_off=self._empty((NBt + 1,), t.int32))
         pw = self.L.tred_plan_work_bytes(self.h)
         p["work"] = self._empty((pw,), t.uint8)
         _check(self.L.tred_convolve_plan(self.h, nblocks, _ptr(keys),
                                          cap_cp, _ptr(p["cp_keys"]), _ptr(p["cp_off"]), _ptr(p["ncp"]),
                                          cap_sp, _ptr(p["sp_keys"]), _ptr(p["sp_off"]), _ptr(p["nsp"]),
                                          cap_tiles, _ptr(p["tile_keys"]), _ptr(p["ntiles"]),
+                                         _ptr(p["rt_off"]),
                                          _ptr(p["work"]), p["work"].numel(), self._stream()), "tred_convolve_plan")
         return p
 
     def convolve(self, nblocks: int, keys, payload, rhat, plan: dict, ncp: int, nsp: int,
-                 cp_off_host, sp_off_host, sp_data=None, work_bytes: int | None = None):
+                 cp_off_host, sp_off_host, sp_data=None, work_bytes: int | None = None, rt_off_host=None):
         t = self.torch
         import numpy as np
         row = self.dims.n_over * self.cfg.block[2]
@@ -286,6 +290,9 @@ class Tred:
             sp_data = self._empty((max(nsp, 1), row), t.float32)
         co = np.ascontiguousarray(cp_off_host, dtype=np.int32)
         po = np.ascontiguousarray(sp_off_host, dtype=np.int32)
+        if rt_off_host is None:
+            rt_off_host = plan["rt_off"].cpu().numpy()
+        ro = np.ascontiguousarray(rt_off_host, dtype=np.int32)
         ns_max = int(np.diff(po).max()) if len(po) > 1 else 0
         need = self.L.tred_convolve_work_bytes(self.h, 128, ns_max)
         if work_bytes is None:
@@ -297,6 +304,7 @@ class Tred:
         _check(self.L.tred_convolve(self.h, nblocks, _ptr(keys), _ptr(payload), _ptr(rhat),
                                     ncp, _ptr(plan["cp_keys"]), co.ctypes.data_as(_c_p),
                                     nsp, _ptr(plan["sp_keys"]), po.ctypes.data_as(_c_p),
+                                    ro.ctypes.data_as(_c_p),
                                     _ptr(plan["work"]), _ptr(sp_data), _ptr(work), work.numel(), self._stream()),
                "tred_convolve")
         return sp_data
@@ -329,11 +337,11 @@ class Tred:
         payload = self.effq(nblocks, keys, blk_off, pair_seg, augf, augi)
         plan = self.convolve_plan(nblocks, keys)
         counts = t.cat([plan["ncp"], plan["nsp"], plan["ntiles"], plan["cp_off"].to(t.int64),
-                        plan["sp_off"].to(t.int64)]).cpu().numpy()
+                        plan["sp_off"].to(t.int64), plan["rt_off"].to(t.int64)]).cpu().numpy()
         ncp, nsp, ntiles = int(counts[0]), int(counts[1]), int(counts[2])
         NBt = int(self.dims.NB[2])
-        co, po = counts[3:3 + NBt + 1], counts[3 + NBt + 1:]
-        sp_data = self.convolve(nblocks, keys, payload, rhat, plan, ncp, nsp, co, po)
+        co, po, ro = (counts[3 + i * (NBt + 1):3 + (i + 1) * (NBt + 1)] for i in range(3))
+        sp_data = self.convolve(nblocks, keys, payload, rhat, plan, ncp, nsp, co, po, rt_off_host=ro)
         tile_data, dense = self.gather_waveforms(nsp, sp_data, plan, ntiles, pix_ids)
         tile_keys, sp_keys, sp_off = plan["tile_keys"], plan["sp_keys"], plan["sp_off"]
         out = dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ncp=ncp, nsp=nsp, ntiles=ntiles,

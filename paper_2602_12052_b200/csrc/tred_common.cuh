@@ -81,6 +81,15 @@ void tred_set_cuda_error(cudaError_t e, const char* where);
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
+// ---- row tiles of the tensor-core convolution path (tred_conv.cu, tred_mac_tc.cu) ----
+constexpr int RT_SW = 8;         // strip width in pixels
+constexpr int RT_ROWS = 128;     // rows per tile = MMA M
+constexpr int RT_PY = 64;        // patch height (py) in global memory
+constexpr int RT_PYS = 66;       // patch row stride in shared memory (66 = 2 mod 16: conflict-free)
+constexpr int RT_MAXH = 5;       // largest response half-width the patch buffers hold
+constexpr int RT_PXMAX = RT_SW + 2 * RT_MAXH;
+
+
 // ---- S2 variants (tred_effq.cu: closed form; tred_effq_fact.cu: factored, dispatch) ---
 int tred_effq_closed_form(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
                           const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,

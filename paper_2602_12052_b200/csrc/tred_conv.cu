@@ -135,6 +135,115 @@ k_fill_blockmap(int64_t nblocks, const int64_t* __restrict__ keys, int32_t* __re
   if (i < nblocks) blockmap[keys[i]] = (int32_t)i;
 }
 
+// ------------------------------------------------------------------ row tiles
+// The tensor-core path orders the charge pixels of a slab by (strip = px / 8, py, px % 8)
+// and cuts every (slab, strip) sequence into row tiles of at most RT_ROWS rows made of
+// whole py-lines, at most RT_PY - 2H lines tall.  The outputs of a row tile then fall in
+// the patch [8 strip - H, 8 strip + 7 + H] x [py0 - H, py0 + ny - 1 + H], small enough to
+// be summed over the offsets in shared memory by the GEMM epilogue.
+struct RtGeom { int nstrip, ngrp, capy; int64_t nmap2, cap_rt; };
+
+static inline RtGeom rt_geom(const tred_ctx* c) {
+  RtGeom r;
+  r.nstrip = (c->cfg.npix_x + RT_SW - 1) / RT_SW;
+  r.ngrp = (int)c->dims.NB[2] * r.nstrip;
+  r.capy = RT_PY - 2 * c->cfg.resp_half;
+  if (r.capy < 1) r.capy = 1;
+  r.nmap2 = (int64_t)r.ngrp * c->cfg.npix_y * RT_SW;
+  const int npy = c->cfg.npix_y;
+  r.cap_rt = (int64_t)r.ngrp * ((npy * RT_SW + RT_ROWS - RT_SW) / (RT_ROWS - RT_SW + 1) + (npy + r.capy - 1) / r.capy + 1);
+  return r;
+}
+
+// occupancy flags in strip order: m2 = ((bt * nstrip + strip) * npy + py) * 8 + px % 8
+__global__ void __launch_bounds__(256)
+k_rt_flags(int64_t nmap2, const int32_t* __restrict__ cp_idx, int32_t* __restrict__ ridx, int nstrip, TredGrid g) {
+  const int64_t m2 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m2 > nmap2) return;
+  int v = 0;
+  if (m2 < nmap2) {
+    const int xl = (int)(m2 & (RT_SW - 1));
+    const int64_t rest = m2 >> 3;
+    const int py = (int)(rest % g.npy);
+    const int64_t grp = rest / g.npy;
+    const int strip = (int)(grp % nstrip), bt = (int)(grp / nstrip);
+    const int px = strip * RT_SW + xl;
+    if (px < g.npx) {
+      const int64_t m = ((int64_t)bt * g.npx + px) * g.npy + py;
+      v = cp_idx[m + 1] != cp_idx[m];
+    }
+  }
+  ridx[m2] = v;
+}
+
+__global__ void __launch_bounds__(256)
+k_rt_rows(int64_t nmap2, const int32_t* __restrict__ ridx, int32_t* __restrict__ row_m2) {
+  const int64_t m2 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m2 >= nmap2) return;
+  const int r = ridx[m2];
+  if (ridx[m2 + 1] != r) row_m2[r] = (int32_t)m2;
+}
+
+// One thread per (slab, strip): greedy cut into row tiles.  WRITE = false counts them.
+template <bool WRITE>
+__global__ void __launch_bounds__(128)
+k_rt_tiles(int ngrp, int npy, int capy, const int32_t* __restrict__ ridx, int32_t* __restrict__ cnt,
+           const int32_t* __restrict__ off, int4* __restrict__ desc, int64_t cap_rt) {
+  const int grp = blockIdx.x * blockDim.x + threadIdx.x;
+  if (grp >= ngrp) return;
+  const int32_t* line = ridx + (int64_t)grp * npy * RT_SW;      // line[py * 8] = first row of the line
+  int t = WRITE ? off[grp] : 0;
+  int py = 0;
+  while (py < npy) {
+    if (line[(py + 1) * RT_SW] == line[py * RT_SW]) { ++py; continue; }
+    const int py0 = py, row0 = line[py * RT_SW];
+    int rows = 0, last = py;
+    while (py < npy && py - py0 < capy) {
+      const int c = line[(py + 1) * RT_SW] - line[py * RT_SW];
+      if (rows + c > RT_ROWS) break;
+      if (c > 0) last = py;
+      rows += c;
+      ++py;
+    }
+    if (WRITE && t < cap_rt) desc[t] = make_int4(row0, rows, py0, last - py0 + 1);
+    ++t;
+  }
+  if (!WRITE) cnt[grp] = t;
+}
+
+// first row tile of every slab (and the total in slot NBt)
+__global__ void k_rt_slab_off(int NBt, int nstrip, const int32_t* __restrict__ off, int32_t* __restrict__ rt_off) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i <= NBt) rt_off[i] = off[i * nstrip];
+}
+
+// Where the forward FFT finds the charge pixel of the row a CTA works on: the sorted
+// charge-pixel list (row = index from r0), or the row tiles (row = padded row of the
+// chunk, 128 per tile; rows beyond the tile's count do not exist).
+struct RowSrc {
+  const int64_t* cp_keys; int r0;
+  const int4* rt_desc; const int32_t* row_m2; int t0, nstrip, tiled;
+};
+
+__device__ __forceinline__ bool row_pixel(const RowSrc& rs, int row, const TredGrid& g, int& px, int& py, int& bt) {
+  if (!rs.tiled) {
+    const int64_t key = rs.cp_keys[rs.r0 + row];
+    py = (int)(key % g.npy); px = (int)((key / g.npy) % g.npx);
+    bt = (int)(key / ((int64_t)g.npy * g.npx));
+    return true;
+  }
+  const int4 d = rs.rt_desc[rs.t0 + (row >> 7)];
+  const int r = row & (RT_ROWS - 1);
+  if (r >= d.y) return false;
+  const int m2 = rs.row_m2[d.x + r];
+  const int rest = m2 >> 3;
+  py = rest % g.npy;
+  const int grp = rest / g.npy;
+  bt = grp / rs.nstrip;
+  px = (grp - bt * rs.nstrip) * RT_SW + (m2 & (RT_SW - 1));
+  return true;
+}
+
 // ------------------------------------------------------------------ twiddles
 __global__ void __launch_bounds__(256) k_fill_twiddles(float2* __restrict__ tw, int N) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -147,7 +256,7 @@ __global__ void __launch_bounds__(256) k_fill_twiddles(float2* __restrict__ tw, 
 // rp rows.
 __global__ void __launch_bounds__(256)
 k_fft_fwd(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
-          const int64_t* __restrict__ cp_keys, int r0, int nrows, int rp, int JG,
+          RowSrc rs, int rp, int JG,
           float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g, FftPlan pl) {
   extern __shared__ float2 sm[];
   const int N = g.L, M = N >> 1;
@@ -158,9 +267,8 @@ k_fft_fwd(const float* __restrict__ payload, const int32_t* __restrict__ blockma
   __shared__ long long colbase[64];
   const int ngrp = (g.S + JG - 1) / JG;
   const int row = blockIdx.x / ngrp, grp = blockIdx.x - row * ngrp;
-  const int64_t key = cp_keys[r0 + row];
-  const int py = (int)(key % g.npy), px = (int)((key / g.npy) % g.npx);
-  const int bt = (int)(key / ((int64_t)g.npy * g.npx));
+  int px, py, bt;
+  if (!row_pixel(rs, row, g, px, py, bt)) return;
   load_twiddles_N(tw, gtw, N);
   if (threadIdx.x < CG) {
     const int jx = grp * JG + threadIdx.x / g.S, jy = threadIdx.x % g.S;
@@ -193,6 +301,53 @@ k_fft_fwd(const float* __restrict__ payload, const int32_t* __restrict__ blockma
   for (int i = threadIdx.x; i < M * CG; i += blockDim.x) {
     const int f = i / CG, c = i - f * CG;
     if (c < ncol) qhat[((int64_t)f * rp + row) * g.nph + jbase + c] = rfft_post(Z, CG, c, tw, M, f);
+  }
+}
+
+// Same kernel with the length M = L/2 and the CG = 20 columns per CTA (S = 10, JG = 2) as
+// compile-time constants (tred_fft.cuh, fft_stockham_ct): no runtime divisions.
+template <int M>
+__global__ void __launch_bounds__(256)
+k_fft_fwd_ct(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
+             RowSrc rs, int rp,
+             float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g) {
+  extern __shared__ float2 sm[];
+  constexpr int N = 2 * M, CG = 20, S = 10, JG = 2, NGRP = 5, NPH = 100;
+  float2* A = sm;                   // [M][CG]
+  float2* B = sm + CG * M;          // [M][CG]
+  float2* tw = sm + 2 * CG * M;     // [N]
+  __shared__ long long colbase[CG];
+  const int row = blockIdx.x / NGRP, grp = blockIdx.x - row * NGRP;
+  int px, py, bt;
+  if (!row_pixel(rs, row, g, px, py, bt)) return;
+  load_twiddles_N(tw, gtw, N);
+  if (threadIdx.x < CG) {
+    const int jx = grp * JG + threadIdx.x / S, jy = threadIdx.x % S;
+    const int i = px * S + jx, j = py * S + jy;
+    const int bx = i / g.Bx, by = j / g.By;
+    const int slot = blockmap[((int64_t)bt * g.NBx + bx) * g.NBy + by];
+    long long base = -1;
+    if (slot >= 0) base = (((long long)slot * g.Bx + (i - bx * g.Bx)) * g.By + (j - by * g.By)) * g.Bt;
+    colbase[threadIdx.x] = base;
+  }
+  __syncthreads();
+  const int hb = g.Bt >> 1, hq = (hb + 3) >> 2;
+  for (int i = threadIdx.x; i < CG * hq * 4; i += 256) {
+    const int m4 = i & 3, rest = i >> 2;
+    const int c = rest % CG, m = (rest / CG) * 4 + m4;
+    if (m >= hb) continue;
+    float2 v = make_float2(0.0f, 0.0f);
+    const long long base = colbase[c];
+    if (base >= 0) v = *reinterpret_cast<const float2*>(payload + base + 2 * m);
+    A[m * CG + c] = v;
+  }
+  __syncthreads();
+  const float2* Z = fft_stockham_ct<M, 1, false, CG, 256>(A, B, tw, hb);
+  float2* out = qhat + (int64_t)row * NPH + grp * CG;
+  const int64_t fstride = (int64_t)rp * NPH;
+  for (int i = threadIdx.x; i < M * CG; i += 256) {
+    const int f = i / CG, c = i - f * CG;
+    out[f * fstride + c] = rfft_post(Z, CG, c, tw, M, f);
   }
 }
 
@@ -330,6 +485,81 @@ k_accum(const float2* __restrict__ T, const int64_t* __restrict__ sp_keys, int s
   }
 }
 
+// ------------------------------------------------------------------ (c') sum of the row-tile patches
+// Tensor-core path: the GEMM epilogue (tred_mac_tc.cu) has already summed the products
+// over the offsets inside every row tile's patch, opart[tile][f][X][Y].  A slab pixel is
+// covered by at most two tiles of each of at most three strips; they are added in ascending
+// tile order onto the running value of ohat, so the sequence of additions is the same for
+// any chunking.  One CTA per 32 consecutive slab pixels; reads are coalesced over the
+// pixels, the ohat update over the frequencies (transposed through shared memory).
+constexpr int ACC_MAXE = 8;
+
+__global__ void __launch_bounds__(256)
+k_accum_tiles(const float2* __restrict__ opart, const int64_t* __restrict__ sp_keys, int s0, int ns,
+              const int32_t* __restrict__ grp_off, const int4* __restrict__ rt_desc, int t0, int t1, int nstrip,
+              float2* __restrict__ ohat, int sbase, TredGrid g) {
+  __shared__ int32_t ent[32][ACC_MAXE];
+  __shared__ int cnt[32];
+  __shared__ float2 tile[32][33];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int PX = RT_SW + 2 * g.H;
+  const int64_t npos = (int64_t)PX * RT_PY;
+  int n = 0;
+  if (threadIdx.x < 32) {
+    const int spl = blockIdx.x * 32 + threadIdx.x;
+    if (spl < ns) {
+      const int64_t key = sp_keys[s0 + spl];
+      const int py = (int)(key % g.npy), px = (int)((key / g.npy) % g.npx);
+      const int bt = (int)(key / ((int64_t)g.npy * g.npx));
+      const int s_lo = px >= g.H ? (px - g.H) >> 3 : 0;
+      const int s_hi = min(nstrip - 1, (px + g.H) >> 3);
+      for (int sx = s_lo; sx <= s_hi; ++sx) {
+        const int grp = bt * nstrip + sx;
+        const int ta = max(grp_off[grp], t0), tb = min(grp_off[grp + 1], t1);
+        for (int t = ta; t < tb; ++t) {
+          const int4 d = rt_desc[t];
+          if (py >= d.z - g.H && py <= d.z + d.w - 1 + g.H && n < ACC_MAXE)
+            ent[threadIdx.x][n++] = ((t - t0) << 11) | ((px - (sx * RT_SW - g.H)) * RT_PY + (py - (d.z - g.H)));
+        }
+      }
+    }
+    cnt[threadIdx.x] = n;
+  }
+  if (!__syncthreads_or(n > 0)) return;
+  const int my_n = cnt[lane];
+  for (int f0 = 0; f0 < g.nf; f0 += 32) {
+    // running values, coalesced over f
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int sl = w * 4 + i, f = f0 + lane;
+      float2 v = make_float2(0.0f, 0.0f);
+      if (cnt[sl] > 0 && f < g.nf) v = ohat[(int64_t)(s0 + blockIdx.x * 32 + sl - sbase) * g.nf + f];
+      tile[lane][sl] = v;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int fl = w * 4 + i, f = f0 + fl;
+      if (f < g.nf && my_n > 0) {
+        float2 a = tile[fl][lane];
+        for (int e = 0; e < my_n; ++e) {
+          const int en = ent[lane][e];
+          const float2 v = opart[((int64_t)(en >> 11) * g.nf + f) * npos + (en & 2047)];
+          a.x += v.x; a.y += v.y;
+        }
+        tile[fl][lane] = a;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int sl = w * 4 + i, f = f0 + lane;
+      if (cnt[sl] > 0 && f < g.nf) ohat[(int64_t)(s0 + blockIdx.x * 32 + sl - sbase) * g.nf + f] = tile[lane][sl];
+    }
+    __syncthreads();
+  }
+}
+
 // ------------------------------------------------------------------ (d) inverse FFT
 // One CTA per IP slab pixels ([sample][pixel] in shared memory); sp_data[sp][n_over*Bt].
 // Lanes: pixel fastest, 4 consecutive samples per pixel -> full 32-byte sectors in HBM,
@@ -376,6 +606,52 @@ k_ifft(const float2* __restrict__ ohat, int s0, int ns, int sbase, float* __rest
   }
 }
 
+template <int M, int IP>
+__global__ void __launch_bounds__(256)
+k_ifft_ct(const float2* __restrict__ ohat, int s0, int ns, int sbase, float* __restrict__ sp_data,
+          const float2* __restrict__ gtw, TredGrid g, int out_len) {
+  extern __shared__ float2 sm[];
+  constexpr int N = 2 * M;
+  float2* A = sm;                   // [M][IP]
+  float2* B = sm + IP * M;          // [M][IP]
+  float2* tw = sm + 2 * IP * M;     // [N]
+  const int a0 = blockIdx.x * IP;
+  load_twiddles_N(tw, gtw, N);
+  __syncthreads();
+  constexpr int MQ = (M + 3) >> 2;
+  for (int i = threadIdx.x; i < IP * MQ * 4; i += 256) {
+    const int k4 = i & 3, rest = i >> 2;
+    const int c = rest % IP, k = (rest / IP) * 4 + k4;
+    if (k >= M) continue;
+    float2 z = make_float2(0.0f, 0.0f);
+    if (a0 + c < ns) {
+      const float2* X = ohat + (int64_t)(s0 + a0 + c - sbase) * M;
+      const float2 p = X[k], q = X[k ? M - k : 0];
+      z = rfft_pre_inverse(p, q, tw, k);
+    }
+    A[k * IP + c] = z;
+  }
+  __syncthreads();
+  const float2* Z = fft_stockham_ct<M, 1, true, IP, 256>(A, B, tw, M);
+  const int row = g.nover * g.Bt, hrow = row >> 1, hq = (hrow + 3) >> 2;
+  const float sc = 1.0f / (float)N;
+  for (int i = threadIdx.x; i < IP * hq * 4; i += 256) {
+    const int m4 = i & 3, rest = i >> 2;
+    const int c = rest % IP, m = (rest / IP) * 4 + m4;
+    if (m >= hrow || a0 + c >= ns) continue;
+    float2 v = make_float2(0.0f, 0.0f);
+    if (m < M) {
+      const float2 z = Z[m * IP + c];
+      v.x = (2 * m < out_len) ? z.x * sc : 0.0f;
+      v.y = (2 * m + 1 < out_len) ? z.y * sc : 0.0f;
+    }
+    reinterpret_cast<float2*>(sp_data + (int64_t)(s0 + a0 + c) * row)[m] = v;
+  }
+}
+
+// lengths with a compile-time instance (others use the run-time plan kernels)
+#define TRED_FFT_CT_LENGTHS(X) X(128) X(144) X(216) X(256) X(288) X(384) X(512)
+
 // ------------------------------------------------------------------ (e) S5 overlap-add
 __global__ void __launch_bounds__(256)
 k_gather_tiles(int64_t ntiles, const int64_t* __restrict__ tile_keys, const int32_t* __restrict__ sp_idx,
@@ -416,7 +692,61 @@ k_gather_dense(int64_t npix_req, const int32_t* __restrict__ pix_ids, const int3
   }
 }
 
-struct PlanWork { int32_t* cp_idx; int32_t* sp_idx; int32_t* tile_idx; void* scan; size_t total; int64_t nmap; };
+// Launch helpers: 1 if a compile-time instance ran, 0 if there is none for this shape,
+// < 0 on a CUDA error.
+static int launch_fft_fwd_ct(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
+                             const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
+  if (g.S != 10 || nr < 1) return 0;
+  const int M = g.L / 2;
+  const size_t smem = (size_t)(2 * 20 * M + g.L) * sizeof(float2);
+  if (smem > (size_t)ctx->smem_optin) return 0;
+  switch (M) {
+#define X(MM)                                                                                             \
+  case MM: {                                                                                              \
+    static bool set = false;                                                                              \
+    if (!set) {                                                                                           \
+      TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_ct<MM>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
+                                     (int)smem));                                                         \
+      set = true;                                                                                         \
+    }                                                                                                     \
+    k_fft_fwd_ct<MM><<<(unsigned)(nr * 5), 256, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);      \
+    return 1;                                                                                             \
+  }
+    TRED_FFT_CT_LENGTHS(X)
+#undef X
+    default: return 0;
+  }
+}
+
+static int launch_ifft_ct(const tred_ctx* ctx, const TredGrid& g, const float2* ohat, int s0, int ns, int sbase,
+                          float* sp_data, const float2* tw, int out_len, cudaStream_t st) {
+  constexpr int IP = 8;
+  const int M = g.L / 2;
+  const size_t smem = (size_t)(2 * IP * M + g.L) * sizeof(float2);
+  if (smem > (size_t)ctx->smem_optin || ns < 1) return 0;
+  switch (M) {
+#define X(MM)                                                                                             \
+  case MM: {                                                                                              \
+    static bool set = false;                                                                              \
+    if (!set) {                                                                                           \
+      TRED_CUDA(cudaFuncSetAttribute(k_ifft_ct<MM, IP>, cudaFuncAttributeMaxDynamicSharedMemorySize,      \
+                                     (int)smem));                                                         \
+      set = true;                                                                                         \
+    }                                                                                                     \
+    k_ifft_ct<MM, IP><<<cdiv(ns, IP), 256, smem, st>>>(ohat, s0, ns, sbase, sp_data, tw, g, out_len);     \
+    return 1;                                                                                             \
+  }
+    TRED_FFT_CT_LENGTHS(X)
+#undef X
+    default: return 0;
+  }
+}
+
+struct PlanWork {
+  int32_t* cp_idx; int32_t* sp_idx; int32_t* tile_idx; void* scan;
+  int32_t* ridx; int32_t* row_m2; int32_t* grp_off; int4* rt_desc;      // row tiles
+  size_t total; int64_t nmap;
+};
 
 static PlanWork carve_plan(const tred_ctx* c, void* base) {
   PlanWork w;
@@ -426,7 +756,12 @@ static PlanWork carve_plan(const tred_ctx* c, void* base) {
   w.cp_idx = (int32_t*)take((w.nmap + 1) * 4);
   w.sp_idx = (int32_t*)take((w.nmap + 1) * 4);
   w.tile_idx = (int32_t*)take((w.nmap + 1) * 4);
-  w.scan = take(tred_scan_work_bytes(w.nmap + 1));
+  const RtGeom rg = rt_geom(c);
+  w.scan = take(tred_scan_work_bytes((rg.nmap2 > w.nmap ? rg.nmap2 : w.nmap) + 1));
+  w.ridx = (int32_t*)take((rg.nmap2 + 1) * 4);
+  w.row_m2 = (int32_t*)take(rg.nmap2 * 4);
+  w.grp_off = (int32_t*)take((size_t)(rg.ngrp + 1) * 4);
+  w.rt_desc = (int4*)take((size_t)rg.cap_rt * sizeof(int4));
   w.total = o;
   return w;
 }
@@ -455,12 +790,146 @@ static ConvWork carve_conv(const tred_ctx* c, void* base, int64_t rows, int64_t 
   return w;
 }
 
+struct TiledWork {
+  int32_t* blockmap; float2* tw; float2* ohat; float2* qhat; float2* opart;
+  size_t total, per_tile;
+};
+
+static TiledWork carve_tiled(const tred_ctx* c, void* base, int64_t ntile, int64_t nsp) {
+  TiledWork w;
+  size_t o = 0; char* b = (char*)base;
+  auto take = [&](size_t bytes) { void* p = b ? b + o : nullptr; o += align_up(bytes, 1024); return p; };
+  const tred_dims& d = c->dims;
+  if (ntile < 1) ntile = 1;
+  if (nsp < 1) nsp = 1;
+  const size_t npos = (size_t)(RT_SW + 2 * c->cfg.resp_half) * RT_PY;
+  w.blockmap = (int32_t*)take((size_t)(d.NB[0] * d.NB[1] * d.NB[2]) * 4);
+  w.tw = (float2*)take((size_t)d.fft_len * 8);
+  w.ohat = (float2*)take((size_t)nsp * d.n_freq * 8);
+  w.qhat = (float2*)take((size_t)d.n_freq * ntile * RT_ROWS * d.n_phase * 8);
+  w.opart = (float2*)take((size_t)ntile * d.n_freq * npos * 8);
+  w.per_tile = (size_t)d.n_freq * (RT_ROWS * d.n_phase + npos) * 8;
+  w.total = o;
+  return w;
+}
+
 }  // namespace
 
 // tensor-core variant of step (b) (tred_mac_tc.cu); returns TRED_EUNSUPPORTED if it
 // cannot run this configuration
 int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* T,
                 int nrows, int rp, cudaStream_t st);
+// fused variant over row tiles: the epilogue sums the products over the offsets
+bool tred_mac_tc_fused_supported(const tred_ctx* ctx);
+int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
+                      int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
+
+static bool use_tiled(const tred_ctx* ctx) {
+  return ctx->cfg.mac_mode != 1 && ctx->cfg.mac_mode != 2 && tred_mac_tc_fused_supported(ctx);
+}
+
+// Tensor-core path of tred_convolve: row tiles (tred_convolve_plan), forward FFT into
+// qhat[f][tile * 128 + r][phase], fused spectrum product + sum over offsets per tile,
+// sum of the tile patches onto the slab pixels, inverse FFT.
+static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys, const float* d_payload,
+                          const float* d_rhat, const int64_t* d_sp_keys, const int32_t* h_sp_off,
+                          const int32_t* h_rt_off, const PlanWork& pw, float* d_sp_data,
+                          void* d_work, size_t work_bytes, cudaStream_t st) {
+  const TredGrid g = make_grid(ctx);
+  const tred_dims& d = ctx->dims;
+  const RtGeom rg = rt_geom(ctx);
+  FftPlan pl;
+  if (!tred_make_fft_plan(g.L / 2, &pl)) return TRED_EUNSUPPORTED;
+  const int M = g.L / 2;
+  int JG = g.S;
+  auto fwd_smem = [&](int jg) { return (size_t)(2 * jg * g.S * M + g.L) * sizeof(float2); };
+  while (JG > 1 && (fwd_smem(JG) > 100 * 1024 || JG * g.S > 64)) --JG;
+  if (fwd_smem(JG) > (size_t)ctx->smem_optin || JG * g.S > 64) return TRED_EUNSUPPORTED;
+  const int ngrp = (g.S + JG - 1) / JG;
+  TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fwd_smem(JG)));
+  int IP = 8;
+  auto inv_smem = [&](int ip) { return (size_t)(2 * ip * M + g.L) * sizeof(float2); };
+  while (IP > 1 && inv_smem(IP) > 64 * 1024) IP /= 2;
+  if (inv_smem(IP) > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
+  TRED_CUDA(cudaFuncSetAttribute(k_ifft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)inv_smem(IP)));
+
+  const TiledWork w0 = carve_tiled(ctx, d_work, 1, 1);
+  if (work_bytes < w0.total) return TRED_ECAP;
+  {
+    TredProfScope ps(ctx, ST_MISC, st);
+    TRED_CUDA(cudaMemsetAsync(w0.blockmap, 0xff, (size_t)g.NBx * g.NBy * g.NBt * 4, st));
+    k_fill_blockmap<<<cdiv(nblocks, 256), 256, 0, st>>>(nblocks, d_keys, w0.blockmap);
+    k_fill_twiddles<<<cdiv(g.L, 256), 256, 0, st>>>(w0.tw, g.L);
+    TRED_COUNT_LAUNCH(3);
+  }
+  const int64_t wfl = d.rhat_floats / 10 * 2, bfl = d.rhat_floats / 10 * 4;
+  int b0 = 0;
+  while (b0 < g.NBt) {
+    if (h_rt_off[b0 + 1] == h_rt_off[b0]) { ++b0; continue; }
+    int b1 = b0 + 1;
+    while (b1 < g.NBt && carve_tiled(ctx, nullptr, 1, h_sp_off[b1 + 1] - h_sp_off[b0]).total <= work_bytes / 4) ++b1;
+    const int sbase = h_sp_off[b0], nsb = h_sp_off[b1] - sbase;
+    const int T0 = h_rt_off[b0], T1 = h_rt_off[b1];
+    const TiledWork w1 = carve_tiled(ctx, nullptr, 1, nsb);
+    if (w1.total > work_bytes) return TRED_ECAP;
+    int64_t cap = 1 + (int64_t)((work_bytes - w1.total) / w1.per_tile);
+    while (cap > 1 && carve_tiled(ctx, nullptr, cap, nsb).total > work_bytes) --cap;
+    if (cap > T1 - T0) cap = T1 - T0;
+    if (cap * RT_ROWS * (int64_t)ngrp >= (1ll << 31)) cap = ((1ll << 31) - 1) / (RT_ROWS * ngrp);
+    const TiledWork w = carve_tiled(ctx, d_work, cap, nsb);
+    {
+      TredProfScope ps(ctx, ST_ACCUM, st);
+      TRED_CUDA(cudaMemsetAsync(w.ohat, 0, (size_t)nsb * g.nf * 8, st));
+      TRED_COUNT_LAUNCH(1);
+    }
+    for (int t0 = T0; t0 < T1; t0 += (int)cap) {
+      const int nt = (int)((T1 - t0 < cap) ? (T1 - t0) : cap);
+      const int rp = nt * RT_ROWS;
+      {
+        TredProfScope ps(ctx, ST_FFT_FWD, st);
+        const RowSrc rs{nullptr, 0, pw.rt_desc, pw.row_m2, t0, rg.nstrip, 1};
+        const int ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
+        if (ct < 0) return ct;
+        if (ct == 0)
+          k_fft_fwd<<<(unsigned)(rp * ngrp), 256, fwd_smem(JG), st>>>(d_payload, w.blockmap, rs, rp, JG, w.qhat,
+                                                                    w.tw, g, pl);
+        TRED_COUNT_LAUNCH(1);
+      }
+      {
+        TredProfScope ps(ctx, ST_MAC, st);
+        const int rc = tred_mac_tc_fused(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl,
+                                         (float*)w.opart, nt, t0, pw.rt_desc, pw.row_m2, st);
+        if (rc != TRED_OK) return rc;
+        TRED_COUNT_LAUNCH(1);
+      }
+      {
+        int sa = b0;
+        while (h_rt_off[sa + 1] <= t0) ++sa;
+        int sb = sa;
+        while (sb + 1 < b1 && h_rt_off[sb + 1] < t0 + nt) ++sb;
+        const int s0 = h_sp_off[sa], ns = h_sp_off[sb + 1] - s0;
+        TredProfScope ps(ctx, ST_ACCUM, st);
+        if (ns > 0)
+          k_accum_tiles<<<cdiv(ns, 32), 256, 0, st>>>(w.opart, d_sp_keys, s0, ns, pw.grp_off, pw.rt_desc, t0,
+                                                     t0 + nt, rg.nstrip, w.ohat, sbase, g);
+        TRED_COUNT_LAUNCH(1);
+      }
+      TRED_LAUNCH_CHECK("convolve tile chunk");
+    }
+    {
+      TredProfScope ps(ctx, ST_IFFT, st);
+      const int ct = launch_ifft_ct(ctx, g, w.ohat, sbase, nsb, sbase, d_sp_data, w.tw, d.out_len, st);
+      if (ct < 0) return ct;
+      if (ct == 0)
+        k_ifft<<<cdiv(nsb, IP), 256, inv_smem(IP), st>>>(w.ohat, sbase, nsb, sbase, d_sp_data, w.tw, g, pl, IP,
+                                                         d.out_len);
+      TRED_COUNT_LAUNCH(1);
+    }
+    TRED_LAUNCH_CHECK("convolve ifft");
+    b0 = b1;
+  }
+  return TRED_OK;
+}
 
 // ==================================================================== exported calls
 extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* d_rhat, void* stream) {
@@ -491,8 +960,10 @@ extern "C" int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t*
                                   int64_t cap_cp, int64_t* d_cp_keys, int32_t* d_cp_off, int64_t* d_ncp,
                                   int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
                                   int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
+                                  int32_t* d_rt_off,
                                   void* d_plan_work, size_t plan_work_bytes, void* stream) {
-  if (!ctx || nblocks < 0 || !d_ncp || !d_cp_off || !d_nsp || !d_ntiles || !d_sp_off) return TRED_EINVAL;
+  if (!ctx || nblocks < 0 || !d_ncp || !d_cp_off || !d_nsp || !d_ntiles || !d_sp_off || !d_rt_off)
+    return TRED_EINVAL;
   PlanWork w = carve_plan(ctx, d_plan_work);
   if (!d_plan_work || plan_work_bytes < w.total) return TRED_ECAP;
   if (nblocks > 0 && !d_keys) return TRED_EINVAL;
@@ -518,18 +989,39 @@ extern "C" int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t*
   if (rc != TRED_OK) return rc;
   k_compact_keys<<<cdiv(w.nmap + 1, 256), 256, 0, st>>>(w.nmap, w.tile_idx, cap_tiles, d_tile_keys, d_ntiles,
                                                        nullptr, 0, npix);
+  {
+    // row tiles of the tensor-core path (strip order of the charge pixels)
+    const RtGeom rg = rt_geom(ctx);
+    k_rt_flags<<<cdiv(rg.nmap2 + 1, 256), 256, 0, st>>>(rg.nmap2, w.cp_idx, w.ridx, rg.nstrip, g);
+    rc = tred_exclusive_scan_i32(w.ridx, w.ridx, rg.nmap2 + 1, nullptr, w.scan, st);
+    if (rc != TRED_OK) return rc;
+    k_rt_rows<<<cdiv(rg.nmap2, 256), 256, 0, st>>>(rg.nmap2, w.ridx, w.row_m2);
+    TRED_CUDA(cudaMemsetAsync(w.grp_off, 0, (size_t)(rg.ngrp + 1) * 4, st));
+    k_rt_tiles<false><<<cdiv(rg.ngrp, 128), 128, 0, st>>>(rg.ngrp, g.npy, rg.capy, w.ridx, w.grp_off, nullptr,
+                                                         nullptr, 0);
+    rc = tred_exclusive_scan_i32(w.grp_off, w.grp_off, rg.ngrp + 1, nullptr, w.scan, st);
+    if (rc != TRED_OK) return rc;
+    k_rt_tiles<true><<<cdiv(rg.ngrp, 128), 128, 0, st>>>(rg.ngrp, g.npy, rg.capy, w.ridx, nullptr, w.grp_off,
+                                                        w.rt_desc, rg.cap_rt);
+    k_rt_slab_off<<<cdiv(g.NBt + 1, 128), 128, 0, st>>>(g.NBt, rg.nstrip, w.grp_off, d_rt_off);
+    TRED_COUNT_LAUNCH(8);
+  }
   TRED_LAUNCH_CHECK("convolve_plan");
   return TRED_OK;
 }
 
 extern "C" size_t tred_convolve_work_bytes(const tred_ctx* ctx, int64_t rows_chunk, int64_t nsp_batch) {
-  return ctx ? carve_conv(ctx, nullptr, rows_chunk, nsp_batch).total : 0;
+  if (!ctx) return 0;
+  if (use_tiled(ctx))      // row tiles are >= 121 rows full unless cut by a strip end or the patch height
+    return carve_tiled(ctx, nullptr, rows_chunk / 100 + 2, nsp_batch).total;
+  return carve_conv(ctx, nullptr, rows_chunk, nsp_batch).total;
 }
 
 extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys, const float* d_payload,
                              const float* d_rhat,
                              int64_t ncp, const int64_t* d_cp_keys, const int32_t* h_cp_off,
                              int64_t nsp, const int64_t* d_sp_keys, const int32_t* h_sp_off,
+                             const int32_t* h_rt_off,
                              const void* d_plan_work, float* d_sp_data,
                              void* d_work, size_t work_bytes, void* stream) {
   if (!ctx || nblocks < 0 || nsp < 0 || ncp < 0) return TRED_EINVAL;
@@ -544,6 +1036,11 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
   if (h_cp_off[g.NBt] != ncp || h_sp_off[g.NBt] != nsp) return TRED_EINVAL;
   if (g.Bt < 2 || (g.Bt & 1)) return TRED_EUNSUPPORTED;
   const PlanWork pw = carve_plan(ctx, (void*)d_plan_work);
+  if (use_tiled(ctx)) {
+    if (!h_rt_off) return TRED_EINVAL;
+    return convolve_tiled(ctx, nblocks, d_keys, d_payload, d_rhat, d_sp_keys, h_sp_off, h_rt_off, pw, d_sp_data,
+                          d_work, work_bytes, st);
+  }
   FftPlan pl;
   if (!tred_make_fft_plan(g.L / 2, &pl)) return TRED_EUNSUPPORTED;
   const int M = g.L / 2;
@@ -606,8 +1103,12 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
       const int nr = (int)((R1 - r0 < cap) ? (R1 - r0) : cap);
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
-        k_fft_fwd<<<(unsigned)(nr * ngrp), 256, fwd_smem(JG), st>>>(d_payload, w.blockmap, d_cp_keys, r0, nr, rp,
-                                                                  JG, w.qhat, w.tw, g, pl);
+        const RowSrc rs{d_cp_keys, r0, nullptr, nullptr, 0, 0, 0};
+        const int ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
+        if (ct < 0) return ct;
+        if (ct == 0)
+          k_fft_fwd<<<(unsigned)(nr * ngrp), 256, fwd_smem(JG), st>>>(d_payload, w.blockmap, rs, rp, JG, w.qhat,
+                                                                    w.tw, g, pl);
         TRED_COUNT_LAUNCH(1);
       }
       {
@@ -643,7 +1144,11 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
     }
     {
       TredProfScope ps(ctx, ST_IFFT, st);
-      k_ifft<<<cdiv(nsb, IP), 256, inv_smem(IP), st>>>(w.ohat, sbase, nsb, sbase, d_sp_data, w.tw, g, pl, IP, d.out_len);
+      const int ct = launch_ifft_ct(ctx, g, w.ohat, sbase, nsb, sbase, d_sp_data, w.tw, d.out_len, st);
+      if (ct < 0) return ct;
+      if (ct == 0)
+        k_ifft<<<cdiv(nsb, IP), 256, inv_smem(IP), st>>>(w.ohat, sbase, nsb, sbase, d_sp_data, w.tw, g, pl, IP,
+                                                         d.out_len);
       TRED_COUNT_LAUNCH(1);
     }
     TRED_LAUNCH_CHECK("convolve ifft");

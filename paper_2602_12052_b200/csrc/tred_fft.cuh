@@ -176,3 +176,60 @@ __device__ __forceinline__ float2 rfft_pre_inverse(float2 p, float2 q, const flo
   const float2 wo = cmulf(w, o);
   return make_float2(e.x - wo.y, e.y + wo.x);                                // e + i w o
 }
+
+// ---------------------------------------------------------------------------------
+// Compile-time variant of the same Stockham passes: length M, transforms per CTA NB and
+// threads NT are template parameters, so every index (division by NB, modulo by the
+// pass stride, twiddle step) is a constant expression and the passes unroll.  Same
+// radix order as tred_make_fft_plan (8s, 4s, 2s, then 3s), same arithmetic.
+template <int REM> struct NextRadix {
+  static constexpr int R = (REM % 8 == 0) ? 8 : (REM % 4 == 0) ? 4 : (REM % 2 == 0) ? 2 : 3;
+};
+
+template <int R, int M, int NS, bool INV, int NB, int NT>
+__device__ __forceinline__ void stockham_pass_ct(const float2* __restrict__ src, float2* __restrict__ dst,
+                                                 const float2* __restrict__ twN, int nz) {
+  constexpr int PER = M / R;
+  constexpr int TWS = (M / (NS * R)) * 2;
+  constexpr int JSTEP = NT / NB;
+  const int b = threadIdx.x % NB;
+  const int jt = threadIdx.x / NB;
+  if (jt >= JSTEP) return;
+#pragma unroll 1
+  for (int j = jt; j < PER; j += JSTEP) {
+    const int k = j % NS;
+    float2 v[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) {
+      const int e = j + t * PER;
+      v[t] = (e < nz) ? src[e * NB + b] : make_float2(0.0f, 0.0f);
+    }
+    if (NS > 1) {
+#pragma unroll
+      for (int t = 1; t < R; ++t) {
+        float2 w = twN[k * (t * TWS)];
+        if (INV) w.y = -w.y;
+        v[t] = cmulf(v[t], w);
+      }
+    }
+    if (R == 2) dft2<INV>(v[0], v[1]);
+    else if (R == 3) dft3<INV>(v);
+    else if (R == 4) dft4<INV>(v);
+    else dft8<INV>(v);
+    const int o = (j - k) * R + k;
+#pragma unroll
+    for (int t = 0; t < R; ++t) dst[(o + t * NS) * NB + b] = v[t];
+  }
+}
+
+template <int M, int NS, bool INV, int NB, int NT>
+__device__ __forceinline__ float2* fft_stockham_ct(float2* a, float2* b, const float2* twN, int nz) {
+  if constexpr (NS >= M) {
+    return a;
+  } else {
+    constexpr int R = NextRadix<M / NS>::R;
+    stockham_pass_ct<R, M, NS, INV, NB, NT>(a, b, twN, nz);
+    __syncthreads();
+    return fft_stockham_ct<M, NS * R, INV, NB, NT>(b, a, twN, M);
+  }
+}

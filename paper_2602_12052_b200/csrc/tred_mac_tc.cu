@@ -25,13 +25,16 @@ namespace {
 
 constexpr int TC_M = 128;                 // rows per tile (TMEM lanes)
 constexpr int TC_KC = 16;                 // floats per K chunk = one 64-byte swizzle row
-constexpr int TC_STAGES = 4;
+constexpr int TC_STAGES_PLAIN = 4;        // K-chunk pipeline depth, T written to memory
+constexpr int TC_STAGES_FUSED = 3;        // with the patch buffers of the fused epilogue
 constexpr int TC_NMAX = 256;              // max N = 2 kp
 constexpr int TC_A_BYTES = TC_M * TC_KC * 4;          // 8 KB
 constexpr int TC_B_BYTES = TC_NMAX * TC_KC * 4;       // 16 KB
 constexpr int TC_STAGE_BYTES = 2 * TC_A_BYTES + 2 * TC_B_BYTES;   // A, A_lo, B_hi, B_lo
 constexpr int TC_THREADS = 320;
-constexpr size_t TC_SMEM = (size_t)TC_STAGES * TC_STAGE_BYTES + 1024 + 256;
+constexpr int TC_PATCH_FLOAT2 = RT_PXMAX * RT_PYS;                  // one warp's patch accumulator
+constexpr size_t TC_SMEM_PLAIN = (size_t)TC_STAGES_PLAIN * TC_STAGE_BYTES + 1024 + 256;
+constexpr size_t TC_SMEM_FUSED = (size_t)TC_STAGES_FUSED * TC_STAGE_BYTES + 1024 + 256 + 4 * TC_PATCH_FLOAT2 * 8;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -105,11 +108,18 @@ struct TcParams {
   int N;                        // 2 kp (multiple of 16, <= 256)
   int K2;                       // 2 nph floats per row (multiple of 8)
   int noff, kp;
+  // fused epilogue (row tiles, tred_conv.cu): sum over the offsets into the tile's patch
+  int K, H, npy, t0;            // 2H+1, H, pixels along y, first row tile of the chunk
+  const int4* rt_desc;          // {first row, rows, py0, ny} per row tile
+  const int32_t* row_m2;        // strip-order map index of every row
+  float2* opart;                // [tile][f][8 + 2H][RT_PY]
 };
 
+template <bool FUSED>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_mac_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmBh,
          const __grid_constant__ CUtensorMap tmBl, float2* __restrict__ T, TcParams p) {
+  constexpr int TC_STAGES = FUSED ? TC_STAGES_FUSED : TC_STAGES_PLAIN;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;                  // swizzle atoms need aligned tiles
@@ -223,8 +233,8 @@ k_mac_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtens
         if (++stage == TC_STAGES) { stage = 0; phase ^= 1; }
       }
     }
-  } else {
-    // ------------------------------------------------------------ epilogue
+  } else if (!FUSED) {
+    // ------------------------------------------------------------ epilogue: store T
     const int q = warp & 3;                                        // TMEM lane quadrant of this warp
     int as = 0, aphase = 0;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
@@ -259,6 +269,84 @@ k_mac_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtens
       tc_fence_before();
       mbar_arrive(tempty_bar(as));
       if (++as == 2) { as = 0; aphase ^= 1; }
+    }
+  } else {
+    // ------------------------------------------------------------ epilogue: sum over offsets
+    // Row r of the tile is the charge pixel (8 strip + xl, py0 + yl); its product with
+    // offset (kx, ky) belongs to patch cell (xl + kx + H, yl + ky + H).  For a fixed offset
+    // the rows of a warp hit distinct cells, so each warp adds into its own patch copy
+    // without atomics; the four copies are then summed in a fixed order.
+    const int q = warp & 3;                                        // TMEM lane quadrant of this warp
+    const int et = threadIdx.x - 192;                              // 0..127
+    float2* patch = reinterpret_cast<float2*>(base_ptr + TC_STAGES * TC_STAGE_BYTES + 256);
+    float2* P = patch + q * TC_PATCH_FLOAT2;
+    for (int i = et; i < 4 * TC_PATCH_FLOAT2; i += 128) patch[i] = make_float2(0.0f, 0.0f);
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    const int PX = RT_SW + 2 * p.H;
+    int as = 0, aphase = 0;
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+      const int f = item / p.ntile, mt = item - f * p.ntile;
+      const int4 d = p.rt_desc[p.t0 + mt];
+      const int r = q * 32 + lane;
+      const bool valid = r < d.y;
+      const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
+      int cell0 = 0;
+      if (valid) {
+        const int m2 = p.row_m2[d.x + r];
+        cell0 = (m2 & (RT_SW - 1)) * RT_PYS + ((m2 >> 3) % p.npy - d.z);
+      }
+      mbar_wait(tfull_bar(as), aphase);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (uint32_t)(as * TC_NMAX) + ((uint32_t)(q * 32) << 16);
+      for (int c0 = 0; c0 * 16 < p.noff; ++c0) {
+        uint32_t v[32];
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+            "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+            "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+            : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+              "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+              "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+              "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+            : "r"(taddr + (uint32_t)(c0 * 32))
+            : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (valid) {
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const int off = c0 * 16 + j;
+            if (off < p.noff) {
+              const int kx = off / p.K, ky = off - kx * p.K;
+              float2* e = P + cell0 + kx * RT_PYS + ky;
+              float2 a = *e;
+              a.x += __uint_as_float(v[2 * j]);
+              a.y += __uint_as_float(v[2 * j + 1]);
+              *e = a;
+            }
+            __syncwarp(vmask);       // another row's next offset may land on this cell
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(tempty_bar(as));                                 // accumulator free for the next tile
+      if (++as == 2) { as = 0; aphase ^= 1; }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      const int nyp = d.w + 2 * p.H, ncell = PX * nyp;
+      float2* dst = p.opart + ((int64_t)mt * p.nf + f) * (PX * RT_PY);
+      for (int i = et; i < ncell; i += 128) {
+        const int X = i / nyp, Y = i - X * nyp;
+        const int c = X * RT_PYS + Y;
+        float2 a = patch[c];
+#pragma unroll
+        for (int w = 1; w < 4; ++w) {
+          const float2 b = patch[w * TC_PATCH_FLOAT2 + c];
+          a.x += b.x; a.y += b.y;
+        }
+#pragma unroll
+        for (int w = 0; w < 4; ++w) patch[w * TC_PATCH_FLOAT2 + c] = make_float2(0.0f, 0.0f);
+        dst[X * RT_PY + Y] = a;
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
     }
   }
   tc_fence_before();
@@ -302,6 +390,58 @@ static bool make_map(PFN_encodeTiled enc, CUtensorMap* tm, const float* base, in
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+static int tc_check(const tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, int rp, size_t smem,
+                    PFN_encodeTiled* enc) {
+  const tred_dims& d = ctx->dims;
+  const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
+  if (N > TC_NMAX || (N & 15) || (K2 & 7) || (rp % TC_M) || rp < TC_M) return TRED_EUNSUPPORTED;
+  if ((size_t)ctx->smem_optin < smem) return TRED_EUNSUPPORTED;
+  if ((((uintptr_t)qhat) | ((uintptr_t)Bhi) | ((uintptr_t)Blo)) & 15) return TRED_EUNSUPPORTED;
+  *enc = get_encode_fn();
+  return *enc ? TRED_OK : TRED_EUNSUPPORTED;
+}
+
+// Can the fused (row tile) path run this configuration at all?  (tred_conv.cu asks before
+// it lays the workspace out.)
+bool tred_mac_tc_fused_supported(const tred_ctx* ctx) {
+  const tred_dims& d = ctx->dims;
+  const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
+  return !(N > TC_NMAX || (N & 15) || (K2 & 7)) && (size_t)ctx->smem_optin >= TC_SMEM_FUSED &&
+         ctx->cfg.resp_half <= RT_MAXH && get_encode_fn() != nullptr;
+}
+
+// Fused variant: ntile row tiles of 128 padded rows each (rp = 128 ntile), the products
+// summed over the offsets into opart[tile][f][8 + 2H][RT_PY].
+int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
+                      int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st) {
+  const tred_dims& d = ctx->dims;
+  const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
+  const int rp = ntile * TC_M;
+  PFN_encodeTiled enc = nullptr;
+  if (ntile < 1 || ctx->cfg.resp_half > RT_MAXH) return TRED_EUNSUPPORTED;
+  int rc = tc_check(ctx, qhat, Bhi, Blo, rp, TC_SMEM_FUSED, &enc);
+  if (rc != TRED_OK) return rc;
+  CUtensorMap tmA, tmBh, tmBl;
+  if (!make_map(enc, &tmA, qhat, K2, rp, d.n_freq, TC_M) || !make_map(enc, &tmBh, Bhi, K2, N, d.n_freq, N) ||
+      !make_map(enc, &tmBl, Blo, K2, N, d.n_freq, N))
+    return TRED_EUNSUPPORTED;
+  static bool attr_set = false;
+  if (!attr_set) {
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_FUSED));
+    attr_set = true;
+  }
+  TcParams p;
+  p.nf = d.n_freq; p.ntile = ntile; p.nrows = rp; p.rp = rp;
+  p.N = N; p.K2 = K2; p.noff = d.n_off; p.kp = d.n_off_pad;
+  p.K = 2 * ctx->cfg.resp_half + 1; p.H = ctx->cfg.resp_half; p.npy = ctx->cfg.npix_y; p.t0 = t0;
+  p.rt_desc = (const int4*)rt_desc; p.row_m2 = row_m2; p.opart = reinterpret_cast<float2*>(opart);
+  const int64_t items = (int64_t)p.nf * p.ntile;
+  const int grid = (int)(items < ctx->num_sms ? items : ctx->num_sms);
+  k_mac_tc<true><<<grid, TC_THREADS, TC_SMEM_FUSED, st>>>(tmA, tmBh, tmBl, nullptr, p);
+  TRED_LAUNCH_CHECK("k_mac_tc<fused>");
+  return TRED_OK;
+}
+
 // Returns TRED_EUNSUPPORTED when this configuration cannot run on the tensor-core kernel
 // (tred_convolve then uses the fp32 FMA kernel unless mac_mode forces this one).
 int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* T, int nrows, int rp,
@@ -309,7 +449,7 @@ int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float*
   const tred_dims& d = ctx->dims;
   const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
   if (N > TC_NMAX || (N & 15) || (K2 & 7) || (rp % TC_M) || nrows < 1) return TRED_EUNSUPPORTED;
-  if ((size_t)ctx->smem_optin < TC_SMEM) return TRED_EUNSUPPORTED;
+  if ((size_t)ctx->smem_optin < TC_SMEM_PLAIN) return TRED_EUNSUPPORTED;
   if ((((uintptr_t)qhat) | ((uintptr_t)Bhi) | ((uintptr_t)Blo)) & 15) return TRED_EUNSUPPORTED;
   PFN_encodeTiled enc = get_encode_fn();
   if (!enc) return TRED_EUNSUPPORTED;
@@ -319,15 +459,16 @@ int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float*
     return TRED_EUNSUPPORTED;
   static bool attr_set = false;
   if (!attr_set) {
-    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_PLAIN));
     attr_set = true;
   }
   TcParams p;
   p.nf = d.n_freq; p.ntile = (nrows + TC_M - 1) / TC_M; p.nrows = nrows; p.rp = rp;
   p.N = N; p.K2 = K2; p.noff = d.n_off; p.kp = d.n_off_pad;
+  p.K = 0; p.H = 0; p.npy = 0; p.t0 = 0; p.rt_desc = nullptr; p.row_m2 = nullptr; p.opart = nullptr;
   const int64_t items = (int64_t)p.nf * p.ntile;
   const int grid = (int)(items < ctx->num_sms ? items : ctx->num_sms);
-  k_mac_tc<<<grid, TC_THREADS, TC_SMEM, st>>>(tmA, tmBh, tmBl, reinterpret_cast<float2*>(T), p);
+  k_mac_tc<false><<<grid, TC_THREADS, TC_SMEM_PLAIN, st>>>(tmA, tmBh, tmBl, reinterpret_cast<float2*>(T), p);
   TRED_LAUNCH_CHECK("k_mac_tc");
   return TRED_OK;
 }
