@@ -115,7 +115,9 @@ struct TcParams {
   float2* opart;                // [tile][f][8 + 2H][RT_PY]
 };
 
-template <bool FUSED>
+// KC: compile-time 2H+1 of the fused epilogue (offset -> patch cell becomes an immediate
+// address offset), 0 = read it from the parameters.
+template <bool FUSED, int KC>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_mac_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmBh,
          const __grid_constant__ CUtensorMap tmBl, float2* __restrict__ T, TcParams p) {
@@ -298,7 +300,11 @@ k_mac_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtens
       mbar_wait(tfull_bar(as), aphase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + (uint32_t)(as * TC_NMAX) + ((uint32_t)(q * 32) << 16);
-      for (int c0 = 0; c0 * 16 < p.noff; ++c0) {
+      const int KK = KC ? KC : p.K;
+      const int noff = KC ? KC * KC : p.noff;
+#pragma unroll
+      for (int c0 = 0; c0 < (KC ? (KC * KC + 15) / 16 : 8); ++c0) {
+        if (!KC && c0 * 16 >= noff) break;
         uint32_t v[32];
         asm volatile(
             "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -312,12 +318,13 @@ k_mac_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtens
             : "memory");
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         if (valid) {
+          float2* Pc = P + cell0;
 #pragma unroll
           for (int j = 0; j < 16; ++j) {
             const int off = c0 * 16 + j;
-            if (off < p.noff) {
-              const int kx = off / p.K, ky = off - kx * p.K;
-              float2* e = P + cell0 + kx * RT_PYS + ky;
+            if (off < noff) {
+              const int kx = off / KK, ky = off - kx * KK;
+              float2* e = Pc + kx * RT_PYS + ky;
               float2 a = *e;
               a.x += __uint_as_float(v[2 * j]);
               a.y += __uint_as_float(v[2 * j + 1]);
@@ -427,7 +434,8 @@ int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const 
     return TRED_EUNSUPPORTED;
   static bool attr_set = false;
   if (!attr_set) {
-    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_FUSED));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_FUSED));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<true, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_FUSED));
     attr_set = true;
   }
   TcParams p;
@@ -437,7 +445,10 @@ int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const 
   p.rt_desc = (const int4*)rt_desc; p.row_m2 = row_m2; p.opart = reinterpret_cast<float2*>(opart);
   const int64_t items = (int64_t)p.nf * p.ntile;
   const int grid = (int)(items < ctx->num_sms ? items : ctx->num_sms);
-  k_mac_tc<true><<<grid, TC_THREADS, TC_SMEM_FUSED, st>>>(tmA, tmBh, tmBl, nullptr, p);
+  if (p.K == 11)
+    k_mac_tc<true, 11><<<grid, TC_THREADS, TC_SMEM_FUSED, st>>>(tmA, tmBh, tmBl, nullptr, p);
+  else
+    k_mac_tc<true, 0><<<grid, TC_THREADS, TC_SMEM_FUSED, st>>>(tmA, tmBh, tmBl, nullptr, p);
   TRED_LAUNCH_CHECK("k_mac_tc<fused>");
   return TRED_OK;
 }
@@ -459,7 +470,7 @@ int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float*
     return TRED_EUNSUPPORTED;
   static bool attr_set = false;
   if (!attr_set) {
-    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_PLAIN));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_PLAIN));
     attr_set = true;
   }
   TcParams p;
@@ -468,7 +479,7 @@ int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float*
   p.K = 0; p.H = 0; p.npy = 0; p.t0 = 0; p.rt_desc = nullptr; p.row_m2 = nullptr; p.opart = nullptr;
   const int64_t items = (int64_t)p.nf * p.ntile;
   const int grid = (int)(items < ctx->num_sms ? items : ctx->num_sms);
-  k_mac_tc<false><<<grid, TC_THREADS, TC_SMEM_PLAIN, st>>>(tmA, tmBh, tmBl, reinterpret_cast<float2*>(T), p);
+  k_mac_tc<false, 0><<<grid, TC_THREADS, TC_SMEM_PLAIN, st>>>(tmA, tmBh, tmBl, reinterpret_cast<float2*>(T), p);
   TRED_LAUNCH_CHECK("k_mac_tc");
   return TRED_OK;
 }
