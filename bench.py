@@ -196,10 +196,20 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # config 4: device-memory-bounded chunks of occupied blocks (peak <= 40 GB)
+    if args.config == 4:
+        sim.conv_work_bytes = (args.work_gb or 8) << 30
+
+        def simulate(s):
+            return sim.simulate_chunked(s, rhat, payload_budget_bytes=args.budget_gb << 30)
+    else:
+        def simulate(s):
+            return sim.simulate(s, rhat)
+
     # ---- warm-up
     out = None
     for _ in range(max(args.warmup, 3)):
-        out = sim.simulate(seg_d, rhat)
+        out = simulate(seg_d)
     barrier()
     info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles")}
     # Gauss-Legendre node evaluations of one step = cuboids of every bounding box x n^3
@@ -217,7 +227,7 @@ def run_cuda(args):
     for a, b in ev:
         flush.zero_()                       # flush L2 between timed iterations
         a.record()
-        out = sim.simulate(seg_d, rhat)
+        out = simulate(seg_d)
         b.record()
     barrier()
     t_wall = time.perf_counter() - t_wall0
@@ -232,7 +242,7 @@ def run_cuda(args):
     for _ in range(args.steps):
         flush.zero_()
         sim.profile_begin(events=True)
-        sim.simulate(seg_d, rhat)
+        simulate(seg_d)
         torch.cuda.synchronize()
         stage_prof_last = sim.profile_end()
         for k, (m, n) in stage_prof_last.items():
@@ -248,7 +258,7 @@ def run_cuda(args):
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         sd = seg_pinned.to(dev, non_blocking=True)
-        o2 = sim.simulate(sd, rhat)
+        o2 = simulate(sd)
         keys_h = o2["tile_keys"].cpu()
         data_h = o2["tile_data"].cpu()
         torch.cuda.synchronize()
@@ -321,7 +331,8 @@ def run_cuda(args):
                            "pixels": [cfg.npix_x, cfg.npix_y], "nticks": cfg.nticks, "gl_n": cfg.gl_n,
                            "block": list(cfg.block), "resp_nticks": cfg.resp_nticks, "fft_len": d.fft_len,
                            "l2": "flushed between timed iterations (256 MiB write)",
-                           "parallelism": f"events x{world}, no collective", **info},
+                           "parallelism": f"events x{world}, no collective",
+                           "chunks": len(out.get("chunks", [])) or 1, **info},
                 "e2e": {"value": total_seg / (e2e_max * 1e-3), "unit": UNIT, "ms_per_step": e2e_max,
                         "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
                 "gpu_launches": int(launches),
@@ -346,6 +357,109 @@ def run_cuda(args):
     return 0
 
 
+# --------------------------------------------------------------------------- config 5
+def dense_grid_convolution(torch, cfg, keys, payload, R_d, pix_ids):
+    """Comparison point of BASELINE config 5: FFT convolution of the WHOLE plane on the
+    dense grid (no block sparsity), one sub-pixel phase at a time (Eq. (14) with the 3-D
+    FFT over pixel x pixel x time), with torch.fft (cuFFT): a timed
+    comparison only, not the product path.  Returns (dense rows for pix_ids, ms, peak bytes)."""
+    dev = payload.device
+    S, H, Tr = cfg.sub, cfg.resp_half, cfg.resp_nticks
+    Bx, By, Bt = cfg.block
+    NBx, NBy = -(-cfg.npix_x * S // Bx), -(-cfg.npix_y * S // By)
+    NBt = -(-cfg.nticks // Bt)
+    K = 2 * H + 1
+    nx, ny, nt = cfg.npix_x + K - 1, cfg.npix_y + K - 1, NBt * Bt + Tr - 1
+    nt += nt & 1
+    torch.cuda.reset_peak_memory_stats(dev)
+    base = torch.cuda.memory_allocated(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    nb = keys.numel()
+    bmap = torch.full((NBt * NBx * NBy,), nb, dtype=torch.int64, device=dev)      # nb = the zero block
+    bmap[keys] = torch.arange(nb, device=dev)
+    bmap = bmap.view(NBt, NBx, NBy)
+    pay = torch.cat([payload.view(nb, Bx, By, Bt), torch.zeros((1, Bx, By, Bt), device=dev)])
+    px = torch.arange(cfg.npix_x, device=dev)
+    py = torch.arange(cfg.npix_y, device=dev)
+    acc = None
+    for jx in range(S):
+        ix = px * S + jx
+        for jy in range(S):
+            iy = py * S + jy
+            slot = bmap[:, (ix // Bx)[:, None], (iy // By)[None, :]]                # [NBt][npx][npy]
+            q = pay[slot, (ix % Bx)[None, :, None], (iy % By)[None, None, :], :]     # [NBt][npx][npy][Bt]
+            q = q.permute(1, 2, 0, 3).reshape(cfg.npix_x, cfg.npix_y, NBt * Bt)
+            qh = torch.fft.rfftn(q, s=(nx, ny, nt))
+            rh = torch.fft.rfftn(R_d[jx, jy], s=(nx, ny, nt))
+            acc = qh * rh if acc is None else acc.addcmul_(qh, rh)
+            del q, qh, rh, slot
+    out = torch.fft.irfftn(acc, s=(nx, ny, nt))[H:H + cfg.npix_x, H:H + cfg.npix_y, :cfg.nticks]
+    rows = out.reshape(cfg.npix_x * cfg.npix_y, cfg.nticks)[pix_ids.long()].contiguous()
+    e1.record()
+    torch.cuda.synchronize()
+    return rows, e0.elapsed_time(e1), torch.cuda.max_memory_allocated(dev) - base
+
+
+def run_sweep(args):
+    """BASELINE config 5: block shapes x Gauss-Legendre orders on config-3 inputs, one JSON
+    line each (ms per spill, peak GB, occupied-block fraction), then the dense-grid line."""
+    import torch
+    from paper_2602_12052_b200 import Tred
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    cfg0, segs, seg_h, R = workload(3, 0)
+    seg_d = torch.from_numpy(seg_h).to(dev)
+    R_d = torch.from_numpy(R).to(dev)
+    steps = max(1, min(args.steps, 3))
+    for block in ((4, 4, 32), (8, 8, 64), (16, 16, 128), (32, 32, 256)):
+        for n in (1, 2, 3, 4):
+            cfg = cfg0.with_(block=block, gl_n=n)
+            torch.cuda.empty_cache()
+            torch.cuda.reset_peak_memory_stats(dev)
+            sim = Tred(cfg, device=dev)
+            rhat = sim.prepare_response(R_d)
+            out = sim.simulate(seg_d, rhat)                      # warm-up
+            ms = []
+            for _ in range(steps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                out = sim.simulate(seg_d, rhat)
+                b.record()
+                torch.cuda.synchronize()
+                ms.append(a.elapsed_time(b))
+            d = sim.dims
+            nb_all = int(d.NB[0] * d.NB[1] * d.NB[2])
+            print(json.dumps({"sweep": "block x gl_n", "workload": cfg0.name, "block": list(block), "gl_n": n,
+                              "fft_len": d.fft_len, "ms_per_spill": float(np.mean(ms)),
+                              "segments_per_s": seg_h.shape[1] / (float(np.mean(ms)) * 1e-3),
+                              "nblocks": out["nblocks"], "occupied_block_fraction": out["nblocks"] / nb_all,
+                              "payload_gb": out["nblocks"] * d.block_floats * 4 / 1e9,
+                              "peak_gb": torch.cuda.max_memory_allocated(dev) / 1e9}), flush=True)
+            del sim, rhat, out
+    # dense-grid comparison on the config-3 representation
+    cfg = cfg0
+    torch.cuda.empty_cache()
+    sim = Tred(cfg, device=dev)
+    rhat = sim.prepare_response(R_d)
+    rng = np.random.default_rng(5)
+    pix = torch.from_numpy(np.sort(rng.choice(cfg.npix_x * cfg.npix_y, 64, replace=False)).astype(np.int32)).to(dev)
+    out = sim.simulate(seg_d, rhat, pix_ids=pix, keep=True)
+    sparse_rows = out["dense"]
+    keys, payload = out["keys"].clone(), out["payload"].clone()
+    del out, rhat
+    sim._work.clear()
+    torch.cuda.empty_cache()
+    rows, ms, peak = dense_grid_convolution(torch, cfg, keys, payload, R_d, pix)      # warm-up (cuFFT plans)
+    rows, ms, peak = dense_grid_convolution(torch, cfg, keys, payload, R_d, pix)
+    err = float((rows - sparse_rows).abs().max() / sparse_rows.abs().max())
+    print(json.dumps({"sweep": "dense grid", "workload": cfg.name, "impl": "torch.fft (cuFFT), comparison only",
+                      "ms_per_spill_convolution_only": ms, "peak_gb_convolution_only": peak / 1e9,
+                      "dense_fine_grid_gb_if_materialised": cfg.npix_x * cfg.npix_y * cfg.sub ** 2 * cfg.nticks * 4 / 1e9,
+                      "max_abs_diff_vs_block_sparse_over_max": err, "pixels_compared": int(pix.numel())}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -355,10 +469,13 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--ref-segments", type=int, default=0, help="oracle sample size (0 = per config)")
     ap.add_argument("--work-gb", type=int, default=0, help="tred_convolve workspace cap (GiB), 0 = default")
+    ap.add_argument("--budget-gb", type=int, default=10, help="config 4: block payload per chunk (GiB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.config == 5:
+        return run_sweep(args)
     return run_cuda(args)
 
 

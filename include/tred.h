@@ -226,13 +226,23 @@ int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys, const f
  * tred_gather_waveforms -- overlap-add: every tile
  * (pixel, Tt = Bt ticks) is the sum, in ascending slab order, of the slab outputs that
  * cover it; optionally also writes dense rows for requested pixels.
- *   d_tile_keys [ntiles] from tred_convolve_plan; d_tile_data [ntiles][Bt] float32 out
+ *   d_plan_work      plan of the blocks d_sp_data belongs to (its slab-pixel index map)
+ *   d_tile_plan_work plan whose tile list d_tile_keys / d_tile_data follow (NULL: the same
+ *                    plan).  A chunked run (config 4: bounded sets of occupied blocks,
+ *                    PAPER.md:L242-250) makes one plan over all block keys for the tile
+ *                    list and one per chunk of time slabs for the convolution.
+ *   tile_begin, ntiles  the range of the tile list this call fills
+ *   d_tile_keys [.] from tred_convolve_plan; d_tile_data [.][Bt] float32 in/out
+ *   accumulate  0: tiles are overwritten; 1: the slab outputs are added onto the values
+ *               already there (chunks processed in ascending slab order give the same
+ *               sequence of additions, hence the same bits, as a single pass)
  *   d_pix_ids   [npix_req] int32 flat pixel ids px*npix_y+py (may be NULL if npix_req=0)
- *   d_dense     [npix_req][nticks] float32 out (may be NULL)
+ *   d_dense     [npix_req][nticks] float32 out (may be NULL), read from d_tile_data
  */
 int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_sp_data,
-                          const void* d_plan_work,
-                          int64_t ntiles, const int64_t* d_tile_keys, float* d_tile_data,
+                          const void* d_plan_work, const void* d_tile_plan_work,
+                          int64_t tile_begin, int64_t ntiles, const int64_t* d_tile_keys,
+                          float* d_tile_data, int accumulate,
                           int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
                           void* stream);
 

@@ -72,8 +72,8 @@ EXPORTS = {
                                 _c_i64, _c_p, _c_p,
                                 _c_p,
                                 _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
-    "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p,
-                                        _c_p]),
+    "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_i64, _c_i64, _c_p, _c_p, C.c_int,
+                                        _c_i64, _c_p, _c_p, _c_p]),
     "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
     "tred_profile_end": (C.c_int, [_c_p, C.c_int, _c_p, _c_p]),
     "tred_stage_count": (C.c_int, []),
@@ -309,19 +309,25 @@ class Tred:
                "tred_convolve")
         return sp_data
 
-    def gather_waveforms(self, nsp: int, sp_data, plan: dict, ntiles: int, pix_ids=None):
+    def gather_waveforms(self, nsp: int, sp_data, plan: dict, ntiles: int, pix_ids=None, tile_plan=None,
+                         tile_data=None, tile_begin: int = 0, accumulate: bool = False):
+        """`plan`: plan of the blocks sp_data belongs to; `tile_plan` (default: the same): plan
+        whose tile list is filled; [tile_begin, tile_begin + ntiles) is the range of it."""
         t = self.torch
         Bt = self.cfg.block[2]
-        tile_data = self._empty((max(ntiles, 1), Bt), t.float32)
+        tp = plan if tile_plan is None else tile_plan
+        if tile_data is None:
+            tile_data = self._empty((max(ntiles, 1), Bt), t.float32)
         dense = None
         npix = 0
         if pix_ids is not None and pix_ids.numel() > 0:
             assert pix_ids.dtype == t.int32 and pix_ids.is_cuda
             npix = pix_ids.numel()
             dense = self._empty((npix, self.cfg.nticks), t.float32)
-        _check(self.L.tred_gather_waveforms(self.h, nsp, _ptr(sp_data), _ptr(plan["work"]), ntiles,
-                                            _ptr(plan["tile_keys"]), _ptr(tile_data), npix, _ptr(pix_ids),
-                                            _ptr(dense), self._stream()), "tred_gather_waveforms")
+        _check(self.L.tred_gather_waveforms(self.h, nsp, _ptr(sp_data), _ptr(plan["work"]), _ptr(tp["work"]),
+                                            tile_begin, ntiles, _ptr(tp["tile_keys"]), _ptr(tile_data),
+                                            1 if accumulate else 0, npix, _ptr(pix_ids), _ptr(dense),
+                                            self._stream()), "tred_gather_waveforms")
         return tile_data, dense
 
     # -- whole path -----------------------------------------------------------------
@@ -351,3 +357,69 @@ class Tred:
                        pair_seg=pair_seg[:cap_pairs], slab_off=slab_off, payload=payload[:nblocks],
                        sp_keys=sp_keys[:nsp], sp_data=sp_data[:nsp], sp_off=sp_off)
         return out
+
+    # -- whole path in bounded-memory chunks of occupied blocks (BASELINE config 4) --------
+    def simulate_chunked(self, seg, rhat, pix_ids=None, payload_budget_bytes: int = 8 << 30):
+        """Same result as `simulate`, bit for bit, with the block payload, the convolution
+        workspace and the slab outputs held for one range of time slabs at a time
+        (chunks bounded by device memory).  The occupied blocks are
+        sorted slab-major, so a chunk is a contiguous range of the block list whose payload
+        fits `payload_budget_bytes`; a slab's output depends on that slab's blocks only, and
+        the overlap-add continues the running sum of the tiles (`accumulate`)."""
+        t = self.torch
+        import numpy as np
+        nseg = seg.shape[1]
+        NBt = int(self.dims.NB[2])
+        Bt = self.cfg.block[2]
+        npix = self.cfg.npix_x * self.cfg.npix_y
+        augf, augi, npairs = self.drift(seg)
+        cap_pairs = int(npairs.item())
+        keys, blk_off, pair_seg, slab_off, nblocks_d = self.blockbin(augi, cap_pairs)
+        nblocks = int(nblocks_d.item())
+        so = slab_off.cpu().numpy().astype(np.int64)
+        gplan = self.convolve_plan(nblocks, keys)                    # tile list of the whole event
+        ntiles = int(gplan["ntiles"].item())
+        tile_keys = gplan["tile_keys"]
+        tile_data = t.zeros((max(ntiles, 1), Bt), dtype=t.float32, device=self.device)
+        # first tile of every time tile index tb (tile keys are sorted, tb-major)
+        bounds = t.arange(0, NBt + self.dims.n_over + 1, device=self.device, dtype=t.int64) * npix
+        tile_lo = t.searchsorted(tile_keys[:ntiles], bounds).cpu().numpy()
+        blk_bytes = int(self.dims.block_floats) * 4
+        max_blk = max(1, int(payload_budget_bytes) // blk_bytes)
+        payload = None
+        chunks = []
+        b0 = 0
+        while b0 < NBt:
+            if so[b0 + 1] == so[b0]:
+                b0 += 1
+                continue
+            b1 = b0 + 1
+            while b1 < NBt and so[b1 + 1] - so[b0] <= max_blk:
+                b1 += 1
+            k0, k1 = int(so[b0]), int(so[b1])
+            nb = k1 - k0
+            if payload is None or payload.shape[0] < nb:
+                payload = None
+                payload = self._empty((nb, self.cfg.block[0], self.cfg.block[1], Bt), t.float32)
+            kc = keys[k0:k1]
+            self.effq(nb, kc, blk_off[k0:k1 + 1], pair_seg, augf, augi, payload=payload)
+            plan = self.convolve_plan(nb, kc)
+            counts = t.cat([plan["ncp"], plan["nsp"], plan["cp_off"].to(t.int64), plan["sp_off"].to(t.int64),
+                            plan["rt_off"].to(t.int64)]).cpu().numpy()
+            ncp, nsp = int(counts[0]), int(counts[1])
+            co, po, ro = (counts[2 + i * (NBt + 1):2 + (i + 1) * (NBt + 1)] for i in range(3))
+            sp_data = self.convolve(nb, kc, payload, rhat, plan, ncp, nsp, co, po, rt_off_host=ro)
+            t_lo = int(tile_lo[b0])
+            t_hi = int(tile_lo[min(b1 - 1 + self.dims.n_over, NBt + self.dims.n_over)])
+            if t_hi > t_lo:
+                self.gather_waveforms(nsp, sp_data, plan, t_hi - t_lo, tile_plan=gplan, tile_data=tile_data,
+                                      tile_begin=t_lo, accumulate=True)
+            chunks.append((b0, b1, nb, ncp, nsp))
+            del plan, sp_data
+            b0 = b1
+        dense = None
+        if pix_ids is not None and pix_ids.numel() > 0:
+            _, dense = self.gather_waveforms(0, None, gplan, 0, pix_ids=pix_ids, tile_data=tile_data)
+        return dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ntiles=ntiles, tile_keys=tile_keys[:ntiles],
+                    tile_data=tile_data[:ntiles], dense=dense, chunks=chunks,
+                    ncp=sum(c[3] for c in chunks), nsp=sum(c[4] for c in chunks))

@@ -654,16 +654,18 @@ k_ifft_ct(const float2* __restrict__ ohat, int s0, int ns, int sbase, float* __r
 
 // ------------------------------------------------------------------ (e) S5 overlap-add
 __global__ void __launch_bounds__(256)
-k_gather_tiles(int64_t ntiles, const int64_t* __restrict__ tile_keys, const int32_t* __restrict__ sp_idx,
-               const float* __restrict__ sp_data, float* __restrict__ tile_data, TredGrid g) {
-  const int64_t tile = blockIdx.x;
+k_gather_tiles(int64_t tile_begin, const int64_t* __restrict__ tile_keys, const int32_t* __restrict__ sp_idx,
+               const float* __restrict__ sp_data, float* __restrict__ tile_data, int accumulate, TredGrid g) {
+  const int64_t tile = tile_begin + blockIdx.x;
   const int64_t key = tile_keys[tile];
   const int64_t npix = (int64_t)g.npx * g.npy;
   const int tb = (int)(key / npix);
   const int64_t p = key - tb * npix;
   const int row = g.nover * g.Bt;
   for (int t = threadIdx.x; t < g.Bt; t += blockDim.x) {
-    float acc = 0.0f;
+    // accumulate: continue the running sum left by the earlier chunks (slab ranges in
+    // ascending order), so the additions are the same sequence as in one pass
+    float acc = accumulate ? tile_data[tile * g.Bt + t] : 0.0f;
     for (int bt = max(tb - g.nover + 1, 0); bt <= tb; ++bt) {        // ascending slab order
       const int64_t m = bt * npix + p;
       const int i0 = sp_idx[m];
@@ -1158,25 +1160,28 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
 }
 
 extern "C" int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_sp_data,
-                                     const void* d_plan_work,
-                                     int64_t ntiles, const int64_t* d_tile_keys, float* d_tile_data,
+                                     const void* d_plan_work, const void* d_tile_plan_work,
+                                     int64_t tile_begin, int64_t ntiles, const int64_t* d_tile_keys,
+                                     float* d_tile_data, int accumulate,
                                      int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
                                      void* stream) {
-  if (!ctx || nsp < 0 || ntiles < 0 || npix_req < 0 || !d_plan_work) return TRED_EINVAL;
+  if (!ctx || nsp < 0 || ntiles < 0 || tile_begin < 0 || npix_req < 0 || !d_plan_work) return TRED_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);
   PlanWork w = carve_plan(ctx, (void*)d_plan_work);
+  const PlanWork wt = carve_plan(ctx, (void*)(d_tile_plan_work ? d_tile_plan_work : d_plan_work));
   TredProfScope ps(ctx, ST_GATHER, st);
   TRED_COUNT_LAUNCH((ntiles > 0 ? 1 : 0) + (npix_req > 0 ? 1 : 0));
   if (ntiles > 0) {
     if (!d_tile_keys || !d_tile_data || (nsp > 0 && !d_sp_data)) return TRED_EINVAL;
     if (ntiles >= (1ll << 31)) return TRED_EUNSUPPORTED;
     k_gather_tiles<<<(unsigned)ntiles, g.Bt < 256 ? (g.Bt < 32 ? 32 : g.Bt) : 256, 0, st>>>(
-        ntiles, d_tile_keys, w.sp_idx, d_sp_data, d_tile_data, g);
+        tile_begin, d_tile_keys, w.sp_idx, d_sp_data, d_tile_data, accumulate, g);
   }
   if (npix_req > 0) {
     if (!d_pix_ids || !d_dense) return TRED_EINVAL;
-    k_gather_dense<<<(unsigned)npix_req, 256, 0, st>>>(npix_req, d_pix_ids, w.tile_idx, d_tile_data, d_dense, g);
+    if (!d_tile_data) return TRED_EINVAL;
+    k_gather_dense<<<(unsigned)npix_req, 256, 0, st>>>(npix_req, d_pix_ids, wt.tile_idx, d_tile_data, d_dense, g);
   }
   TRED_LAUNCH_CHECK("gather_waveforms");
   return TRED_OK;
