@@ -209,6 +209,7 @@ def run_cuda(args):
     # ---- warm-up
     out = None
     for _ in range(max(args.warmup, 3)):
+        out = None                          # a step's outputs are released before the next step
         out = simulate(seg_d)
     barrier()
     info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles")}
@@ -224,7 +225,9 @@ def run_cuda(args):
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     t_wall0 = time.perf_counter()
+    torch.cuda.reset_peak_memory_stats(dev)
     for a, b in ev:
+        out = None
         flush.zero_()                       # flush L2 between timed iterations
         a.record()
         out = simulate(seg_d)
@@ -232,6 +235,9 @@ def run_cuda(args):
     barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
+    peak_mem = torch.cuda.max_memory_allocated(dev)
+    nchunks = len(out.get("chunks", [])) or 1
+    out = None
     launches = sum(v[1] for v in sim.profile_end().values())
     ms_steps = [a.elapsed_time(b) for a, b in ev]
     ms = float(np.mean(ms_steps))
@@ -253,7 +259,9 @@ def run_cuda(args):
     e2e_ms = []
     h2d = seg_pinned.numel() * 4
     d2h = 0
+    o2 = keys_h = data_h = None
     for i in range(args.steps + 1):
+        o2 = None
         flush.zero_()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -332,7 +340,7 @@ def run_cuda(args):
                            "block": list(cfg.block), "resp_nticks": cfg.resp_nticks, "fft_len": d.fft_len,
                            "l2": "flushed between timed iterations (256 MiB write)",
                            "parallelism": f"events x{world}, no collective",
-                           "chunks": len(out.get("chunks", [])) or 1, **info},
+                           "chunks": nchunks, **info},
                 "e2e": {"value": total_seg / (e2e_max * 1e-3), "unit": UNIT, "ms_per_step": e2e_max,
                         "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
                 "gpu_launches": int(launches),
@@ -343,7 +351,7 @@ def run_cuda(args):
                                        for kk, vv in v.items() if kk in ("bound", "achieved", "peak", "unit", "frac",
                                                                           "traffic")}
                                    for k, v in stage_roof.items()},
-                "peak_mem_gb": torch.cuda.max_memory_allocated(dev) / 1e9,
+                "peak_mem_gb": peak_mem / 1e9,
                 "payload_gb": payload_gb,
                 "wall_s_timed_region": t_wall}
         if not args.no_cpu_baseline and world == 1:

@@ -351,6 +351,108 @@ k_fft_fwd_ct(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   }
 }
 
+// Forward FFT, two-step form for the zero-padded columns (only the first Bt/2 of the
+// M complex samples are non-zero).  M = A B with B a power of two, sample n = B a + b,
+// frequency k = ka + A kb:
+//   step 1 (thread per column and b):  Y_b[ka] = sum_{a < nza} z[B a + b] W_M^{(B a + b) ka}
+//           -- a pruned DFT, nza = ceil(Bt / 2 / B) <= 4 terms, twiddles by recurrence;
+//   step 2 (thread per column and ka): X[ka + A kb] = sum_b Y_b[ka] W_B^{b kb}
+//           -- a B-point FFT held in registers (fft_reg_dif);
+//   then the half-length real-FFT post-processing on pairs (k, M - k).
+// One shared-memory round trip between the steps and one before the post-processing,
+// instead of one per radix pass.  CG = 20 columns (S = 10, two phase rows) per CTA.
+template <int M, int B>
+__global__ void __launch_bounds__((20 * (M / B) + 31) / 32 * 32)
+k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
+             RowSrc rs, int rp, float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g) {
+  constexpr int A = M / B, CG = 20, S = 10, JG = 2, NGRP = 5, NPH = 100;
+  constexpr int NT = (CG * A + 31) / 32 * 32;
+  constexpr int BP = B + 1, ZP = M + 1;
+  constexpr int LOGB = tred_log2(B);
+  extern __shared__ float2 buf[];           // step 1 -> 2: [col][ka][b (+1)]; then Z: [col][k (+1)]
+  __shared__ long long colbase[CG];
+  const int row = blockIdx.x / NGRP, grp = blockIdx.x - row * NGRP;
+  int px, py, bt;
+  if (!row_pixel(rs, row, g, px, py, bt)) return;
+  if (threadIdx.x < CG) {
+    const int jx = grp * JG + threadIdx.x / S, jy = threadIdx.x % S;
+    const int i = px * S + jx, j = py * S + jy;
+    const int bx = i / g.Bx, by = j / g.By;
+    const int slot = blockmap[((int64_t)bt * g.NBx + bx) * g.NBy + by];
+    long long base = -1;
+    if (slot >= 0) base = (((long long)slot * g.Bx + (i - bx * g.Bx)) * g.By + (j - by * g.By)) * g.Bt;
+    colbase[threadIdx.x] = base;
+  }
+  __syncthreads();
+  const int hb = g.Bt >> 1;
+  // ---- step 1
+  for (int it = threadIdx.x; it < CG * B; it += NT) {
+    const int c = it / B, b = it - c * B;
+    const long long base = colbase[c];
+    float2 p[4], w[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const int n = B * a + b;
+      p[a] = make_float2(0.0f, 0.0f);
+      w[a] = make_float2(1.0f, 0.0f);
+      if (n < hb && base >= 0) {
+        p[a] = __ldg(reinterpret_cast<const float2*>(payload + base + 2 * n));
+        w[a] = __ldg(gtw + 2 * n);                       // W_M^n = exp(-2 pi i 2n / N)
+      }
+    }
+    float2* dst = buf + (c * A) * BP + b;
+#pragma unroll
+    for (int ka = 0; ka < A; ++ka) {
+      dst[ka * BP] = make_float2((p[0].x + p[1].x) + (p[2].x + p[3].x), (p[0].y + p[1].y) + (p[2].y + p[3].y));
+#pragma unroll
+      for (int a = 0; a < 4; ++a) p[a] = cmulf(p[a], w[a]);
+    }
+  }
+  __syncthreads();
+  // ---- step 2
+  {
+    const int it = threadIdx.x;                            // NT >= CG * A: one item per thread
+    float2 y[B];
+    const bool on = it < CG * A;
+    const int c = it / A, ka = it - c * A;
+    if (on) {
+      const float2* src = buf + it * BP;
+#pragma unroll
+      for (int b = 0; b < B; ++b) y[b] = src[b];
+      fft_reg_dif<B>(y);
+    }
+    __syncthreads();                                       // every Y read before Z overwrites the buffer
+    if (on) {
+      float2* z = buf + c * ZP + ka;
+#pragma unroll
+      for (int q = 0; q < B; ++q) z[A * tred_bitrev(q, LOGB)] = y[q];
+    }
+  }
+  __syncthreads();
+  // ---- real-FFT post-processing on pairs (k, M - k); slot 0 packs (DC, Nyquist)
+  float2* out = qhat + (int64_t)row * NPH + grp * CG;
+  const int64_t fstride = (int64_t)rp * NPH;
+  constexpr int NPAIR = M / 2 + 1;
+  for (int it = threadIdx.x; it < NPAIR * CG; it += NT) {
+    const int k = it / CG, c = it - k * CG;
+    const float2* Z = buf + c * ZP;
+    if (k == 0) {
+      const float2 z0 = Z[0];
+      out[c] = make_float2(z0.x + z0.y, z0.x - z0.y);
+    } else if (2 * k == M) {
+      const float2 z = Z[k];                                // X[M/2] = conj(Z[M/2])
+      out[k * fstride + c] = make_float2(z.x, -z.y);
+    } else {
+      const float2 pz = Z[k], qz = Z[M - k];
+      const float2 e = make_float2(0.5f * (pz.x + qz.x), 0.5f * (pz.y - qz.y));
+      const float2 o = make_float2(0.5f * (pz.x - qz.x), 0.5f * (pz.y + qz.y));
+      const float2 wo = cmulf(__ldg(gtw + k), o);
+      out[k * fstride + c] = make_float2(e.x + wo.y, e.y - wo.x);              // X[k]
+      out[(M - k) * fstride + c] = make_float2(e.x - wo.y, -e.y - wo.x);       // X[M-k]
+    }
+  }
+}
+
 // ------------------------------------------------------------------ (b) spectrum product, fp32 FMA
 // T[f][off][row] = sum_phase qhat[f][row][phase] * W[f][phase][off]  (complex).
 // grid (nf, Y).  CTA: W[f] in shared memory; tiles of MT rows x all offsets; thread tile
@@ -720,6 +822,35 @@ static int launch_fft_fwd_ct(const tred_ctx* ctx, const TredGrid& g, const float
   }
 }
 
+#define TRED_FFT_2S_SHAPES(X) X(128, 32) X(144, 16) X(256, 32) X(288, 32) X(384, 32) X(512, 32)
+
+static int launch_fft_fwd_2s(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
+                             const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
+  if (g.S != 10 || nr < 1) return 0;
+  const int M = g.L / 2, hb = g.Bt / 2;
+  switch (M) {
+#define X(MM, BB)                                                                                          \
+  case MM: {                                                                                               \
+    constexpr int A = MM / BB;                                                                             \
+    constexpr int NT = (20 * A + 31) / 32 * 32;                                                            \
+    constexpr size_t smem = sizeof(float2) * (size_t)((20 * A * (BB + 1) > 20 * (MM + 1)) ? 20 * A * (BB + 1) \
+                                                                                           : 20 * (MM + 1)); \
+    if (hb > 4 * BB || smem > (size_t)ctx->smem_optin) return 0;                                           \
+    static bool set = false;                                                                               \
+    if (!set) {                                                                                            \
+      TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
+                                     (int)smem));                                                          \
+      set = true;                                                                                          \
+    }                                                                                                      \
+    k_fft_fwd_2s<MM, BB><<<(unsigned)(nr * 5), NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);    \
+    return 1;                                                                                              \
+  }
+    TRED_FFT_2S_SHAPES(X)
+#undef X
+    default: return 0;
+  }
+}
+
 static int launch_ifft_ct(const tred_ctx* ctx, const TredGrid& g, const float2* ohat, int s0, int ns, int sbase,
                           float* sp_data, const float2* tw, int out_len, cudaStream_t st) {
   constexpr int IP = 8;
@@ -890,7 +1021,8 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{nullptr, 0, pw.rt_desc, pw.row_m2, t0, rg.nstrip, 1};
-        const int ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
+        int ct = launch_fft_fwd_2s(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
+        if (ct == 0) ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
         if (ct < 0) return ct;
         if (ct == 0)
           k_fft_fwd<<<(unsigned)(rp * ngrp), 256, fwd_smem(JG), st>>>(d_payload, w.blockmap, rs, rp, JG, w.qhat,
@@ -1106,7 +1238,8 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{d_cp_keys, r0, nullptr, nullptr, 0, 0, 0};
-        const int ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
+        int ct = launch_fft_fwd_2s(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
+        if (ct == 0) ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
         if (ct < 0) return ct;
         if (ct == 0)
           k_fft_fwd<<<(unsigned)(nr * ngrp), 256, fwd_smem(JG), st>>>(d_payload, w.blockmap, rs, rp, JG, w.qhat,

@@ -233,3 +233,56 @@ __device__ __forceinline__ float2* fft_stockham_ct(float2* a, float2* b, const f
     return fft_stockham_ct<M, NS * R, INV, NB, NT>(b, a, twN, M);
   }
 }
+
+// ---------------------------------------------------------------------------------
+// In-register radix-2 decimation-in-frequency FFT of B = 8, 16 or 32 points (forward).
+// Fully unrolled: every index and twiddle is a compile-time constant.  Element p of the
+// result holds X[bitrev_B(p)].
+__device__ constexpr float TRED_C32[17] = {
+    1.0f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f,
+    0.55557023301960218f, 0.38268343236508978f, 0.19509032201612825f, 0.0f, -0.19509032201612825f,
+    -0.38268343236508978f, -0.55557023301960218f, -0.70710678118654752f, -0.83146961230254524f,
+    -0.92387953251128674f, -0.98078528040323043f, -1.0f};
+__device__ constexpr float TRED_S32[17] = {
+    0.0f, 0.19509032201612825f, 0.38268343236508978f, 0.55557023301960218f, 0.70710678118654752f,
+    0.83146961230254524f, 0.92387953251128674f, 0.98078528040323043f, 1.0f, 0.98078528040323043f,
+    0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f, 0.55557023301960218f,
+    0.38268343236508978f, 0.19509032201612825f, 0.0f};
+
+__host__ __device__ constexpr int tred_bitrev(int x, int bits) {
+  int r = 0;
+  for (int i = 0; i < bits; ++i) r |= ((x >> i) & 1) << (bits - 1 - i);
+  return r;
+}
+__host__ __device__ constexpr int tred_log2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
+
+template <int B, int H> struct FftRegStage {
+  static __device__ __forceinline__ void run(float2 (&y)[B]) {
+    constexpr float HS = 0.70710678118654752f;
+#pragma unroll
+    for (int i0 = 0; i0 < B; i0 += 2 * H) {
+#pragma unroll
+      for (int j = 0; j < H; ++j) {
+        const float2 a = y[i0 + j], b = y[i0 + j + H];
+        y[i0 + j] = make_float2(a.x + b.x, a.y + b.y);
+        const float2 d = make_float2(a.x - b.x, a.y - b.y);
+        const int t = j * (16 / H);                        // twiddle exp(-2 pi i t / 32)
+        float2 r;
+        if (t == 0) r = d;
+        else if (t == 8) r = make_float2(d.y, -d.x);
+        else if (t == 4) r = make_float2(HS * (d.x + d.y), HS * (d.y - d.x));
+        else if (t == 12) r = make_float2(HS * (d.y - d.x), -HS * (d.x + d.y));
+        else r = make_float2(d.x * TRED_C32[t] + d.y * TRED_S32[t], d.y * TRED_C32[t] - d.x * TRED_S32[t]);
+        y[i0 + j + H] = r;
+      }
+    }
+    FftRegStage<B, H / 2>::run(y);
+  }
+};
+template <int B> struct FftRegStage<B, 0> {
+  static __device__ __forceinline__ void run(float2 (&)[B]) {}
+};
+template <int B> __device__ __forceinline__ void fft_reg_dif(float2 (&y)[B]) {
+  static_assert(B == 8 || B == 16 || B == 32, "register FFT sizes");
+  FftRegStage<B, B / 2>::run(y);
+}
