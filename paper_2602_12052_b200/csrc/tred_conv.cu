@@ -361,7 +361,7 @@ k_fft_fwd_ct(const float* __restrict__ payload, const int32_t* __restrict__ bloc
 //   then the half-length real-FFT post-processing on pairs (k, M - k).
 // One shared-memory round trip between the steps and one before the post-processing,
 // instead of one per radix pass.  CG = 20 columns (S = 10, two phase rows) per CTA.
-template <int M, int B>
+template <int M, int B, int NZA>
 __global__ void __launch_bounds__((20 * (M / B) + 31) / 32 * 32)
 k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
              RowSrc rs, int rp, float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g) {
@@ -389,23 +389,31 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   for (int it = threadIdx.x; it < CG * B; it += NT) {
     const int c = it / B, b = it - c * B;
     const long long base = colbase[c];
-    float2 p[4], w[4];
+    float2* dst = buf + (c * A) * BP + b;
+    if (base < 0) {                                        // column outside the occupied blocks
 #pragma unroll
-    for (int a = 0; a < 4; ++a) {
+      for (int ka = 0; ka < A; ++ka) dst[ka * BP] = make_float2(0.0f, 0.0f);
+      continue;
+    }
+    float2 p[NZA], w[NZA];
+#pragma unroll
+    for (int a = 0; a < NZA; ++a) {
       const int n = B * a + b;
       p[a] = make_float2(0.0f, 0.0f);
       w[a] = make_float2(1.0f, 0.0f);
-      if (n < hb && base >= 0) {
+      if (n < hb) {
         p[a] = __ldg(reinterpret_cast<const float2*>(payload + base + 2 * n));
         w[a] = __ldg(gtw + 2 * n);                       // W_M^n = exp(-2 pi i 2n / N)
       }
     }
-    float2* dst = buf + (c * A) * BP + b;
 #pragma unroll
     for (int ka = 0; ka < A; ++ka) {
-      dst[ka * BP] = make_float2((p[0].x + p[1].x) + (p[2].x + p[3].x), (p[0].y + p[1].y) + (p[2].y + p[3].y));
+      float2 acc = p[0];
 #pragma unroll
-      for (int a = 0; a < 4; ++a) p[a] = cmulf(p[a], w[a]);
+      for (int a = 1; a < NZA; ++a) { acc.x += p[a].x; acc.y += p[a].y; }
+      dst[ka * BP] = acc;
+#pragma unroll
+      for (int a = 0; a < NZA; ++a) p[a] = cmulf(p[a], w[a]);
     }
   }
   __syncthreads();
@@ -415,11 +423,15 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
     float2 y[B];
     const bool on = it < CG * A;
     const int c = it / A, ka = it - c * A;
-    if (on) {
+    const bool live = on && colbase[c] >= 0;
+    if (live) {
       const float2* src = buf + it * BP;
 #pragma unroll
       for (int b = 0; b < B; ++b) y[b] = src[b];
       fft_reg_dif<B>(y);
+    } else {
+#pragma unroll
+      for (int b = 0; b < B; ++b) y[b] = make_float2(0.0f, 0.0f);
     }
     __syncthreads();                                       // every Y read before Z overwrites the buffer
     if (on) {
@@ -824,6 +836,23 @@ static int launch_fft_fwd_ct(const tred_ctx* ctx, const TredGrid& g, const float
 
 #define TRED_FFT_2S_SHAPES(X) X(128, 32) X(144, 16) X(256, 32) X(288, 32) X(384, 32) X(512, 32)
 
+template <int MM, int BB, int NZA>
+static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
+                               const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
+  constexpr int A = MM / BB;
+  constexpr int NT = (20 * A + 31) / 32 * 32;
+  constexpr size_t smem =
+      sizeof(float2) * (size_t)((20 * A * (BB + 1) > 20 * (MM + 1)) ? 20 * A * (BB + 1) : 20 * (MM + 1));
+  if (smem > (size_t)ctx->smem_optin) return 0;
+  static bool set = false;
+  if (!set) {
+    TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    set = true;
+  }
+  k_fft_fwd_2s<MM, BB, NZA><<<(unsigned)(nr * 5), NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);
+  return 1;
+}
+
 static int launch_fft_fwd_2s(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
                              const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
   if (g.S != 10 || nr < 1) return 0;
@@ -831,19 +860,11 @@ static int launch_fft_fwd_2s(const tred_ctx* ctx, const TredGrid& g, const float
   switch (M) {
 #define X(MM, BB)                                                                                          \
   case MM: {                                                                                               \
-    constexpr int A = MM / BB;                                                                             \
-    constexpr int NT = (20 * A + 31) / 32 * 32;                                                            \
-    constexpr size_t smem = sizeof(float2) * (size_t)((20 * A * (BB + 1) > 20 * (MM + 1)) ? 20 * A * (BB + 1) \
-                                                                                           : 20 * (MM + 1)); \
-    if (hb > 4 * BB || smem > (size_t)ctx->smem_optin) return 0;                                           \
-    static bool set = false;                                                                               \
-    if (!set) {                                                                                            \
-      TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
-                                     (int)smem));                                                          \
-      set = true;                                                                                          \
-    }                                                                                                      \
-    k_fft_fwd_2s<MM, BB><<<(unsigned)(nr * 5), NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);    \
-    return 1;                                                                                              \
+    const int nza = (hb + BB - 1) / BB;                                                                    \
+    if (nza <= 1) return launch_fft_fwd_2s_t<MM, BB, 1>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    if (nza == 2) return launch_fft_fwd_2s_t<MM, BB, 2>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    if (nza <= 4) return launch_fft_fwd_2s_t<MM, BB, 4>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    return 0;                                                                                              \
   }
     TRED_FFT_2S_SHAPES(X)
 #undef X

@@ -112,23 +112,36 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
   for (int i = threadIdx.x; i < P.TS * P.plane; i += NT) tile[i] = 0.0f;
   // the first __syncthreads of the segment loop (or the one after it) orders this
 
+  // Segment records of the block are staged in shared memory SB at a time (one pass of
+  // coalesced loads instead of two dependent global loads per segment and thread).
+  constexpr int SB = 32, NF = 17;                      // 7 int fields (bbox, flag) + 10 floats
+  __shared__ int32_t s_rec[SB][NF + 1];
   const int s_beg = blk_off[blk], s_end = blk_off[blk + 1];
   int it = 0;
-  for (int si = s_beg; si < s_end; ++si) {
-    const int s = pair_seg[si];
-    const int lox = augi[0 * nseg + s], loy = augi[1 * nseg + s], lot = augi[2 * nseg + s];
-    const int hix = augi[3 * nseg + s], hiy = augi[4 * nseg + s], hit = augi[5 * nseg + s];
+  for (int b0 = s_beg; b0 < s_end; b0 += SB) {
+  const int nbatch = min(SB, s_end - b0);
+  __syncthreads();                                     // the previous batch's records are no longer read
+  for (int e = threadIdx.x; e < nbatch * NF; e += NT) {
+    const int j = e / NF, f = e - j * NF;
+    const int64_t s = pair_seg[b0 + j];
+    s_rec[j][f] = f < 7 ? augi[f * nseg + s] : __float_as_int(augf[(f - 7) * nseg + s]);
+  }
+  __syncthreads();
+  for (int sj = 0; sj < nbatch; ++sj) {
+    const int32_t* rec = s_rec[sj];
+    const int lox = rec[0], loy = rec[1], lot = rec[2];
+    const int hix = rec[3], hiy = rec[4], hit = rec[5];
     // grid points of the segment's footprint inside this tile (and the grid)
     const int ix0 = max(lox - E, I0), ix1 = min(min(hix + E, I0 + g.Bx - 1), g.NGx - 1);
     const int iy0 = max(loy - E, J0), iy1 = min(min(hiy + E, J0 + g.By - 1), g.NGy - 1);
     const int kt0 = max(lot - E, K0), kt1 = min(min(hit + E, K0 + P.TS - 1), g.NGt - 1);
     if (ix0 > ix1 || iy0 > iy1 || kt0 > kt1) continue;            // CTA-uniform
     const int nx = ix1 - ix0 + 1, ny = iy1 - iy0 + 1, nt = kt1 - kt0 + 1;
-    const int flag = augi[6 * nseg + s];
-    const float p0x = augf[0 * nseg + s], p0y = augf[1 * nseg + s], p0t = augf[2 * nseg + s];
-    const float p1x = augf[3 * nseg + s], p1y = augf[4 * nseg + s], p1t = augf[5 * nseg + s];
-    const float sx = augf[6 * nseg + s], sy = augf[7 * nseg + s], st = augf[8 * nseg + s];
-    const float Qp = augf[9 * nseg + s];
+    const int flag = rec[6];
+    const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
+    const float p1x = __int_as_float(rec[10]), p1y = __int_as_float(rec[11]), p1t = __int_as_float(rec[12]);
+    const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
+    const float Qp = __int_as_float(rec[16]);
     const float dx = p1x - p0x, dy = p1y - p0y, dt = p1t - p0t;
     const float k2x = LOG2E_HALF / (sx * sx), k2y = LOG2E_HALF / (sy * sy), k2t = LOG2E_HALF / (st * st);
     const float K = Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f;   // (2 pi)^-3/2 / 8
@@ -196,6 +209,7 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
       // no barrier here: the next phase A writes the other table set, and its barrier
       // orders this phase B before the next one
     }
+  }
   }
   __syncthreads();
   // tile -> payload[blk][i][j][k], k contiguous
