@@ -369,6 +369,7 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   constexpr int NT = (CG * A + 31) / 32 * 32;
   constexpr int BP = B + 1, ZP = M + 1;
   constexpr int LOGB = tred_log2(B);
+  static_assert(NT % B == 0, "step 1 keeps one b per thread");
   extern __shared__ float2 buf[];           // step 1 -> 2: [col][ka][b (+1)]; then Z: [col][k (+1)]
   __shared__ long long colbase[CG];
   const int row = blockIdx.x / NGRP, grp = blockIdx.x - row * NGRP;
@@ -385,35 +386,48 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   }
   __syncthreads();
   const int hb = g.Bt >> 1;
-  // ---- step 1
-  for (int it = threadIdx.x; it < CG * B; it += NT) {
-    const int c = it / B, b = it - c * B;
-    const long long base = colbase[c];
-    float2* dst = buf + (c * A) * BP + b;
-    if (base < 0) {                                        // column outside the occupied blocks
-#pragma unroll
-      for (int ka = 0; ka < A; ++ka) dst[ka * BP] = make_float2(0.0f, 0.0f);
-      continue;
-    }
-    float2 p[NZA], w[NZA];
+  // ---- step 1 (NT is a multiple of B: a thread keeps the same b for all its columns; all
+  // global loads are issued before the arithmetic)
+  {
+    constexpr int NIT = (CG * B + NT - 1) / NT;
+    const int b = threadIdx.x % B;
+    float2 w[NZA], p[NIT][NZA];
 #pragma unroll
     for (int a = 0; a < NZA; ++a) {
       const int n = B * a + b;
-      p[a] = make_float2(0.0f, 0.0f);
-      w[a] = make_float2(1.0f, 0.0f);
-      if (n < hb) {
-        p[a] = __ldg(reinterpret_cast<const float2*>(payload + base + 2 * n));
-        w[a] = __ldg(gtw + 2 * n);                       // W_M^n = exp(-2 pi i 2n / N)
+      w[a] = n < hb ? __ldg(gtw + 2 * n) : make_float2(1.0f, 0.0f);       // W_M^n = exp(-2 pi i 2n / N)
+    }
+#pragma unroll
+    for (int i = 0; i < NIT; ++i) {
+      const int it = threadIdx.x + i * NT;
+      const long long base = it < CG * B ? colbase[it / B] : -1;
+#pragma unroll
+      for (int a = 0; a < NZA; ++a) {
+        const int n = B * a + b;
+        p[i][a] = (n < hb && base >= 0) ? __ldg(reinterpret_cast<const float2*>(payload + base + 2 * n))
+                                        : make_float2(0.0f, 0.0f);
       }
     }
 #pragma unroll
-    for (int ka = 0; ka < A; ++ka) {
-      float2 acc = p[0];
+    for (int i = 0; i < NIT; ++i) {
+      const int it = threadIdx.x + i * NT;
+      if (it >= CG * B) break;
+      const int c = it / B;
+      float2* dst = buf + (c * A) * BP + b;
+      if (colbase[c] < 0) {                                // column outside the occupied blocks
 #pragma unroll
-      for (int a = 1; a < NZA; ++a) { acc.x += p[a].x; acc.y += p[a].y; }
-      dst[ka * BP] = acc;
+        for (int ka = 0; ka < A; ++ka) dst[ka * BP] = make_float2(0.0f, 0.0f);
+        continue;
+      }
 #pragma unroll
-      for (int a = 0; a < NZA; ++a) p[a] = cmulf(p[a], w[a]);
+      for (int ka = 0; ka < A; ++ka) {
+        float2 acc = p[i][0];
+#pragma unroll
+        for (int a = 1; a < NZA; ++a) { acc.x += p[i][a].x; acc.y += p[i][a].y; }
+        dst[ka * BP] = acc;
+#pragma unroll
+        for (int a = 0; a < NZA; ++a) p[i][a] = cmulf(p[i][a], w[a]);
+      }
     }
   }
   __syncthreads();
@@ -445,6 +459,7 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   float2* out = qhat + (int64_t)row * NPH + grp * CG;
   const int64_t fstride = (int64_t)rp * NPH;
   constexpr int NPAIR = M / 2 + 1;
+#pragma unroll 4
   for (int it = threadIdx.x; it < NPAIR * CG; it += NT) {
     const int k = it / CG, c = it - k * CG;
     const float2* Z = buf + c * ZP;
