@@ -69,8 +69,10 @@ typedef struct tred_config {
                                     1 = closed form with erf per Gauss-Legendre node          */
   int32_t mac_mode;              /* spectrum multiply-accumulate of tred_convolve:
                                     0 = default: tensor cores (3xTF32) over row tiles with
-                                        the sum over the offsets fused into the epilogue,
-                                        if supported, else as 2, else as 1,
+                                        the sum over the offsets fused into the epilogue, on
+                                        CTA pairs (tcgen05 cta_group::2) if supported, else
+                                        as 3, else as 2, else as 1,
+                                    3 = as 0 on single CTAs,
                                     1 = fp32 FMA pipe, products written to memory,
                                     2 = tensor cores 3xTF32, products written to memory       */
 } tred_config;

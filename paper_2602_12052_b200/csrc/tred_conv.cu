@@ -993,8 +993,13 @@ bool tred_mac_tc_fused_supported(const tred_ctx* ctx);
 int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
                       int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
 
+// the same on CTA pairs (tred_mac_tc2.cu)
+bool tred_mac_tc2_supported(const tred_ctx* ctx);
+int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
+                 int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
+
 static bool use_tiled(const tred_ctx* ctx) {
-  return ctx->cfg.mac_mode != 1 && ctx->cfg.mac_mode != 2 && tred_mac_tc_fused_supported(ctx);
+  return (ctx->cfg.mac_mode == 0 || ctx->cfg.mac_mode == 3) && tred_mac_tc_fused_supported(ctx);
 }
 
 // Tensor-core path of tred_convolve: row tiles (tred_convolve_plan), forward FFT into
@@ -1067,8 +1072,13 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
       }
       {
         TredProfScope ps(ctx, ST_MAC, st);
-        const int rc = tred_mac_tc_fused(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl,
-                                         (float*)w.opart, nt, t0, pw.rt_desc, pw.row_m2, st);
+        int rc = TRED_EUNSUPPORTED;
+        if (ctx->cfg.mac_mode == 0 && tred_mac_tc2_supported(ctx))
+          rc = tred_mac_tc2(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.opart, nt, t0,
+                            pw.rt_desc, pw.row_m2, st);
+        if (rc == TRED_EUNSUPPORTED)
+          rc = tred_mac_tc_fused(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.opart, nt,
+                                 t0, pw.rt_desc, pw.row_m2, st);
         if (rc != TRED_OK) return rc;
         TRED_COUNT_LAUNCH(1);
       }

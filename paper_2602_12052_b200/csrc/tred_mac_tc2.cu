@@ -1,0 +1,421 @@
+// Spectrum product of Eq. (14) on CTA PAIRS: tcgen05.mma.cta_group::2,
+// M = 256 (two row tiles of 128 charge pixels, one per CTA), N = 2 kp, 3xTF32, with the sum
+// over the response offsets fused into the epilogue (same arithmetic and layouts as
+// k_mac_tc<true> in tred_mac_tc.cu; see there and tred_conv.cu for the row tiles).
+//
+// Why pairs: with one CTA per tile every MMA reads 4 KB of A and 8 KB of B from shared
+// memory in 128 cycles (96 B/clk of the SM's 128 B/clk) and every K chunk refills 40 KB
+// through TMA; ncu showed the tensor pipe 63 % active with the shared-memory pipe as the
+// co-bottleneck.  In a pair each CTA stages only half of B (its N/2 rows), so the operand
+// reads drop to 64 B/clk per SM, the TMA fill to 24 KB per chunk, and a stage to 32 KB
+// (5 stages instead of 3).
+//
+// Per CTA: warp 0 TMA producer (own A tile, own half of B_hi / B_lo), warp 1 MMA issuer
+// (leader CTA only), warps 2-5 converters (A -> A_hi in place, A_lo), warps 6-9 epilogue.
+// Barriers: full / empty / tfull are local to each CTA (empty and tfull arrive through
+// tcgen05.commit multicast); conv and tempty live in the leader and count one arrival per CTA.
+#include <cuda.h>
+#include "tred_common.cuh"
+
+namespace {
+
+constexpr int T2_M = 128;                 // rows per CTA
+constexpr int T2_KC = 16;                 // floats per K chunk = one 64-byte swizzle row
+constexpr int T2_STAGES = 5;
+constexpr int T2_NMAX = 256;
+constexpr int T2_A_BYTES = T2_M * T2_KC * 4;               // 8 KB
+constexpr int T2_BH_BYTES = (T2_NMAX / 2) * T2_KC * 4;     // 8 KB: half of B per CTA
+constexpr int T2_STAGE_BYTES = 2 * T2_A_BYTES + 2 * T2_BH_BYTES;   // A, A_lo, B_hi half, B_lo half
+constexpr int T2_THREADS = 320;
+constexpr int T2_PATCH_FLOAT2 = RT_PXMAX * RT_PYS;
+constexpr size_t T2_SMEM = (size_t)T2_STAGES * T2_STAGE_BYTES + 1024 + 256 + 4 * T2_PATCH_FLOAT2 * 8;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+// shared::cluster address of the same variable in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// Arrive on a barrier of any CTA of the cluster (address from mapa).  Default semantics
+// (release at CTA scope): the data the arrival orders -- this CTA's shared memory for its own
+// tensor core, this CTA's TMEM -- never leaves the SM; a cluster-scope release would cost a
+// MEMBAR.GPU per K chunk and the matching acquire an L1 invalidate per poll (seen in ncu).
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
+}
+// Waits for the phase of the given parity.  A wait longer than
+// ~2 s means a broken pipeline: trap instead of hanging the device.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  long long t0 = 0;
+  for (int it = 0;; ++it) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (ok) return;
+    if (it == 64) t0 = clock64();
+    if (it > 64 && (it & 1023) == 0 && clock64() - t0 > 4000000000ll) {
+      printf("tred_mac_tc2: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x,
+             threadIdx.x, bar, parity);
+      __trap();
+    }
+  }
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2,
+                                            uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// arrives (once the MMAs issued so far retire) on the barrier at this offset in BOTH CTAs
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
+  asm volatile(
+      "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+      ::"r"(bar), "h"((uint16_t)3)
+      : "memory");
+}
+__device__ __forceinline__ void tc_mma_tf32_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                                 uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// K-major operand tile of 64-byte swizzled rows (8 rows = one 512-byte swizzle atom)
+__device__ __forceinline__ uint64_t make_desc_sw64(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3ffff) >> 4);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(512 >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)4 << 61;
+  return d;
+}
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+
+struct T2Params {
+  int nf, ntile, npair;         // frequency slots, row tiles of the chunk, ceil(ntile / 2)
+  int N, K2, noff;
+  int K, H, npy, t0;
+  const int4* rt_desc;
+  const int32_t* row_m2;
+  float2* opart;                // [tile][f][8 + 2H][RT_PY]
+};
+
+template <int KC>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1)
+k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmBh,
+          const __grid_constant__ CUtensorMap tmBl, T2Params p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;                  // identical in both CTAs of the pair
+  uint8_t* base_ptr = smem_raw + (base - raw);
+  const uint32_t bars = base + T2_STAGES * T2_STAGE_BYTES;
+  auto full_bar = [&](int s) { return bars + 8u * s; };
+  auto conv_bar = [&](int s) { return bars + 8u * (T2_STAGES + s); };          // used in the leader
+  auto empty_bar = [&](int s) { return bars + 8u * (2 * T2_STAGES + s); };
+  auto tfull_bar = [&](int a) { return bars + 8u * (3 * T2_STAGES + a); };
+  auto tempty_bar = [&](int a) { return bars + 8u * (3 * T2_STAGES + 2 + a); }; // used in the leader
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(base_ptr + T2_STAGES * T2_STAGE_BYTES + 8 * (3 * T2_STAGES + 4));
+  auto sA = [&](int s) { return base + s * T2_STAGE_BYTES; };
+  auto sAlo = [&](int s) { return base + s * T2_STAGE_BYTES + T2_A_BYTES; };
+  auto sBh = [&](int s) { return base + s * T2_STAGE_BYTES + 2 * T2_A_BYTES; };
+  auto sBl = [&](int s) { return base + s * T2_STAGE_BYTES + 2 * T2_A_BYTES + T2_BH_BYTES; };
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int nkc = (p.K2 + T2_KC - 1) / T2_KC;
+  const int nitems = p.nf * p.npair;
+  const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < T2_STAGES; ++s) {
+      mbar_init(full_bar(s), 1);
+      mbar_init(conv_bar(s), 2);
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(tfull_bar(a), 1);
+      mbar_init(tempty_bar(a), 2);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
+                 "r"(512)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();                                             // both CTAs' barriers exist
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ------------------------------------------------------------ TMA producer (each CTA)
+    if (lane == 0) {
+      const int nh = p.N >> 1;
+      const uint32_t tx = (uint32_t)(T2_A_BYTES + 2 * nh * T2_KC * 4);
+      int stage = 0, phase = 0;
+      for (int item = cid; item < nitems; item += ncl) {
+        const int f = item / p.npair, pr = item - f * p.npair;
+        const int mt = min(2 * pr + (int)rank, p.ntile - 1);
+        for (int kc = 0; kc < nkc; ++kc) {
+          mbar_wait(empty_bar(stage), phase ^ 1);
+          mbar_expect_tx(full_bar(stage), tx);
+          tma_load_3d(sA(stage), &tmA, kc * T2_KC, mt * T2_M, f, full_bar(stage));
+          tma_load_3d(sBh(stage), &tmBh, kc * T2_KC, (int)rank * nh, f, full_bar(stage));
+          tma_load_3d(sBl(stage), &tmBl, kc * T2_KC, (int)rank * nh, f, full_bar(stage));
+          if (++stage == T2_STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------ MMA issuer (leader CTA)
+    if (lane == 0 && rank == 0) {
+      // instruction descriptor: D fp32, A/B tf32, both K-major, N, M = 256 over the pair
+      const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(p.N >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
+      int stage = 0, phase = 0, as = 0, aphase = 0;
+      for (int item = cid; item < nitems; item += ncl) {
+        mbar_wait(tempty_bar(as), aphase ^ 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + (uint32_t)(as * T2_NMAX);
+        for (int kc = 0; kc < nkc; ++kc) {
+          mbar_wait(conv_bar(stage), phase);                       // both CTAs: loaded and split
+          tc_fence_after();
+          const int nks = min(T2_KC, p.K2 - kc * T2_KC) >> 3;
+          const uint64_t da = make_desc_sw64(sA(stage)), dl = make_desc_sw64(sAlo(stage));
+          const uint64_t dbh = make_desc_sw64(sBh(stage)), dbl = make_desc_sw64(sBl(stage));
+          for (int ks = 0; ks < nks; ++ks) {
+            const uint64_t adv = (uint64_t)(ks * 2);
+            tc_mma_tf32_pair(d_tmem, da + adv, dbh + adv, idesc, (kc | ks) != 0);
+            tc_mma_tf32_pair(d_tmem, dl + adv, dbh + adv, idesc, 1);
+            tc_mma_tf32_pair(d_tmem, da + adv, dbl + adv, idesc, 1);
+          }
+          tc_commit_pair(empty_bar(stage));                        // frees the stage in both CTAs
+          if (++stage == T2_STAGES) { stage = 0; phase ^= 1; }
+        }
+        tc_commit_pair(tfull_bar(as));                             // accumulators complete in both CTAs
+        if (++as == 2) { as = 0; aphase ^= 1; }
+      }
+    }
+  } else if (warp < 6) {
+    // ------------------------------------------------------------ converters: A -> A_hi, A_lo
+    const int tc = threadIdx.x - 64;
+    int stage = 0, phase = 0;
+    for (int item = cid; item < nitems; item += ncl) {
+      for (int kc = 0; kc < nkc; ++kc) {
+        mbar_wait(full_bar(stage), phase);
+        float4* a = reinterpret_cast<float4*>(base_ptr + stage * T2_STAGE_BYTES);
+        float4* lo = reinterpret_cast<float4*>(base_ptr + stage * T2_STAGE_BYTES + T2_A_BYTES);
+#pragma unroll
+        for (int i = 0; i < T2_A_BYTES / 16 / 128; ++i) {
+          const float4 v = a[tc + 128 * i];
+          float4 h, l;
+          h.x = tf32_hi(v.x); h.y = tf32_hi(v.y); h.z = tf32_hi(v.z); h.w = tf32_hi(v.w);
+          l.x = tf32_hi(v.x - h.x); l.y = tf32_hi(v.y - h.y); l.z = tf32_hi(v.z - h.z); l.w = tf32_hi(v.w - h.w);
+          a[tc + 128 * i] = h;
+          lo[tc + 128 * i] = l;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor core reads
+        asm volatile("bar.sync 2, 128;" ::: "memory");
+        if (tc == 0) mbar_arrive_cluster(mapa(conv_bar(stage), 0));
+        if (++stage == T2_STAGES) { stage = 0; phase ^= 1; }
+      }
+    }
+  } else {
+    // ------------------------------------------------------------ epilogue: sum over offsets
+    const int q = warp & 3;
+    const int et = threadIdx.x - 192;
+    float2* patch = reinterpret_cast<float2*>(base_ptr + T2_STAGES * T2_STAGE_BYTES + 256);
+    float2* P = patch + q * T2_PATCH_FLOAT2;
+    for (int i = et; i < 4 * T2_PATCH_FLOAT2; i += 128) patch[i] = make_float2(0.0f, 0.0f);
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    const int PX = RT_SW + 2 * p.H;
+    int as = 0, aphase = 0;
+    for (int item = cid; item < nitems; item += ncl) {
+      const int f = item / p.npair, pr = item - f * p.npair;
+      const int mt = 2 * pr + (int)rank;
+      const bool has_tile = mt < p.ntile;
+      int4 d = make_int4(0, 0, 0, 0);
+      if (has_tile) d = p.rt_desc[p.t0 + mt];
+      const int r = q * 32 + lane;
+      const bool valid = r < d.y;
+      const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
+      int cell0 = 0;
+      if (valid) {
+        const int m2 = p.row_m2[d.x + r];
+        cell0 = (m2 & (RT_SW - 1)) * RT_PYS + ((m2 >> 3) % p.npy - d.z);
+      }
+      mbar_wait(tfull_bar(as), aphase);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (uint32_t)(as * T2_NMAX) + ((uint32_t)(q * 32) << 16);
+      const int KK = KC ? KC : p.K;
+      const int noff = KC ? KC * KC : p.noff;
+      if (vmask) {
+#pragma unroll
+        for (int c0 = 0; c0 < (KC ? (KC * KC + 15) / 16 : 8); ++c0) {
+          if (!KC && c0 * 16 >= noff) break;
+          uint32_t v[32];
+          asm volatile(
+              "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+              "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+              "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+              : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+              : "r"(taddr + (uint32_t)(c0 * 32))
+              : "memory");
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+          if (valid) {
+            float2* Pc = P + cell0;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+              const int off = c0 * 16 + j;
+              if (off < noff) {
+                const int kx = off / KK, ky = off - kx * KK;
+                float2* e = Pc + kx * RT_PYS + ky;
+                float2 a = *e;
+                a.x += __uint_as_float(v[2 * j]);
+                a.y += __uint_as_float(v[2 * j + 1]);
+                *e = a;
+              }
+              __syncwarp(vmask);     // another row's next offset may land on this cell
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      if (et == 0) mbar_arrive_cluster(mapa(tempty_bar(as), 0));   // this CTA's accumulator is free
+      if (++as == 2) { as = 0; aphase ^= 1; }
+      if (has_tile) {
+        const int nyp = d.w + 2 * p.H, ncell = PX * nyp;
+        float2* dst = p.opart + ((int64_t)mt * p.nf + f) * (PX * RT_PY);
+        for (int i = et; i < ncell; i += 128) {
+          const int X = i / nyp, Y = i - X * nyp;
+          const int c = X * RT_PYS + Y;
+          float2 a = patch[c];
+#pragma unroll
+          for (int w = 1; w < 4; ++w) {
+            const float2 b = patch[w * T2_PATCH_FLOAT2 + c];
+            a.x += b.x; a.y += b.y;
+          }
+#pragma unroll
+          for (int w = 0; w < 4; ++w) patch[w * T2_PATCH_FLOAT2 + c] = make_float2(0.0f, 0.0f);
+          dst[X * RT_PY + Y] = a;
+        }
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();                 // the peer's shared memory and barriers are no longer in use
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------- host side
+typedef CUresult (*PFN_encodeTiled2)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_encodeTiled2 get_encode_fn2() {
+  static PFN_encodeTiled2 fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (PFN_encodeTiled2)p;
+  }
+  return fn;
+}
+
+// [nslot][rows][k2] fp32, K contiguous; box = 16 floats x box_rows rows of one slot, 64-byte swizzle
+static bool make_map2(PFN_encodeTiled2 enc, CUtensorMap* tm, const float* base, int k2, int64_t rows, int nslot,
+                      int box_rows) {
+  const cuuint64_t dims[3] = {(cuuint64_t)k2, (cuuint64_t)rows, (cuuint64_t)nslot};
+  const cuuint64_t strides[2] = {(cuuint64_t)k2 * 4, (cuuint64_t)k2 * 4 * (cuuint64_t)rows};
+  const cuuint32_t box[3] = {(cuuint32_t)T2_KC, (cuuint32_t)box_rows, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+bool tred_mac_tc2_supported(const tred_ctx* ctx) {
+  const tred_dims& d = ctx->dims;
+  const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
+  return N <= T2_NMAX && (N % 32) == 0 && (K2 & 7) == 0 && (size_t)ctx->smem_optin >= T2_SMEM &&
+         ctx->cfg.resp_half <= RT_MAXH && ctx->num_sms >= 2 && get_encode_fn2() != nullptr;
+}
+
+// Same contract as tred_mac_tc_fused (tred_mac_tc.cu), on CTA pairs.
+int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
+                 int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st) {
+  const tred_dims& d = ctx->dims;
+  const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
+  if (ntile < 1 || !tred_mac_tc2_supported(ctx)) return TRED_EUNSUPPORTED;
+  if ((((uintptr_t)qhat) | ((uintptr_t)Bhi) | ((uintptr_t)Blo)) & 15) return TRED_EUNSUPPORTED;
+  PFN_encodeTiled2 enc = get_encode_fn2();
+  const int rp = ntile * T2_M;
+  CUtensorMap tmA, tmBh, tmBl;
+  if (!make_map2(enc, &tmA, qhat, K2, rp, d.n_freq, T2_M) || !make_map2(enc, &tmBh, Bhi, K2, N, d.n_freq, N / 2) ||
+      !make_map2(enc, &tmBl, Blo, K2, N, d.n_freq, N / 2))
+    return TRED_EUNSUPPORTED;
+  static bool attr_set = false;
+  if (!attr_set) {
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
+    attr_set = true;
+  }
+  T2Params p;
+  p.nf = d.n_freq; p.ntile = ntile; p.npair = (ntile + 1) / 2;
+  p.N = N; p.K2 = K2; p.noff = d.n_off;
+  p.K = 2 * ctx->cfg.resp_half + 1; p.H = ctx->cfg.resp_half; p.npy = ctx->cfg.npix_y; p.t0 = t0;
+  p.rt_desc = (const int4*)rt_desc; p.row_m2 = row_m2; p.opart = reinterpret_cast<float2*>(opart);
+  const int64_t items = (int64_t)p.nf * p.npair;
+  int64_t ncl = ctx->num_sms / 2;
+  if (ncl > items) ncl = items;
+  const int grid = (int)(2 * ncl);
+  if (p.K == 11)
+    k_mac_tc2<11><<<grid, T2_THREADS, T2_SMEM, st>>>(tmA, tmBh, tmBl, p);
+  else
+    k_mac_tc2<0><<<grid, T2_THREADS, T2_SMEM, st>>>(tmA, tmBh, tmBl, p);
+  TRED_LAUNCH_CHECK("k_mac_tc2");
+  return TRED_OK;
+}
