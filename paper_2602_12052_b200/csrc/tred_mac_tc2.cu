@@ -87,6 +87,12 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm,
       ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
       : "memory");
 }
+// asks L2 to fetch a box of the tensor (no shared-memory destination, no barrier)
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* tm, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+               ::"l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 // arrives (once the MMAs issued so far retire) on the barrier at this offset in BOTH CTAs
@@ -116,6 +122,19 @@ __device__ __forceinline__ uint64_t make_desc_sw64(uint32_t saddr) {
   return d;
 }
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+
+__device__ __forceinline__ void tmem_ld32(uint32_t (&v)[32], uint32_t taddr) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr)
+      : "memory");
+}
 
 struct T2Params {
   int nf, ntile, npair;         // frequency slots, row tiles of the chunk, ceil(ntile / 2)
@@ -185,6 +204,13 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       for (int item = cid; item < nitems; item += ncl) {
         const int f = item / p.npair, pr = item - f * p.npair;
         const int mt = min(2 * pr + (int)rank, p.ntile - 1);
+        // qhat streams from HBM once: have L2 fetch the next item's A tile now, so that the
+        // loads below (issued when a stage frees up) see an L2 hit instead of a DRAM round trip
+        if (item + ncl < nitems) {
+          const int fn = (item + ncl) / p.npair, prn = (item + ncl) - fn * p.npair;
+          const int mtn = min(2 * prn + (int)rank, p.ntile - 1);
+          for (int kc = 0; kc < nkc; ++kc) tma_prefetch_3d(&tmA, kc * T2_KC, mtn * T2_M, fn);
+        }
         for (int kc = 0; kc < nkc; ++kc) {
           mbar_wait(empty_bar(stage), phase ^ 1);
           mbar_expect_tx(full_bar(stage), tx);
@@ -258,59 +284,107 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     asm volatile("bar.sync 1, 128;" ::: "memory");
     const int PX = RT_SW + 2 * p.H;
     int as = 0, aphase = 0;
+    // Row tile descriptor and this thread's row record are fetched one / two items ahead
+    // (two dependent global loads otherwise sit on the epilogue's critical path).
+    auto item_tile = [&](int it) { return it < nitems ? 2 * (it % p.npair) + (int)rank : p.ntile; };
+    auto load_desc = [&](int it) {
+      const int t = item_tile(it);
+      return t < p.ntile ? p.rt_desc[p.t0 + t] : make_int4(0, 0, 0, 0);
+    };
+    const int r = q * 32 + lane;
+    int4 d_cur = load_desc(cid), d_nxt = load_desc(cid + ncl);
+    int m2_cur = r < d_cur.y ? p.row_m2[d_cur.x + r] : 0;
     for (int item = cid; item < nitems; item += ncl) {
       const int f = item / p.npair, pr = item - f * p.npair;
       const int mt = 2 * pr + (int)rank;
       const bool has_tile = mt < p.ntile;
-      int4 d = make_int4(0, 0, 0, 0);
-      if (has_tile) d = p.rt_desc[p.t0 + mt];
-      const int r = q * 32 + lane;
+      const int4 d = d_cur;
+      const int m2 = m2_cur;
+      // prefetch: record of the next item (its descriptor arrived an iteration ago), descriptor of the one after
+      const int m2_nxt = r < d_nxt.y ? p.row_m2[d_nxt.x + r] : 0;
+      const int4 d_nn = load_desc(item + 2 * ncl);
       const bool valid = r < d.y;
       const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
-      int cell0 = 0;
-      if (valid) {
-        const int m2 = p.row_m2[d.x + r];
-        cell0 = (m2 & (RT_SW - 1)) * RT_PYS + ((m2 >> 3) % p.npy - d.z);
-      }
+      const int yl = (m2 >> 3) % p.npy - d.z;
+      const int cell0 = valid ? (m2 & (RT_SW - 1)) * RT_PYS + yl : 0;
       mbar_wait(tfull_bar(as), aphase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + (uint32_t)(as * T2_NMAX) + ((uint32_t)(q * 32) << 16);
-      const int KK = KC ? KC : p.K;
-      const int noff = KC ? KC * KC : p.noff;
       if (vmask) {
+        if constexpr (KC == 11) {
+          // Offsets (kx, ky) and (kx + 8, ky) never meet in one cell (rows of a tile lie in an
+          // 8-pixel-wide strip), nor do (kx, ky) and (kx, ky + 5) when the rows of this warp span
+          // at most 5 lines: such offsets are added in one step (independent shared-memory
+          // read-modify-writes), the others one after the other.
+          const int ylo = __reduce_min_sync(vmask, valid ? yl : 0x7fffffff);
+          const int yhi = __reduce_max_sync(vmask, valid ? yl : -0x7fffffff);
+          const bool narrow = (yhi - ylo) <= 4;
+          float2* Pc = P + cell0;
+          auto rmw = [&](int kx, int ky, uint32_t re, uint32_t im) {
+            float2* e = Pc + kx * RT_PYS + ky;
+            float2 a = *e;
+            a.x += __uint_as_float(re);
+            a.y += __uint_as_float(im);
+            *e = a;
+          };
 #pragma unroll
-        for (int c0 = 0; c0 < (KC ? (KC * KC + 15) / 16 : 8); ++c0) {
-          if (!KC && c0 * 16 >= noff) break;
-          uint32_t v[32];
-          asm volatile(
-              "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-              "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-              "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-              : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-                "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-                "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-              : "r"(taddr + (uint32_t)(c0 * 32))
-              : "memory");
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          if (valid) {
-            float2* Pc = P + cell0;
+          for (int g = 0; g < 8; ++g) {
+            const bool paired = g < 3;
+            uint32_t va[32], vb[32];
+            tmem_ld32(va, taddr + (uint32_t)(22 * g));
+            if (paired) tmem_ld32(vb, taddr + (uint32_t)(22 * (g + 8)));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (valid) {
+              if (narrow) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-              const int off = c0 * 16 + j;
-              if (off < noff) {
-                const int kx = off / KK, ky = off - kx * KK;
-                float2* e = Pc + kx * RT_PYS + ky;
-                float2 a = *e;
-                a.x += __uint_as_float(v[2 * j]);
-                a.y += __uint_as_float(v[2 * j + 1]);
-                *e = a;
+                for (int ky = 0; ky < 5; ++ky) {
+                  rmw(g, ky, va[2 * ky], va[2 * ky + 1]);
+                  rmw(g, ky + 5, va[2 * ky + 10], va[2 * ky + 11]);
+                  if (paired) {
+                    rmw(g + 8, ky, vb[2 * ky], vb[2 * ky + 1]);
+                    rmw(g + 8, ky + 5, vb[2 * ky + 10], vb[2 * ky + 11]);
+                  }
+                  __syncwarp(vmask);
+                }
+                rmw(g, 10, va[20], va[21]);
+                if (paired) rmw(g + 8, 10, vb[20], vb[21]);
+                __syncwarp(vmask);
+              } else {
+#pragma unroll
+                for (int ky = 0; ky < 11; ++ky) {
+                  rmw(g, ky, va[2 * ky], va[2 * ky + 1]);
+                  if (paired) rmw(g + 8, ky, vb[2 * ky], vb[2 * ky + 1]);
+                  __syncwarp(vmask);
+                }
               }
-              __syncwarp(vmask);     // another row's next offset may land on this cell
+            }
+          }
+        } else {
+          const int KK = p.K, noff = p.noff;
+          for (int c0 = 0; c0 * 16 < noff; ++c0) {
+            uint32_t v[32];
+            tmem_ld32(v, taddr + (uint32_t)(c0 * 32));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (valid) {
+              float2* Pc = P + cell0;
+#pragma unroll
+              for (int j = 0; j < 16; ++j) {
+                const int off = c0 * 16 + j;
+                if (off < noff) {
+                  const int kx = off / KK, ky = off - kx * KK;
+                  float2* e = Pc + kx * RT_PYS + ky;
+                  float2 a = *e;
+                  a.x += __uint_as_float(v[2 * j]);
+                  a.y += __uint_as_float(v[2 * j + 1]);
+                  *e = a;
+                }
+                __syncwarp(vmask);   // another row's next offset may land on this cell
+              }
             }
           }
         }
       }
+      d_cur = d_nxt; d_nxt = d_nn; m2_cur = m2_nxt;
       tc_fence_before();
       asm volatile("bar.sync 1, 128;" ::: "memory");
       if (et == 0) mbar_arrive_cluster(mapa(tempty_bar(as), 0));   // this CTA's accumulator is free
