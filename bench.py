@@ -212,7 +212,7 @@ def run_cuda(args):
         out = None                          # a step's outputs are released before the next step
         out = simulate(seg_d)
     barrier()
-    info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles")}
+    info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles", "nrt")}
     # Gauss-Legendre node evaluations of one step = cuboids of every bounding box x n^3
     _, augi0, _ = sim.drift(seg_d)
     ext = (augi0[3:6] - augi0[0:3] + 1).to(torch.float64)
@@ -328,6 +328,12 @@ def run_cuda(args):
                              "frac": ach / peak, "ms_per_launch": stage_ms[k] / nl, "launches_per_step": nl,
                              "work_per_launch": w / nl, "peak_source": src,
                              "traffic": (tr / nl) if tr else None}
+        if "mac" in stage_roof and stage_roof["mac"]["bound"] == "tensor":
+            # what the tensor cores execute: 3 tf32 products per fp32 product, row tiles of 128
+            # rows (partly filled), 2 x 128 output columns for 2 x 121 offsets
+            ex = 3.0 * 2.0 * info["nrt"] * 128 * (2 * d.n_off_pad) * (2 * d.n_phase) * nf
+            stage_roof["mac"]["executed_tflops"] = ex / (stage_ms["mac"] * 1e-3) / 1e12
+            stage_roof["mac"]["executed_frac"] = stage_roof["mac"]["executed_tflops"] / tf32_peak
         dom = max(stage_roof, key=lambda k: stage_ms[k])
         roof = dict(stage_roof[dom])
         payload_gb = nb * d.block_floats * 4 / 1e9
@@ -349,7 +355,8 @@ def run_cuda(args):
                 "roofline": roof,
                 "stage_roofline": {k: {kk: (round(vv, 6) if isinstance(vv, float) else vv)
                                        for kk, vv in v.items() if kk in ("bound", "achieved", "peak", "unit", "frac",
-                                                                          "traffic")}
+                                                                          "traffic", "executed_tflops",
+                                                                          "executed_frac")}
                                    for k, v in stage_roof.items()},
                 "peak_mem_gb": peak_mem / 1e9,
                 "payload_gb": payload_gb,

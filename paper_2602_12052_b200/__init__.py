@@ -350,7 +350,7 @@ class Tred:
         sp_data = self.convolve(nblocks, keys, payload, rhat, plan, ncp, nsp, co, po, rt_off_host=ro)
         tile_data, dense = self.gather_waveforms(nsp, sp_data, plan, ntiles, pix_ids)
         tile_keys, sp_keys, sp_off = plan["tile_keys"], plan["sp_keys"], plan["sp_off"]
-        out = dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ncp=ncp, nsp=nsp, ntiles=ntiles,
+        out = dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ncp=ncp, nsp=nsp, ntiles=ntiles, nrt=int(ro[-1]),
                    tile_keys=tile_keys[:ntiles], tile_data=tile_data[:ntiles], dense=dense)
         if keep:
             out.update(augf=augf, augi=augi, keys=keys[:nblocks], blk_off=blk_off[:nblocks + 1],
@@ -414,7 +414,7 @@ class Tred:
             if t_hi > t_lo:
                 self.gather_waveforms(nsp, sp_data, plan, t_hi - t_lo, tile_plan=gplan, tile_data=tile_data,
                                       tile_begin=t_lo, accumulate=True)
-            chunks.append((b0, b1, nb, ncp, nsp))
+            chunks.append((b0, b1, nb, ncp, nsp, int(ro[-1])))
             del plan, sp_data
             b0 = b1
         dense = None
@@ -422,4 +422,4 @@ class Tred:
             _, dense = self.gather_waveforms(0, None, gplan, 0, pix_ids=pix_ids, tile_data=tile_data)
         return dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ntiles=ntiles, tile_keys=tile_keys[:ntiles],
                     tile_data=tile_data[:ntiles], dense=dense, chunks=chunks,
-                    ncp=sum(c[3] for c in chunks), nsp=sum(c[4] for c in chunks))
+                    ncp=sum(c[3] for c in chunks), nsp=sum(c[4] for c in chunks), nrt=sum(c[5] for c in chunks))

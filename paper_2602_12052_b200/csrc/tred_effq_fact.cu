@@ -89,8 +89,15 @@ __device__ __forceinline__ float axis_entry(int gi, int lo, int hi, float c, flo
   return v;
 }
 
+#ifndef TRED_EFFQ_MINB
+#define TRED_EFFQ_MINB 4            // resident CTAs per SM the register allocation aims at
+#endif
+#ifndef TRED_EFFQ_TILE_KB
+#define TRED_EFFQ_TILE_KB 64        // largest tile (floats x 4) a CTA stages
+#endif
+
 template <int N>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, TRED_EFFQ_MINB)
 k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict__ blk_off,
             const int32_t* __restrict__ pair_seg, const float* __restrict__ augf,
             const int32_t* __restrict__ augi, float* __restrict__ payload, TredGrid g, FactParams P) {
@@ -273,7 +280,7 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
   P.plane = g.Bx * g.By + 1;
   // largest TS (power of two, <= Bt) whose tile fits ~64 KB
   int TS = g.Bt;
-  while (TS > 4 && (size_t)TS * P.plane * sizeof(float) > 64 * 1024) TS /= 2;
+  while (TS > 4 && (size_t)TS * P.plane * sizeof(float) > TRED_EFFQ_TILE_KB * 1024) TS /= 2;
   P.TS = TS; P.nsub = g.Bt / TS;
   const size_t tile_floats = ((size_t)TS * P.plane + 3) & ~(size_t)3;
   const size_t smem = (tile_floats + 2 * (size_t)(g.Bx + g.By + TS) * MP) * sizeof(float);
