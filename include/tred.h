@@ -157,13 +157,18 @@ int tred_blockbin(tred_ctx* ctx, int64_t nseg, const int32_t* d_augi,
  *     the relative error is < 1.5e-7 (below fp32 rounding of the result).  Every term is
  *     separable in (x, y, t), so the sums over the n^3 nodes and the trilinear
  *     coefficients u of Eq. (9) factor into three 1-D tables per segment.
+ *     The tables of the segments a range of blocks refers to are built once, in d_work
+ *     (a segment meets several blocks), and copied by the tile CTAs.
  *   effq_mode 1: Eq. (10) in closed form (exp, erf) at every node.
  *   d_payload [nblocks][Bx][By][Bt] float32 out (fully overwritten).
+ *   d_work    workspace of tred_effq_work_bytes(nseg) bytes (less, or NULL, is allowed: the
+ *             tables are then rebuilt by every CTA -- same values, slower).
  */
+size_t tred_effq_work_bytes(const tred_ctx* ctx, int64_t nseg);
 int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
               const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
               const float* d_augf, const int32_t* d_augi,
-              float* d_payload, void* stream);
+              float* d_payload, void* d_work, size_t work_bytes, void* stream);
 
 /*
  * tred_prepare_response -- FFT(R^j) of Eq. (14), computed once.

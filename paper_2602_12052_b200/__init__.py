@@ -57,7 +57,8 @@ EXPORTS = {
     "tred_blockbin_work_bytes": (C.c_size_t, [_c_p, _c_i64, _c_i64]),
     "tred_blockbin": (C.c_int, [_c_p, _c_i64, _c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p,
                                 _c_p, C.c_size_t, _c_p]),
-    "tred_effq": (C.c_int, [_c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p]),
+    "tred_effq_work_bytes": (C.c_size_t, [_c_p, _c_i64]),
+    "tred_effq": (C.c_int, [_c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_prepare_response": (C.c_int, [_c_p, _c_p, _c_p, _c_p]),
     "tred_plan_work_bytes": (C.c_size_t, [_c_p]),
     "tred_convolve_plan": (C.c_int, [_c_p, _c_i64, _c_p,
@@ -247,8 +248,12 @@ class Tred:
         if payload is None:
             payload = self._empty((max(nblocks, 1), self.cfg.block[0], self.cfg.block[1], self.cfg.block[2]),
                                   t.float32)
+        work = None                                   # default: every CTA builds the tables of its segments
+        if os.environ.get("TRED_EFFQ_TABLES", "0") == "1":   # measured slower at config 3 (46.9 vs 39.6 ms)
+            work = self._workbuf("effq", self.L.tred_effq_work_bytes(self.h, nseg))
         _check(self.L.tred_effq(self.h, nseg, nblocks, _ptr(keys), _ptr(blk_off), _ptr(pair_seg),
-                                _ptr(augf), _ptr(augi), _ptr(payload), self._stream()), "tred_effq")
+                                _ptr(augf), _ptr(augi), _ptr(payload), _ptr(work),
+                                work.numel() if work is not None else 0, self._stream()), "tred_effq")
         return payload
 
     def convolve_plan(self, nblocks: int, keys, cap_cp: int | None = None, cap_sp: int | None = None,

@@ -89,6 +89,132 @@ __device__ __forceinline__ float axis_entry(int gi, int lo, int hi, float c, flo
   return v;
 }
 
+// ------------------------------------------------------------------ tables built once
+// A segment meets ~4 blocks x 2 tick sub-tiles, and every such CTA would rebuild the same
+// three per-axis tables (8 ex2 per entry for n = 4): ncu showed the tile kernel issue-bound
+// on exactly that.  So the tables of the segments a range of blocks refers to are built once
+// (k_effq_tables) into a slot of TAB_ROWS x TAB_M floats and the tile kernel copies the rows
+// it needs.  Segments that do not fit a slot (more than TAB_M quadrature points, several
+// pieces, a bounding box of more than TAB_ROWS grid rows in total, or no free slot) are
+// evaluated in the tile kernel as before.
+constexpr int TAB_M = 12;
+constexpr int TAB_ROWS = 96;
+constexpr int TAB_FLOATS = TAB_ROWS * TAB_M;
+constexpr int64_t EFFQ_MAX_SLOTS = 1 << 18;          // 262144 slots = 1.2 GB of tables at most
+constexpr int EFFQ_RANGE_BLOCKS = 8192;              // blocks per pass of (mark, tables, tiles)
+
+// Quadrature of a segment record: number of pieces and points per piece from its length
+// in sigmas (same arithmetic wherever it is needed).
+struct SegQuad { int npiece, m; };
+__device__ __forceinline__ SegQuad seg_quad(int flag, float dx, float dy, float dt, float sx, float sy, float st) {
+  SegQuad q;
+  q.npiece = 1; q.m = 4;
+  if (!flag) {
+    const float W = sqrtf((dx / sx) * (dx / sx) + (dy / sy) * (dy / sy) + (dt / st) * (dt / st));
+    q.npiece = (int)ceilf(W * (1.0f / 15.5f));
+    if (q.npiece < 1) q.npiece = 1;
+    const float Wp = W / (float)q.npiece;
+    q.m = Wp <= 1.0f ? 4 : Wp <= 3.9f ? 8 : Wp <= 6.9f ? 12 : Wp <= 9.9f ? 16 : Wp <= 12.8f ? 20 : 24;
+  }
+  return q;
+}
+
+// marks the segments the blocks [k0, k0 + nb) refer to (idempotent plain stores)
+__global__ void __launch_bounds__(256)
+k_effq_mark(int nb, int k0, const int32_t* __restrict__ blk_off, const int32_t* __restrict__ pair_seg,
+            int32_t* __restrict__ mark) {
+  const int warp = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+  if (warp >= nb) return;
+  const int p0 = blk_off[k0 + warp], p1 = blk_off[k0 + warp + 1];
+  for (int p = p0 + lane; p < p1; p += 32) mark[pair_seg[p]] = 1;
+}
+
+// slot[] = exclusive scan of the marks; lists the marked segments and resets tabslot
+__global__ void __launch_bounds__(256)
+k_effq_list(int64_t nseg, const int32_t* __restrict__ slot, int32_t* __restrict__ seglist, int cap,
+            int32_t* __restrict__ tabslot) {
+  const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= nseg) return;
+  const int sl = slot[s];
+  const bool marked = slot[s + 1] != sl;
+  if (marked && sl < cap) seglist[sl] = (int32_t)s;
+  tabslot[s] = -1;
+}
+
+// One warp per listed segment: the three tables of its bounding box (grid points
+// lo - E .. hi + E per axis), rows of TAB_M floats, X rows first (with K W_k folded in),
+// then Y, then T.
+template <int N>
+__global__ void __launch_bounds__(128)
+k_effq_tables(int64_t nseg, const int32_t* __restrict__ slot, const int32_t* __restrict__ seglist, int cap,
+              const float* __restrict__ augf, const int32_t* __restrict__ augi, float* __restrict__ tab,
+              int32_t* __restrict__ tabslot) {
+  const int sl = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  const int total = min(slot[nseg], cap);
+  if (sl >= total) return;
+  const int64_t s = seglist[sl];
+  constexpr int E = N > 1 ? 1 : 0;
+  constexpr float LOG2E_HALF = 0.72134752044448170f;
+  const int lox = augi[0 * nseg + s], loy = augi[1 * nseg + s], lot = augi[2 * nseg + s];
+  const int hix = augi[3 * nseg + s], hiy = augi[4 * nseg + s], hit = augi[5 * nseg + s];
+  const int flag = augi[6 * nseg + s];
+  const float p0x = augf[0 * nseg + s], p0y = augf[1 * nseg + s], p0t = augf[2 * nseg + s];
+  const float p1x = augf[3 * nseg + s], p1y = augf[4 * nseg + s], p1t = augf[5 * nseg + s];
+  const float sx = augf[6 * nseg + s], sy = augf[7 * nseg + s], st = augf[8 * nseg + s];
+  const float Qp = augf[9 * nseg + s];
+  const float dx = p1x - p0x, dy = p1y - p0y, dt = p1t - p0t;
+  const SegQuad q = seg_quad(flag, dx, dy, dt, sx, sy, st);
+  const int nxf = hix - lox + 1 + 2 * E, nyf = hiy - loy + 1 + 2 * E, ntf = hit - lot + 1 + 2 * E;
+  if (q.npiece != 1 || q.m > TAB_M || nxf + nyf + ntf > TAB_ROWS) return;      // tile kernel evaluates it
+  const float k2x = LOG2E_HALF / (sx * sx), k2y = LOG2E_HALF / (sy * sy), k2t = LOG2E_HALF / (st * st);
+  const float K = Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f;
+  const int m = q.m, goff = m * (m - 1) / 2;
+  float* T = tab + (int64_t)sl * TAB_FLOATS;
+  const int nent = (nxf + nyf + ntf) * TAB_M;
+  for (int e = lane; e < nent; e += 32) {
+    const int r = e / TAB_M, mi = e - r * TAB_M;
+    float v = 0.0f;
+    if (mi < m) {
+      float sk, wk;
+      if (flag) { sk = 0.5f; wk = mi == 0 ? 1.0f : 0.0f; }
+      else { sk = c_gl_s[goff + mi]; wk = c_gl_w[goff + mi]; }
+      if (r < nxf) v = axis_entry<N>(lox - E + r, lox, hix, fmaf(sk, dx, p0x), k2x) * (K * wk);
+      else if (r < nxf + nyf) v = axis_entry<N>(loy - E + (r - nxf), loy, hiy, fmaf(sk, dy, p0y), k2y);
+      else v = axis_entry<N>(lot - E + (r - nxf - nyf), lot, hit, fmaf(sk, dt, p0t), k2t);
+    }
+    T[e] = v;
+  }
+  if (lane == 0) tabslot[s] = sl;
+}
+
+// Phase B of one (segment, piece): tile[k][i][j] += sum_mi GX[i][mi] GY[j][mi] GT[k][mi] over
+// the clipped footprint.  A thread owns one column (and one tick chunk of it); the products
+// GX GY of its column stay in registers (MQ = m / 4 float4), every tile value is read and
+// written once per piece.
+template <int MQ>
+__device__ __forceinline__ void effq_phase_b(float* __restrict__ tp, int plane, const float* __restrict__ GXr,
+                                             const float* __restrict__ GYr, const float* __restrict__ GT,
+                                             int ka, int kb) {
+  float4 ab[MQ];
+#pragma unroll
+  for (int q = 0; q < MQ; ++q) {
+    const float4 a = *reinterpret_cast<const float4*>(GXr + 4 * q);
+    const float4 b = *reinterpret_cast<const float4*>(GYr + 4 * q);
+    ab[q] = make_float4(a.x * b.x, a.y * b.y, a.z * b.z, a.w * b.w);
+  }
+#pragma unroll 2
+  for (int k = ka; k < kb; ++k) {
+    float v = tp[k * plane];
+#pragma unroll
+    for (int q = 0; q < MQ; ++q) {
+      const float4 c = *reinterpret_cast<const float4*>(GT + k * MP + 4 * q);
+      v = fmaf(ab[q].x, c.x, v); v = fmaf(ab[q].y, c.y, v);
+      v = fmaf(ab[q].z, c.z, v); v = fmaf(ab[q].w, c.w, v);
+    }
+    tp[k * plane] = v;
+  }
+}
+
 #ifndef TRED_EFFQ_MINB
 #define TRED_EFFQ_MINB 4            // resident CTAs per SM the register allocation aims at
 #endif
@@ -100,7 +226,8 @@ template <int N>
 __global__ void __launch_bounds__(256, TRED_EFFQ_MINB)
 k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict__ blk_off,
             const int32_t* __restrict__ pair_seg, const float* __restrict__ augf,
-            const int32_t* __restrict__ augi, float* __restrict__ payload, TredGrid g, FactParams P) {
+            const int32_t* __restrict__ augi, const int32_t* __restrict__ tabslot,
+            const float* __restrict__ tab, float* __restrict__ payload, TredGrid g, FactParams P) {
   extern __shared__ float smf[];
   float* tile = smf;                                   // [TS][plane]
   const int tabn = (g.Bx + g.By + P.TS) * MP;          // floats of one table set
@@ -121,8 +248,11 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
 
   // Segment records of the block are staged in shared memory SB at a time (one pass of
   // coalesced loads instead of two dependent global loads per segment and thread).
-  constexpr int SB = 32, NF = 17;                      // 7 int fields (bbox, flag) + 10 floats
-  __shared__ int32_t s_rec[SB][NF + 1];
+  constexpr int SB = 32, NF = 18;                      // 7 int fields (bbox, flag), 10 floats, table slot
+  constexpr int NX = 6;                                // derived: k2x, k2y, k2t, K, npiece, m
+  __shared__ int32_t s_rec[SB][NF + NX + 1];
+  __shared__ int s_list[SB];
+  __shared__ int s_cnt;
   const int s_beg = blk_off[blk], s_end = blk_off[blk + 1];
   int it = 0;
   for (int b0 = s_beg; b0 < s_end; b0 += SB) {
@@ -131,36 +261,56 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
   for (int e = threadIdx.x; e < nbatch * NF; e += NT) {
     const int j = e / NF, f = e - j * NF;
     const int64_t s = pair_seg[b0 + j];
-    s_rec[j][f] = f < 7 ? augi[f * nseg + s] : __float_as_int(augf[(f - 7) * nseg + s]);
+    s_rec[j][f] = f < 7 ? augi[f * nseg + s]
+                : f < 17 ? __float_as_int(augf[(f - 7) * nseg + s]) : (tabslot ? tabslot[s] : -1);
   }
   __syncthreads();
-  for (int sj = 0; sj < nbatch; ++sj) {
-    const int32_t* rec = s_rec[sj];
+  // one lane per record: does the footprint meet this tile? per-segment constants once
+  if (threadIdx.x < 32) {
+    const int j = threadIdx.x;
+    bool hit_tile = false;
+    if (j < nbatch) {
+      int32_t* rec = s_rec[j];
+      hit_tile = max(rec[0] - E, I0) <= min(min(rec[3] + E, I0 + g.Bx - 1), g.NGx - 1) &&
+                 max(rec[1] - E, J0) <= min(min(rec[4] + E, J0 + g.By - 1), g.NGy - 1) &&
+                 max(rec[2] - E, K0) <= min(min(rec[5] + E, K0 + P.TS - 1), g.NGt - 1);
+      if (hit_tile) {
+        const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
+        const float dx = __int_as_float(rec[10]) - __int_as_float(rec[7]);
+        const float dy = __int_as_float(rec[11]) - __int_as_float(rec[8]);
+        const float dt = __int_as_float(rec[12]) - __int_as_float(rec[9]);
+        const SegQuad q = seg_quad(rec[6], dx, dy, dt, sx, sy, st);
+        rec[NF + 0] = __float_as_int(LOG2E_HALF / (sx * sx));
+        rec[NF + 1] = __float_as_int(LOG2E_HALF / (sy * sy));
+        rec[NF + 2] = __float_as_int(LOG2E_HALF / (st * st));
+        rec[NF + 3] = __float_as_int(__int_as_float(rec[16]) * 0.063493635934240969f / (sx * sy * st) * 0.125f);
+        rec[NF + 4] = q.npiece;
+        rec[NF + 5] = q.m;
+      }
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
+    if (hit_tile) s_list[__popc(bal & ((1u << j) - 1u))] = j;
+    if (j == 0) s_cnt = __popc(bal);
+  }
+  __syncthreads();
+  const int nlist = s_cnt;
+  for (int sl = 0; sl < nlist; ++sl) {
+    const int32_t* rec = s_rec[s_list[sl]];
     const int lox = rec[0], loy = rec[1], lot = rec[2];
     const int hix = rec[3], hiy = rec[4], hit = rec[5];
     // grid points of the segment's footprint inside this tile (and the grid)
     const int ix0 = max(lox - E, I0), ix1 = min(min(hix + E, I0 + g.Bx - 1), g.NGx - 1);
     const int iy0 = max(loy - E, J0), iy1 = min(min(hiy + E, J0 + g.By - 1), g.NGy - 1);
     const int kt0 = max(lot - E, K0), kt1 = min(min(hit + E, K0 + P.TS - 1), g.NGt - 1);
-    if (ix0 > ix1 || iy0 > iy1 || kt0 > kt1) continue;            // CTA-uniform
     const int nx = ix1 - ix0 + 1, ny = iy1 - iy0 + 1, nt = kt1 - kt0 + 1;
     const int flag = rec[6];
     const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
-    const float p1x = __int_as_float(rec[10]), p1y = __int_as_float(rec[11]), p1t = __int_as_float(rec[12]);
-    const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
-    const float Qp = __int_as_float(rec[16]);
-    const float dx = p1x - p0x, dy = p1y - p0y, dt = p1t - p0t;
-    const float k2x = LOG2E_HALF / (sx * sx), k2y = LOG2E_HALF / (sy * sy), k2t = LOG2E_HALF / (st * st);
-    const float K = Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f;   // (2 pi)^-3/2 / 8
-    // number of quadrature points from the segment length in sigmas, W = sqrt(a)
-    int npiece = 1, m = 4;
-    if (!flag) {
-      const float W = sqrtf((dx / sx) * (dx / sx) + (dy / sy) * (dy / sy) + (dt / st) * (dt / st));
-      npiece = (int)ceilf(W * (1.0f / 15.5f));
-      if (npiece < 1) npiece = 1;
-      const float Wp = W / (float)npiece;
-      m = Wp <= 1.0f ? 4 : Wp <= 3.9f ? 8 : Wp <= 6.9f ? 12 : Wp <= 9.9f ? 16 : Wp <= 12.8f ? 20 : 24;
-    }
+    const float dx = __int_as_float(rec[10]) - p0x, dy = __int_as_float(rec[11]) - p0y,
+                dt = __int_as_float(rec[12]) - p0t;
+    const float k2x = __int_as_float(rec[NF + 0]), k2y = __int_as_float(rec[NF + 1]),
+                k2t = __int_as_float(rec[NF + 2]), K = __int_as_float(rec[NF + 3]);
+    const int npiece = rec[NF + 4], m = rec[NF + 5];
+    const int slot = rec[17];
     const int goff = m * (m - 1) / 2;
     const float inv_np = 1.0f / (float)npiece;
     // phase-B work split: ncol columns x nsplit tick chunks
@@ -168,13 +318,30 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
     const int ncolp = (ncol + 31) & ~31;
     const int nsplit = ncolp < NT ? NT / ncolp : 1;
     const int chunk = (nt + nsplit - 1) / nsplit;
+    // item / ncolp and col / ny by multiplication: exact for item, col < 2048 and divisors <= 1024
+    const int inv_ncolp = (65536 + ncolp - 1) / ncolp, inv_ny = (65536 + ny - 1) / ny;
 
     for (int pc = 0; pc < npiece; ++pc, ++it) {
       float* GX = tabs + (it & 1) * tabn;             // [Bx][MP]
       float* GY = GX + g.Bx * MP;                     // [By][MP]
       float* GT = GY + g.By * MP;                     // [TS][MP]
-      // ---- phase A: tables
+      // ---- phase A: tables (copied from the segment's slot if it has one)
       const int nent = (nx + ny + nt) * m;
+      if (slot >= 0) {
+        const float* T = tab + (int64_t)slot * TAB_FLOATS;
+        const int nxf = hix - lox + 1 + 2 * E, nyf = hiy - loy + 1 + 2 * E;
+        const int rx = ix0 - (lox - E), ry = nxf + iy0 - (loy - E), rt = nxf + nyf + kt0 - (lot - E);
+        constexpr int Q = TAB_M / 4;                   // float4 per table row
+        for (int e = threadIdx.x; e < (nx + ny + nt) * Q; e += NT) {
+          const int r = e / Q, c4 = e - r * Q;
+          int src, dst;
+          if (r < nx) { src = rx + r; dst = r * MP; }
+          else if (r < nx + ny) { src = ry + (r - nx); dst = (g.Bx + (r - nx)) * MP; }
+          else { src = rt + (r - nx - ny); dst = (g.Bx + g.By + (r - nx - ny)) * MP; }
+          *reinterpret_cast<float4*>(GX + dst + 4 * c4) =
+              __ldg(reinterpret_cast<const float4*>(T + src * TAB_M) + c4);
+        }
+      } else
       for (int e = threadIdx.x; e < nent; e += NT) {
         const int r = e / m, mi = e - r * m;
         float sk, wk;
@@ -194,23 +361,20 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
       __syncthreads();
       // ---- phase B: tile[k][i][j] += sum_mi GX[i][mi] GY[j][mi] GT[k][mi]
       for (int item = threadIdx.x; item < ncolp * nsplit; item += NT) {
-        const int sp = item / ncolp, col = item - sp * ncolp;
+        const int sp = (item * inv_ncolp) >> 16, col = item - sp * ncolp;      // item / ncolp, exact here
         if (col >= ncol) continue;
-        const int cx = col / ny, cy = col - cx * ny;
+        const int cx = (col * inv_ny) >> 16, cy = col - cx * ny;               // col / ny
         const int ka = sp * chunk, kb = min(ka + chunk, nt);
         float* tp = tile + (size_t)(kt0 - K0) * P.plane + (ix0 - I0 + cx) * g.By + (iy0 - J0 + cy);
-        for (int mg = 0; mg < m; mg += 4) {
-          const float4 a = *reinterpret_cast<const float4*>(GX + cx * MP + mg);
-          const float4 b = *reinterpret_cast<const float4*>(GY + cy * MP + mg);
-          const float4 ab = make_float4(a.x * b.x, a.y * b.y, a.z * b.z, a.w * b.w);
-#pragma unroll 4
-          for (int k = ka; k < kb; ++k) {
-            const float4 c = *reinterpret_cast<const float4*>(GT + k * MP + mg);
-            float v = tp[k * P.plane];
-            v = fmaf(ab.x, c.x, v); v = fmaf(ab.y, c.y, v);
-            v = fmaf(ab.z, c.z, v); v = fmaf(ab.w, c.w, v);
-            tp[k * P.plane] = v;
-          }
+        const float* GXr = GX + cx * MP;
+        const float* GYr = GY + cy * MP;
+        switch (m >> 2) {
+          case 1: effq_phase_b<1>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
+          case 2: effq_phase_b<2>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
+          case 3: effq_phase_b<3>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
+          case 4: effq_phase_b<4>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
+          case 5: effq_phase_b<5>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
+          default: effq_phase_b<6>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
         }
       }
       // no barrier here: the next phase A writes the other table set, and its barrier
@@ -219,12 +383,22 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
   }
   }
   __syncthreads();
-  // tile -> payload[blk][i][j][k], k contiguous
+  // tile -> payload[blk][i][j][k], k contiguous: a thread writes 4 consecutive ticks
   float* out = payload + (int64_t)blk * g.Bx * g.By * g.Bt + sub * P.TS;
   const int nij = g.Bx * g.By;
-  for (int idx = threadIdx.x; idx < nij * P.TS; idx += NT) {
-    const int k = idx % P.TS, ij = idx / P.TS;
-    out[(int64_t)ij * g.Bt + k] = tile[k * P.plane + ij];
+  if ((P.TS & 3) == 0) {
+    const int q4 = P.TS >> 2;                           // float4 per column
+    for (int idx = threadIdx.x; idx < nij * q4; idx += NT) {
+      const int ij = idx / q4, k = (idx - ij * q4) << 2;
+      const float* t = tile + k * P.plane + ij;
+      *reinterpret_cast<float4*>(out + (int64_t)ij * g.Bt + k) =
+          make_float4(t[0], t[P.plane], t[2 * P.plane], t[3 * P.plane]);
+    }
+  } else {
+    for (int idx = threadIdx.x; idx < nij * P.TS; idx += NT) {
+      const int k = idx % P.TS, ij = idx / P.TS;
+      out[(int64_t)ij * g.Bt + k] = tile[k * P.plane + ij];
+    }
   }
 }
 
@@ -263,10 +437,40 @@ int tred_effq_init_tables(void) {
   return TRED_OK;
 }
 
+struct EffqWork { int32_t* slot; int32_t* tabslot; int32_t* seglist; void* scan; float* tab; int cap; size_t total; };
+
+static EffqWork carve_effq(void* base, int64_t nseg, size_t work_bytes) {
+  EffqWork w;
+  size_t o = 0; char* b = (char*)base;
+  auto take = [&](size_t bytes) { void* p = b ? b + o : nullptr; o += align_up(bytes, 256); return p; };
+  w.slot = (int32_t*)take((size_t)(nseg + 1) * 4);
+  w.tabslot = (int32_t*)take((size_t)(nseg > 0 ? nseg : 1) * 4);
+  w.scan = take(tred_scan_work_bytes(nseg + 1));
+  const size_t fixed = o;
+  int64_t cap = nseg < EFFQ_MAX_SLOTS ? nseg : EFFQ_MAX_SLOTS;
+  if (work_bytes) {                                  // what the given workspace holds
+    const size_t per = (size_t)TAB_FLOATS * 4 + 4;
+    cap = work_bytes > fixed + 4096 ? (int64_t)((work_bytes - fixed - 4096) / per) : 0;
+    if (cap > nseg) cap = nseg;
+    if (cap > EFFQ_MAX_SLOTS) cap = EFFQ_MAX_SLOTS;
+  }
+  if (cap < 0) cap = 0;
+  w.cap = (int)cap;
+  w.seglist = (int32_t*)take((size_t)(cap > 0 ? cap : 1) * 4);
+  w.tab = (float*)take((size_t)(cap > 0 ? cap : 1) * TAB_FLOATS * 4);
+  w.total = o;
+  return w;
+}
+
+extern "C" size_t tred_effq_work_bytes(const tred_ctx* ctx, int64_t nseg) {
+  if (!ctx || nseg < 0) return 0;
+  return carve_effq(nullptr, nseg, 0).total;
+}
+
 extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
                          const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
                          const float* d_augf, const int32_t* d_augi,
-                         float* d_payload, void* stream) {
+                         float* d_payload, void* d_work, size_t work_bytes, void* stream) {
   if (!ctx || nseg < 0 || nblocks < 0) return TRED_EINVAL;
   if (nblocks == 0) return TRED_OK;
   if (!d_keys || !d_blk_off || !d_pair_seg || !d_augf || !d_augi || !d_payload) return TRED_EINVAL;
@@ -287,25 +491,41 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
   if (smem > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
   int threads = g.Bx * g.By * 4;
   threads = threads < 64 ? 64 : threads > 256 ? 256 : threads;
-  const int64_t grid = nblocks * P.nsub;
-  if (grid >= (1ll << 31)) return TRED_EUNSUPPORTED;
-#define LAUNCH(NN)                                                                                 \
-  do {                                                                                             \
-    TRED_CUDA(cudaFuncSetAttribute(k_effq_fact<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
-                                   (int)smem));                                                    \
-    k_effq_fact<NN><<<(unsigned)grid, threads, smem, st>>>(nseg, d_keys, d_blk_off, d_pair_seg,    \
-                                                           d_augf, d_augi, d_payload, g, P);       \
-  } while (0)
+  if (nblocks * P.nsub >= (1ll << 31)) return TRED_EUNSUPPORTED;
+  EffqWork w = carve_effq(d_work, nseg, work_bytes);
+  const bool tables = d_work && w.total <= work_bytes && w.cap >= 1024;
   TredProfScope ps(ctx, ST_EFFQ, st);
-  TRED_COUNT_LAUNCH(1);
-  switch (g.gl_n) {
-    case 1: LAUNCH(1); break;
-    case 2: LAUNCH(2); break;
-    case 3: LAUNCH(3); break;
-    case 4: LAUNCH(4); break;
-    default: return TRED_EINVAL;
-  }
+  for (int64_t k0 = 0; k0 < nblocks; k0 += tables ? EFFQ_RANGE_BLOCKS : nblocks) {
+    const int nb = (int)(tables ? (nblocks - k0 < EFFQ_RANGE_BLOCKS ? nblocks - k0 : EFFQ_RANGE_BLOCKS) : nblocks);
+    if (tables) {
+      TRED_CUDA(cudaMemsetAsync(w.slot, 0, (size_t)(nseg + 1) * 4, st));
+      k_effq_mark<<<cdiv((int64_t)nb * 32, 256), 256, 0, st>>>(nb, (int)k0, d_blk_off, d_pair_seg, w.slot);
+      int rc = tred_exclusive_scan_i32(w.slot, w.slot, nseg + 1, nullptr, w.scan, st);
+      if (rc != TRED_OK) return rc;
+      k_effq_list<<<cdiv(nseg, 256), 256, 0, st>>>(nseg, w.slot, w.seglist, w.cap, w.tabslot);
+      TRED_COUNT_LAUNCH(4);
+    }
+#define LAUNCH(NN)                                                                                     \
+  do {                                                                                                 \
+    if (tables)                                                                                        \
+      k_effq_tables<NN><<<cdiv(w.cap, 4), 128, 0, st>>>(nseg, w.slot, w.seglist, w.cap, d_augf, d_augi, \
+                                                        w.tab, w.tabslot);                             \
+    TRED_CUDA(cudaFuncSetAttribute(k_effq_fact<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
+                                   (int)smem));                                                        \
+    k_effq_fact<NN><<<(unsigned)((int64_t)nb * P.nsub), threads, smem, st>>>(                          \
+        nseg, d_keys + k0, d_blk_off + k0, d_pair_seg, d_augf, d_augi, tables ? w.tabslot : nullptr,   \
+        w.tab, d_payload + k0 * g.Bx * g.By * g.Bt, g, P);                                             \
+  } while (0)
+    TRED_COUNT_LAUNCH(tables ? 2 : 1);
+    switch (g.gl_n) {
+      case 1: LAUNCH(1); break;
+      case 2: LAUNCH(2); break;
+      case 3: LAUNCH(3); break;
+      case 4: LAUNCH(4); break;
+      default: return TRED_EINVAL;
+    }
 #undef LAUNCH
+  }
   TRED_LAUNCH_CHECK("k_effq_fact");
   return TRED_OK;
 }
