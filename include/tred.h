@@ -73,6 +73,11 @@ typedef struct tred_config {
                                         CTA pairs (tcgen05 cta_group::2) if supported, else
                                         as 3, else as 2, else as 1,
                                     3 = as 0 on single CTAs,
+                                    4 = as 0 with the mirror symmetry of the response
+                                        (MPCP) spent on the product: sums and
+                                        differences of mirror phase pairs, two products of half
+                                        the size; falls back to 0 if the response prepared last
+                                        is not exactly mirror-symmetric,
                                     1 = fp32 FMA pipe, products written to memory,
                                     2 = tensor cores 3xTF32, products written to memory       */
 } tred_config;
@@ -177,7 +182,11 @@ int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
  *          sub-pixel phase (jx,jy) (readings G3, G12).
  *   d_rhat [rhat_floats] float32 out: the spectrum in the layouts the kernels read
  *          (fp32 [f][phase][offset] complex, and the real-ified matrices
- *          [f][2*offset+c][2*phase+c'] split into tf32 hi / lo parts for the tensor cores).
+ *          [f][2*offset+c][2*phase+c'] split into tf32 hi / lo parts for the tensor cores,
+ *          and the half-size matrices of a mirror-symmetric response).
+ *   Runs once per response and, unlike every other call, waits for the stream: the context
+ *   has to know whether the response has the mirror symmetry R_{-i}^{-j} = R_i^j
+ *   (exact equality is tested on the device).
  */
 int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* d_rhat, void* stream);
 

@@ -17,6 +17,7 @@ struct tred_ctx {
   tred_dims   dims;
   int         num_sms;
   int         smem_optin;     // max dynamic shared memory per block (bytes)
+  const void* sym_rhat;       // last d_rhat prepared from a mirror-symmetric response (or NULL)
   // stage profiling (tred_profile_begin / tred_profile_end)
   int         prof_on;
   int64_t     launches[ST_COUNT];
@@ -80,6 +81,22 @@ void tred_set_cuda_error(cudaError_t e, const char* where);
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ---- layout of the response-spectrum buffer d_rhat (tred_prepare_response) ---------------
+// [W: fp32 complex [f][phase][kp]] [B_hi][B_lo: [f][2 kp][2 nph] tf32 parts]
+// [Bs_hi][Bs_lo][Bd_hi][Bd_lo: [f][SYM_N][nph] mirror-symmetric halves, see tred_conv.cu] [flag]
+constexpr int SYM_N = 128;           // rows of the symmetric matrices: 2 x (noff + 1) / 2 padded
+struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, total; };
+static inline RhatLayout rhat_layout(const tred_dims& d) {
+  RhatLayout L;
+  const int64_t rb = (int64_t)d.n_freq * d.n_phase * d.n_off_pad;
+  const int64_t sb = (int64_t)d.n_freq * SYM_N * d.n_phase;
+  L.w = 0; L.bhi = 2 * rb; L.blo = 6 * rb;
+  L.bs_hi = 10 * rb; L.bs_lo = L.bs_hi + sb; L.bd_hi = L.bs_lo + sb; L.bd_lo = L.bd_hi + sb;
+  L.flag = L.bd_lo + sb;
+  L.total = L.flag + 8;
+  return L;
+}
 
 // ---- row tiles of the tensor-core convolution path (tred_conv.cu, tred_mac_tc.cu) ----
 constexpr int RT_SW = 8;         // strip width in pixels

@@ -83,6 +83,62 @@ k_resp_dft64(const float* __restrict__ resp, float2* __restrict__ W, float* __re
   }
 }
 
+// ------------------------------------------------------------------ mirror symmetry (MPCP)
+// PAPER.md:L199-221 (Mirror-Pair Complex Packing): a pixel response with the reflection
+// symmetry R_{-i}^{-j} = R_i^j lets the paper pack the mirror phases Q^j + i Q^{-j} into one
+// transform and halve the FFT count.  Here the time FFT is already real-to-half-complex, so
+// the same symmetry is spent on the spectrum product instead: with phase p' = nph-1-p the
+// mirror of p and offset o' = noff-1-o the mirror of o,
+//   T[o] + T[o'] = sum_{p < nph/2} (q[p] + q[p']) (W[p][o] + W[p'][o]),
+//   T[o] - T[o'] = sum_{p < nph/2} (q[p] - q[p']) (W[p][o] - W[p'][o]),
+// two products of half the inner length and half the offsets: half the tensor-core work.
+// k_resp_symcheck tests the response (exact equality); k_resp_sym builds the two matrices
+// Bs, Bd [f][SYM_N][nph] (real-ified like B, tf32 hi / lo parts).
+__global__ void __launch_bounds__(256)
+k_resp_symcheck(const float* __restrict__ resp, int nph, int noff, int Tr, int* __restrict__ flag) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n = (int64_t)(nph / 2) * noff * Tr;
+  if (i >= n) return;
+  const int tau = (int)(i % Tr);
+  const int64_t r = i / Tr;
+  const int off = (int)(r % noff), ph = (int)(r / noff);
+  const float a = resp[((int64_t)ph * noff + off) * Tr + tau];
+  const float b = resp[((int64_t)(nph - 1 - ph) * noff + (noff - 1 - off)) * Tr + tau];
+  if (a != b) atomicOr(flag, 1);
+}
+
+__global__ void __launch_bounds__(256)
+k_resp_sym(const float2* __restrict__ W, float* __restrict__ Bs_hi, float* __restrict__ Bs_lo,
+           float* __restrict__ Bd_hi, float* __restrict__ Bd_lo, int nf, int nph, int noff, int kp) {
+  const int nh = nph / 2, no = (noff + 1) / 2;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (int64_t)nf * no * nh) return;
+  const int p = (int)(i % nh);
+  const int o = (int)((i / nh) % no);
+  const int f = (int)(i / ((int64_t)nh * no));
+  const float2 w1 = W[((int64_t)f * nph + p) * kp + o], w2 = W[((int64_t)f * nph + (nph - 1 - p)) * kp + o];
+  const float2 ws = make_float2(w1.x + w2.x, w1.y + w2.y), wd = make_float2(w1.x - w2.x, w1.y - w2.y);
+  const int64_t plane = (int64_t)f * SYM_N * nph;
+  auto put = [&](float* hi, float* lo, int n, int kk, float v) {
+    const float h = tf32_trunc(v);
+    hi[plane + (int64_t)n * nph + kk] = h;
+    lo[plane + (int64_t)n * nph + kk] = tf32_trunc(v - h);
+  };
+  auto fill = [&](float* hi, float* lo, float2 w) {
+    if (f == 0) {                       // slot 0: DC in the real lane, Nyquist in the imaginary lane
+      put(hi, lo, 2 * o, 2 * p, w.x);
+      put(hi, lo, 2 * o + 1, 2 * p + 1, w.y);
+    } else {
+      put(hi, lo, 2 * o, 2 * p, w.x);
+      put(hi, lo, 2 * o + 1, 2 * p, w.y);
+      put(hi, lo, 2 * o, 2 * p + 1, -w.y);
+      put(hi, lo, 2 * o + 1, 2 * p + 1, w.x);
+    }
+  };
+  fill(Bs_hi, Bs_lo, ws);
+  fill(Bd_hi, Bd_lo, wd);
+}
+
 // ------------------------------------------------------------------ plan (O6)
 // flags over the map m = bt * npix + px * npy + py
 __global__ void __launch_bounds__(256)
@@ -361,7 +417,10 @@ k_fft_fwd_ct(const float* __restrict__ payload, const int32_t* __restrict__ bloc
 //   then the half-length real-FFT post-processing on pairs (k, M - k).
 // One shared-memory round trip between the steps and one before the post-processing,
 // instead of one per radix pass.  CG = 20 columns (S = 10, two phase rows) per CTA.
-template <int M, int B, int NZA>
+// SYM: the 20 columns of the CTA are the sums (first 10) and differences (last 10) of the
+// mirror phase pairs p = 10 grp + pl and nph-1-p (the FFT is linear, so they are formed
+// on the samples), written to qhat[f][row][s: 50 | d: 50] for the mirror-symmetric product.
+template <int M, int B, int NZA, bool SYM>
 __global__ void __launch_bounds__((20 * (M / B) + 31) / 32 * 32)
 k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
              RowSrc rs, int rp, float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g) {
@@ -372,17 +431,28 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   static_assert(NT % B == 0, "step 1 keeps one b per thread");
   extern __shared__ float2 buf[];           // step 1 -> 2: [col][ka][b (+1)]; then Z: [col][k (+1)]
   __shared__ long long colbase[CG];
+  __shared__ long long colbase2[SYM ? CG : 1];        // SYM: the mirror column
   const int row = blockIdx.x / NGRP, grp = blockIdx.x - row * NGRP;
   int px, py, bt;
   if (!row_pixel(rs, row, g, px, py, bt)) return;
-  if (threadIdx.x < CG) {
-    const int jx = grp * JG + threadIdx.x / S, jy = threadIdx.x % S;
+  auto column_base = [&](int jx, int jy) {
     const int i = px * S + jx, j = py * S + jy;
     const int bx = i / g.Bx, by = j / g.By;
     const int slot = blockmap[((int64_t)bt * g.NBx + bx) * g.NBy + by];
     long long base = -1;
     if (slot >= 0) base = (((long long)slot * g.Bx + (i - bx * g.Bx)) * g.By + (j - by * g.By)) * g.Bt;
-    colbase[threadIdx.x] = base;
+    return base;
+  };
+  if (threadIdx.x < CG) {
+    if (SYM) {
+      const int pl = threadIdx.x % S;                      // pair p = (jx = grp, jy = pl), mirror (S-1-grp, S-1-pl)
+      long long b1 = column_base(grp, pl), b2 = column_base(S - 1 - grp, S - 1 - pl);
+      if (b1 < 0 && b2 < 0) b2 = -2;                       // both empty: a zero column
+      colbase[threadIdx.x] = b1;
+      colbase2[threadIdx.x] = b2;
+    } else {
+      colbase[threadIdx.x] = column_base(grp * JG + threadIdx.x / S, threadIdx.x % S);
+    }
   }
   __syncthreads();
   const int hb = g.Bt >> 1;
@@ -401,11 +471,18 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
     for (int i = 0; i < NIT; ++i) {
       const int it = threadIdx.x + i * NT;
       const long long base = it < CG * B ? colbase[it / B] : -1;
+      const long long base2 = (SYM && it < CG * B) ? colbase2[it / B] : -1;
+      const float sgn = (SYM && it / B >= S) ? -1.0f : 1.0f;
 #pragma unroll
       for (int a = 0; a < NZA; ++a) {
         const int n = B * a + b;
         p[i][a] = (n < hb && base >= 0) ? __ldg(reinterpret_cast<const float2*>(payload + base + 2 * n))
                                         : make_float2(0.0f, 0.0f);
+        if (SYM && n < hb && base2 >= 0) {
+          const float2 x2 = __ldg(reinterpret_cast<const float2*>(payload + base2 + 2 * n));
+          p[i][a].x = fmaf(sgn, x2.x, p[i][a].x);
+          p[i][a].y = fmaf(sgn, x2.y, p[i][a].y);
+        }
       }
     }
 #pragma unroll
@@ -414,7 +491,7 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
       if (it >= CG * B) break;
       const int c = it / B;
       float2* dst = buf + (c * A) * BP + b;
-      if (colbase[c] < 0) {                                // column outside the occupied blocks
+      if (SYM ? (colbase[c] < 0 && colbase2[c] < 0) : (colbase[c] < 0)) {   // column outside the occupied blocks
 #pragma unroll
         for (int ka = 0; ka < A; ++ka) dst[ka * BP] = make_float2(0.0f, 0.0f);
         continue;
@@ -437,7 +514,7 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
     float2 y[B];
     const bool on = it < CG * A;
     const int c = it / A, ka = it - c * A;
-    const bool live = on && colbase[c] >= 0;
+    const bool live = on && (colbase[c] >= 0 || (SYM && colbase2[c] >= 0));
     if (live) {
       const float2* src = buf + it * BP;
 #pragma unroll
@@ -456,26 +533,28 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   }
   __syncthreads();
   // ---- real-FFT post-processing on pairs (k, M - k); slot 0 packs (DC, Nyquist)
-  float2* out = qhat + (int64_t)row * NPH + grp * CG;
+  // SYM: column c = (pl, sd) goes to float2 slot sd * 50 + 10 grp + pl of the row
+  float2* out = qhat + (int64_t)row * NPH + (SYM ? grp * S : grp * CG);
   const int64_t fstride = (int64_t)rp * NPH;
   constexpr int NPAIR = M / 2 + 1;
 #pragma unroll 4
   for (int it = threadIdx.x; it < NPAIR * CG; it += NT) {
     const int k = it / CG, c = it - k * CG;
+    const int cm = SYM ? (c < S ? c : c - S + NPH / 2) : c;
     const float2* Z = buf + c * ZP;
     if (k == 0) {
       const float2 z0 = Z[0];
-      out[c] = make_float2(z0.x + z0.y, z0.x - z0.y);
+      out[cm] = make_float2(z0.x + z0.y, z0.x - z0.y);
     } else if (2 * k == M) {
       const float2 z = Z[k];                                // X[M/2] = conj(Z[M/2])
-      out[k * fstride + c] = make_float2(z.x, -z.y);
+      out[k * fstride + cm] = make_float2(z.x, -z.y);
     } else {
       const float2 pz = Z[k], qz = Z[M - k];
       const float2 e = make_float2(0.5f * (pz.x + qz.x), 0.5f * (pz.y - qz.y));
       const float2 o = make_float2(0.5f * (pz.x - qz.x), 0.5f * (pz.y + qz.y));
       const float2 wo = cmulf(__ldg(gtw + k), o);
-      out[k * fstride + c] = make_float2(e.x + wo.y, e.y - wo.x);              // X[k]
-      out[(M - k) * fstride + c] = make_float2(e.x - wo.y, -e.y - wo.x);       // X[M-k]
+      out[k * fstride + cm] = make_float2(e.x + wo.y, e.y - wo.x);              // X[k]
+      out[(M - k) * fstride + cm] = make_float2(e.x - wo.y, -e.y - wo.x);       // X[M-k]
     }
   }
 }
@@ -851,7 +930,7 @@ static int launch_fft_fwd_ct(const tred_ctx* ctx, const TredGrid& g, const float
 
 #define TRED_FFT_2S_SHAPES(X) X(128, 32) X(144, 16) X(256, 32) X(288, 32) X(384, 32) X(512, 32)
 
-template <int MM, int BB, int NZA>
+template <int MM, int BB, int NZA, bool SYM>
 static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
                                const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
   constexpr int A = MM / BB;
@@ -861,13 +940,14 @@ static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const flo
   if (smem > (size_t)ctx->smem_optin) return 0;
   static bool set = false;
   if (!set) {
-    TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA, SYM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     set = true;
   }
-  k_fft_fwd_2s<MM, BB, NZA><<<(unsigned)(nr * 5), NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);
+  k_fft_fwd_2s<MM, BB, NZA, SYM><<<(unsigned)(nr * 5), NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);
   return 1;
 }
 
+template <bool SYM>
 static int launch_fft_fwd_2s(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
                              const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
   if (g.S != 10 || nr < 1) return 0;
@@ -876,14 +956,26 @@ static int launch_fft_fwd_2s(const tred_ctx* ctx, const TredGrid& g, const float
 #define X(MM, BB)                                                                                          \
   case MM: {                                                                                               \
     const int nza = (hb + BB - 1) / BB;                                                                    \
-    if (nza <= 1) return launch_fft_fwd_2s_t<MM, BB, 1>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
-    if (nza == 2) return launch_fft_fwd_2s_t<MM, BB, 2>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
-    if (nza <= 4) return launch_fft_fwd_2s_t<MM, BB, 4>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    if (nza <= 1) return launch_fft_fwd_2s_t<MM, BB, 1, SYM>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    if (nza == 2) return launch_fft_fwd_2s_t<MM, BB, 2, SYM>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    if (nza <= 4) return launch_fft_fwd_2s_t<MM, BB, 4, SYM>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
     return 0;                                                                                              \
   }
     TRED_FFT_2S_SHAPES(X)
 #undef X
     default: return 0;
+  }
+}
+
+// is there a two-step forward FFT instance for this shape?
+static bool fft_fwd_2s_available(const TredGrid& g) {
+  if (g.S != 10) return false;
+  const int M = g.L / 2, hb = g.Bt / 2;
+  switch (M) {
+#define X(MM, BB) case MM: return (hb + BB - 1) / BB <= 4;
+    TRED_FFT_2S_SHAPES(X)
+#undef X
+    default: return false;
   }
 }
 
@@ -998,8 +1090,14 @@ bool tred_mac_tc2_supported(const tred_ctx* ctx);
 int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
                  int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
 
+// mirror-symmetric response (tred_mac_tc2s.cu)
+bool tred_mac_tc2s_supported(const tred_ctx* ctx);
+int tred_mac_tc2s(tred_ctx* ctx, const float* qhat, const float* Bs_hi, const float* Bs_lo, const float* Bd_hi,
+                  const float* Bd_lo, float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2,
+                  cudaStream_t st);
+
 static bool use_tiled(const tred_ctx* ctx) {
-  return (ctx->cfg.mac_mode == 0 || ctx->cfg.mac_mode == 3) && tred_mac_tc_fused_supported(ctx);
+  return (ctx->cfg.mac_mode == 0 || ctx->cfg.mac_mode >= 3) && tred_mac_tc_fused_supported(ctx);
 }
 
 // Tensor-core path of tred_convolve: row tiles (tred_convolve_plan), forward FFT into
@@ -1036,7 +1134,12 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
     k_fill_twiddles<<<cdiv(g.L, 256), 256, 0, st>>>(w0.tw, g.L);
     TRED_COUNT_LAUNCH(3);
   }
-  const int64_t wfl = d.rhat_floats / 10 * 2, bfl = d.rhat_floats / 10 * 4;
+  const RhatLayout rl = rhat_layout(d);
+  const int64_t wfl = rl.bhi, bfl = rl.blo - rl.bhi;
+  // mirror-symmetric response: sums / differences of the mirror phase pairs, half-size product
+  // (mac_mode 4 only: measured slower than the general product at config 3)
+  const bool sym = ctx->cfg.mac_mode == 4 && ctx->sym_rhat == (const void*)d_rhat && g.nph == 100 &&
+                   tred_mac_tc2s_supported(ctx) && fft_fwd_2s_available(g);
   int b0 = 0;
   while (b0 < g.NBt) {
     if (h_rt_off[b0 + 1] == h_rt_off[b0]) { ++b0; continue; }
@@ -1062,7 +1165,9 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{nullptr, 0, pw.rt_desc, pw.row_m2, t0, rg.nstrip, 1};
-        int ct = launch_fft_fwd_2s(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
+        int ct = sym ? launch_fft_fwd_2s<true>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st)
+                     : launch_fft_fwd_2s<false>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
+        if (sym && ct == 0) return TRED_EUNSUPPORTED;
         if (ct == 0) ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
         if (ct < 0) return ct;
         if (ct == 0)
@@ -1073,7 +1178,11 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
       {
         TredProfScope ps(ctx, ST_MAC, st);
         int rc = TRED_EUNSUPPORTED;
-        if (ctx->cfg.mac_mode == 0 && tred_mac_tc2_supported(ctx))
+        if (sym) {
+          rc = tred_mac_tc2s(ctx, (const float*)w.qhat, d_rhat + rl.bs_hi, d_rhat + rl.bs_lo, d_rhat + rl.bd_hi,
+                             d_rhat + rl.bd_lo, (float*)w.opart, nt, t0, pw.rt_desc, pw.row_m2, st);
+          if (rc != TRED_OK) return rc;
+        } else if (ctx->cfg.mac_mode != 3 && tred_mac_tc2_supported(ctx))
           rc = tred_mac_tc2(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.opart, nt, t0,
                             pw.rt_desc, pw.row_m2, st);
         if (rc == TRED_EUNSUPPORTED)
@@ -1120,7 +1229,8 @@ extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* 
   const size_t smem = (size_t)(2 * g.L + g.Tr) * sizeof(double);
   if (smem > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
   TRED_CUDA(cudaFuncSetAttribute(k_resp_dft64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const int64_t wfl = ctx->dims.rhat_floats / 10 * 2, bfl = ctx->dims.rhat_floats / 10 * 4;
+  const RhatLayout rl = rhat_layout(ctx->dims);
+  const int64_t wfl = rl.bhi, bfl = rl.blo - rl.bhi;
   {
     TredProfScope ps(ctx, ST_RESP, st);
     TRED_CUDA(cudaMemsetAsync(d_rhat, 0, (size_t)ctx->dims.rhat_floats * 4, st));
@@ -1129,6 +1239,24 @@ extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* 
     TRED_COUNT_LAUNCH(1);
   }
   TRED_LAUNCH_CHECK("k_resp_dft64");
+  // mirror-symmetric responses get the half-size matrices as well.  This
+  // is the one call that waits for the device: it runs once per response, and the host has to
+  // know which path tred_convolve will take.
+  if (ctx->sym_rhat == d_rhat) ctx->sym_rhat = nullptr;
+  if ((g.nph & 1) == 0 && (g.noff & 1) == 1 && g.noff + 1 <= SYM_N) {
+    int* flag = reinterpret_cast<int*>(d_rhat + rl.flag);
+    const int64_t n = (int64_t)(g.nph / 2) * g.noff * g.Tr;
+    k_resp_symcheck<<<cdiv(n, 256), 256, 0, st>>>(d_resp, g.nph, g.noff, g.Tr, flag);
+    const int64_t ns = (int64_t)g.nf * ((g.noff + 1) / 2) * (g.nph / 2);
+    k_resp_sym<<<cdiv(ns, 256), 256, 0, st>>>((const float2*)d_rhat, d_rhat + rl.bs_hi, d_rhat + rl.bs_lo,
+                                             d_rhat + rl.bd_hi, d_rhat + rl.bd_lo, g.nf, g.nph, g.noff, g.kp);
+    TRED_COUNT_LAUNCH(2);
+    TRED_LAUNCH_CHECK("k_resp_sym");
+    int h_flag = 1;
+    TRED_CUDA(cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TRED_CUDA(cudaStreamSynchronize(st));
+    if (h_flag == 0) ctx->sym_rhat = d_rhat;
+  }
   return TRED_OK;
 }
 
@@ -1253,7 +1381,8 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
     TRED_COUNT_LAUNCH(3);
   }
   const float* Wf = d_rhat;
-  const int64_t wfl = d.rhat_floats / 10 * 2, bfl = d.rhat_floats / 10 * 4;
+  const RhatLayout rl = rhat_layout(d);
+  const int64_t wfl = rl.bhi, bfl = rl.blo - rl.bhi;
 
   // slab batches (ohat of all their slab pixels resident) x row chunks (qhat, T resident)
   int b0 = 0;
@@ -1284,7 +1413,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{d_cp_keys, r0, nullptr, nullptr, 0, 0, 0};
-        int ct = launch_fft_fwd_2s(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
+        int ct = launch_fft_fwd_2s<false>(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
         if (ct == 0) ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
         if (ct < 0) return ct;
         if (ct == 0)

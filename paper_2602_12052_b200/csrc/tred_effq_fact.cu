@@ -222,8 +222,12 @@ __device__ __forceinline__ void effq_phase_b(float* __restrict__ tp, int plane, 
 #define TRED_EFFQ_TILE_KB 64        // largest tile (floats x 4) a CTA stages
 #endif
 
+#ifndef TRED_EFFQ_THREADS
+#define TRED_EFFQ_THREADS 256       // largest CTA
+#endif
+
 template <int N>
-__global__ void __launch_bounds__(256, TRED_EFFQ_MINB)
+__global__ void __launch_bounds__(TRED_EFFQ_THREADS, TRED_EFFQ_MINB)
 k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict__ blk_off,
             const int32_t* __restrict__ pair_seg, const float* __restrict__ augf,
             const int32_t* __restrict__ augi, const int32_t* __restrict__ tabslot,
@@ -490,7 +494,7 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
   const size_t smem = (tile_floats + 2 * (size_t)(g.Bx + g.By + TS) * MP) * sizeof(float);
   if (smem > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
   int threads = g.Bx * g.By * 4;
-  threads = threads < 64 ? 64 : threads > 256 ? 256 : threads;
+  threads = threads < 64 ? 64 : threads > TRED_EFFQ_THREADS ? TRED_EFFQ_THREADS : threads;
   if (nblocks * P.nsub >= (1ll << 31)) return TRED_EUNSUPPORTED;
   EffqWork w = carve_effq(d_work, nseg, work_bytes);
   const bool tables = d_work && w.total <= work_bytes && w.cap >= 1024;

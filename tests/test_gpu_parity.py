@@ -280,7 +280,7 @@ def _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix, work_bytes=Non
     return dense.cpu().numpy()
 
 
-@pytest.mark.parametrize("mac_mode", [1, 0, 2, 3])
+@pytest.mark.parametrize("mac_mode", [1, 0, 2, 3, 4])
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
 def test_convolve_parity_from_oracle_charge(cfg_id, mac_mode):
     """S4+S5 alone: the GPU convolves the ORACLE's effective charge (cast to fp32).
