@@ -6,7 +6,7 @@ geometry, charges and a synthetic field response, and carries the plain-data
 configuration record.  See DESIGN.md "Input recipe".
 """
 from .workloads import (Config, make_config, make_segments, make_response,
-                        make_random_response, SEG_FIELDS)
+                        make_random_response, SEG_FIELDS, make_steps, STEP_FIELDS, STEP_PARAMS)
 
 __all__ = ["Config", "make_config", "make_segments", "make_response",
-           "make_random_response", "SEG_FIELDS"]
+           "make_random_response", "SEG_FIELDS", "make_steps", "STEP_FIELDS", "STEP_PARAMS"]

@@ -243,3 +243,37 @@ def make_random_response(cfg: Config, seed: int) -> np.ndarray:
     rng = np.random.default_rng(seed)
     K = 2 * H + 1
     return rng.standard_normal((S, S, K, K, Tr)).astype(np.float32)
+
+
+# ----------------------------------------------------------------------------
+# synthetic G4Steps (input of the step preprocessing): straight tracks cut
+# into steps of random length (exponential, mean 4 mm, up to 40 mm), energy loss per unit
+# length 2.1 MeV/cm x U(0.8, 3).  Geometry and energies only -- no arithmetic of the method.
+# ----------------------------------------------------------------------------
+STEP_FIELDS = ("x0", "y0", "z0", "x1", "y1", "z1", "dE", "t0")
+
+STEP_PARAMS = dict(max_len_mm=5.0, recomb_model=1, w_ion_ev=23.6, efield_kv_cm=0.5, density_g_cm3=1.39,
+                   birks_A=0.8, birks_k=0.0486, box_alpha=0.93, box_beta=0.212)
+
+
+def make_steps(seed: int, n_tracks: int = 20, box_mm=(563.2, 563.2, 500.0)):
+    rng = np.random.default_rng(seed)
+    box = np.asarray(box_mm, dtype=np.float64)
+    rows = []
+    for _ in range(n_tracks):
+        p = rng.uniform(0.0, 1.0, 3) * box
+        d = _isotropic(rng, 1)[0]
+        t0 = rng.uniform(0.0, 10.0)
+        total = float(np.exp(rng.uniform(np.log(50.0), np.log(1500.0))))
+        done = 0.0
+        while done < total:
+            ln = float(min(max(rng.exponential(4.0), 0.05), 40.0))
+            q = p + ln * d
+            if np.any(q < 0.0) or np.any(q > box):
+                break
+            dedx = 2.1 * rng.uniform(0.8, 3.0)                  # MeV/cm
+            rows.append((*p, *q, dedx * ln / 10.0, t0))
+            p = q
+            done += ln
+    a = np.asarray(rows, dtype=np.float32)
+    return {k: np.ascontiguousarray(a[:, i]) for i, k in enumerate(STEP_FIELDS)}

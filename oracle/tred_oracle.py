@@ -351,3 +351,57 @@ def simulate(cfg, segs, R, pix=None, keys_select=None, fft=False) -> dict:
     wave = (conv_fft if fft else conv_direct)(cfg, kk, payload, R, pix)
     return dict(aug=aug, keys=keys, payload_keys=kk, payload=payload, pix=np.asarray(pix),
                 wave=wave, tiles=out_tiles(cfg, keys))
+
+
+# ---------------------------------------------------------------------------
+# N2: G4Step preprocessing -- PAPER.md:L57 (splitting) and
+# PAPER.md:L41,L57 (electrons surviving recombination).  Readings G21, G22 of DESIGN.md:
+#   G21  a step longer than max_len is cut into n = ceil(len / max_len) pieces of EQUAL length
+#        (all <= max_len); every piece keeps dE/dx, its dE is dE * (1 / n); shorter steps are
+#        kept unchanged.
+#   G22  "parameterized models of recombination" without a formula: the caller
+#        picks Birks' law  R = A / (1 + k/(rho E) dE/dx)  or the modified box model
+#        R = ln(alpha + b dE/dx) / (b dE/dx), b = beta/(rho E), clipped to [0, 1];
+#        N_e = dE / W_ion * R.
+# Units: mm, MeV (dE), MeV/cm (dE/dx), kV/cm, g/cm^3, eV (W_ion).
+# ---------------------------------------------------------------------------
+STEP_FIELDS = ("x0", "y0", "z0", "x1", "y1", "z1", "dE", "t0")
+
+
+def recombination(par, dedx):
+    """Surviving fraction R for dE/dx in MeV/cm (float64 array)."""
+    dedx = np.asarray(dedx, dtype=np.float64)
+    rhoE = par["density_g_cm3"] * par["efield_kv_cm"]
+    if par["recomb_model"] == 0:                      # Birks
+        return par["birks_A"] / (1.0 + par["birks_k"] / rhoE * dedx)
+    x = par["box_beta"] / rhoE * dedx                 # modified box
+    with np.errstate(divide="ignore", invalid="ignore"):
+        r = np.log(par["box_alpha"] + x) / x
+    r = np.where(x > 0.0, r, 0.0)
+    return np.clip(r, 0.0, 1.0)
+
+
+def split_steps(par, steps) -> dict:
+    """G4Steps -> step-segments of at most max_len_mm with their ionisation electrons.
+    Returns the segment SoA of drift() (x0..z1, q, t0 as float32), `parent` (int32 step
+    index of every segment) and `count` (int32 pieces per step)."""
+    p0 = np.stack([steps[k].astype(np.float64) for k in ("x0", "y0", "z0")], 1)
+    p1 = np.stack([steps[k].astype(np.float64) for k in ("x1", "y1", "z1")], 1)
+    d = p1 - p0
+    length = np.sqrt((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2])
+    count = np.maximum(np.ceil(length / par["max_len_mm"]), 1.0).astype(np.int32)
+    dE = steps["dE"].astype(np.float64)
+    dedx = np.where(length > 0.0, dE / np.where(length > 0.0, length, 1.0) * 10.0, 0.0)   # MeV/cm
+    ne = dE * 1.0e6 / par["w_ion_ev"] * recombination(par, dedx)                        # electrons per step
+    parent = np.repeat(np.arange(len(count), dtype=np.int32), count)
+    first = np.cumsum(count) - count
+    k = (np.arange(len(parent)) - first[parent]).astype(np.float64)
+    n = count[parent].astype(np.float64)
+    fa, fb = k / n, (k + 1.0) / n
+    out = {}
+    for a, name in enumerate(("x", "y", "z")):
+        out[name + "0"] = (p0[parent, a] + d[parent, a] * fa).astype(np.float32)
+        out[name + "1"] = (p0[parent, a] + d[parent, a] * fb).astype(np.float32)
+    out["q"] = (ne[parent] / n).astype(np.float32)
+    out["t0"] = steps["t0"][parent].astype(np.float32)
+    return dict(segs=out, parent=parent, count=count)
