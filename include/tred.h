@@ -263,6 +263,34 @@ int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_sp_data,
                           void* stream);
 
 /*
+ * tred_steps -- G4Step preprocessing (steps longer than a threshold, 5 mm in the
+ * paper, are divided into step-segments that keep dE/dx; electrons that
+ * survive recombination).  DESIGN.md readings G21 (n = ceil(len / max_len) equal pieces) and
+ * G22 (the recombination law is the caller's choice; the paper gives none).  Needs no context.
+ *   d_step   [8][nstep] float32 SoA rows x0,y0,z0,x1,y1,z1 (mm), dE (MeV), t0 (us)
+ *   d_seg    [8][cap_seg] float32 out: the segment rows tred_drift reads (x0..z1, q electrons, t0),
+ *            row stride cap_seg
+ *   d_parent [cap_seg] int32 out: step every segment comes from
+ *   d_nseg   int64 out: number of segments (may exceed cap_seg: TRED_ECAP semantics, nothing
+ *            beyond the capacity is written)
+ *   d_work   at least tred_steps_work_bytes(nstep) bytes
+ * Piece counts come from fp64 round-to-nearest arithmetic in a fixed order (bit-exact).
+ */
+typedef struct tred_steps_config {
+  double  max_len_mm;            /* threshold, PAPER.md:L57 (5 mm)                           */
+  int32_t recomb_model;          /* 0 = Birks, 1 = modified box                              */
+  double  w_ion_ev;              /* energy per electron-ion pair (eV)                        */
+  double  efield_kv_cm, density_g_cm3;
+  double  birks_A, birks_k;      /* R = A / (1 + k/(rho E) dE/dx)                            */
+  double  box_alpha, box_beta;   /* R = ln(alpha + b dE/dx)/(b dE/dx), b = beta/(rho E)      */
+} tred_steps_config;
+
+size_t tred_steps_work_bytes(int64_t nstep);
+int tred_steps(const tred_steps_config* cfg, int64_t nstep, const float* d_step, int64_t cap_seg,
+               float* d_seg, int32_t* d_parent, int64_t* d_nseg, void* d_work, size_t work_bytes,
+               void* stream);
+
+/*
  * Stage profiling (the paper's "profiler-guided optimization", Fig. 10).
  * tred_profile_begin clears the counters; with record_events != 0 every stage of the
  * following calls is bracketed by CUDA events on the launching stream.

@@ -16,7 +16,7 @@ import os
 
 from . import build as _build
 
-__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS"]
+__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS", "split_steps", "TredStepsConfig"]
 
 _c_i64 = C.c_int64
 _c_p = C.c_void_p
@@ -43,6 +43,14 @@ class TredDims(C.Structure):
                 ("n_freq", C.c_int32), ("n_phase", C.c_int32), ("n_off", C.c_int32),
                 ("n_off_pad", C.c_int32), ("pix_per_block", C.c_int32),
                 ("rhat_floats", _c_i64), ("block_floats", _c_i64), ("conv_row_bytes", _c_i64)]
+
+
+class TredStepsConfig(C.Structure):
+    """Mirror of `tred_steps_config` (include/tred.h)."""
+    _fields_ = [("max_len_mm", C.c_double), ("recomb_model", C.c_int32), ("w_ion_ev", C.c_double),
+                ("efield_kv_cm", C.c_double), ("density_g_cm3", C.c_double),
+                ("birks_A", C.c_double), ("birks_k", C.c_double),
+                ("box_alpha", C.c_double), ("box_beta", C.c_double)]
 
 
 # name -> (restype, argtypes); every symbol include/tred.h declares
@@ -75,6 +83,9 @@ EXPORTS = {
                                 _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_i64, _c_i64, _c_p, _c_p, C.c_int,
                                         _c_i64, _c_p, _c_p, _c_p]),
+    "tred_steps_work_bytes": (C.c_size_t, [_c_i64]),
+    "tred_steps": (C.c_int, [C.POINTER(TredStepsConfig), _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
+                             C.c_size_t, _c_p]),
     "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
     "tred_profile_end": (C.c_int, [_c_p, C.c_int, _c_p, _c_p]),
     "tred_stage_count": (C.c_int, []),
@@ -143,6 +154,34 @@ def get_dims(cfg) -> TredDims:
 
 def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def split_steps(steps, params: dict, cap_seg: int | None = None):
+    """tred_steps: G4Steps [8][nstep] (float32 CUDA tensor: x0,y0,z0,x1,y1,z1,dE,t0) -> step-segments
+    [8][nseg] for Tred.drift / Tred.simulate, and the parent step of every segment.  Sizes the
+    output from the device-side count (one host read) unless cap_seg is given."""
+    import torch
+    if not steps.is_cuda:
+        raise TredError("tred_steps needs CUDA tensors: the TRED path has no CPU fallback")
+    assert steps.dtype == torch.float32 and steps.is_contiguous() and steps.shape[0] == 8
+    L = lib()
+    c = TredStepsConfig()
+    for k, _ in TredStepsConfig._fields_:
+        setattr(c, k, params[k])
+    nstep = steps.shape[1]
+    dev = steps.device
+    stream = C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+    work = torch.empty((max(L.tred_steps_work_bytes(nstep), 256),), dtype=torch.uint8, device=dev)
+    nseg = torch.zeros((1,), dtype=torch.int64, device=dev)
+    if cap_seg is None:                                 # counting pass: capacity 0
+        _check(L.tred_steps(C.byref(c), nstep, _ptr(steps), 0, None, None, _ptr(nseg), _ptr(work), work.numel(),
+                            stream), "tred_steps")
+        cap_seg = int(nseg.item())
+    seg = torch.empty((8, max(cap_seg, 1)), dtype=torch.float32, device=dev)
+    parent = torch.empty((max(cap_seg, 1),), dtype=torch.int32, device=dev)
+    _check(L.tred_steps(C.byref(c), nstep, _ptr(steps), cap_seg, _ptr(seg), _ptr(parent), _ptr(nseg), _ptr(work),
+                        work.numel(), stream), "tred_steps")
+    return seg[:, :cap_seg], parent[:cap_seg], nseg
 
 
 class Tred:

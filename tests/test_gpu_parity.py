@@ -429,3 +429,35 @@ def test_chunked_equals_single_pass(cfg_id):
     c = sim.simulate_chunked(seg, rhat, pix_ids=torch.from_numpy(pix.astype(np.int32)).cuda(),
                              payload_budget_bytes=max(a["nblocks"] // 5, 1) * blk)
     _wave_checks(c["dense"].cpu().numpy().astype(np.float64), ref)
+
+
+# ------------------------------------------------------------------ N2: G4Step preprocessing
+@pytest.mark.parametrize("model", [0, 1])
+def test_steps_parity(model):
+    """tred_steps vs the oracle: piece counts, parents and segment ends bit-exact (fp64
+    round-to-nearest index path), electrons within 1e-6 (log / division rounding)."""
+    torch = _torch()
+    from paper_2602_12052_b200 import split_steps
+    steps = gen.make_steps(21, n_tracks=30)
+    par = dict(gen.STEP_PARAMS, recomb_model=model)
+    ref = o.split_steps(par, steps)
+    st = torch.from_numpy(np.ascontiguousarray(np.stack([steps[k] for k in gen.STEP_FIELDS]))).cuda()
+    seg, parent, nseg = split_steps(st, par)
+    assert int(nseg.item()) == len(ref["parent"])
+    np.testing.assert_array_equal(parent.cpu().numpy(), ref["parent"])
+    got = seg.cpu().numpy()
+    for i, k in enumerate(gen.SEG_FIELDS):
+        if k == "q":
+            np.testing.assert_allclose(got[i], ref["segs"][k], rtol=1e-6)
+        else:
+            np.testing.assert_array_equal(got[i], ref["segs"][k], err_msg=k)
+    # capacity semantics: too small a buffer still reports the count and stays in bounds
+    seg2, parent2, nseg2 = split_steps(st, par, cap_seg=10)
+    assert int(nseg2.item()) == len(ref["parent"]) and seg2.shape[1] == 10
+    np.testing.assert_array_equal(seg2.cpu().numpy()[0], ref["segs"]["x0"][:10])
+    # and the segments feed the hot path
+    cfg = gen.make_config(2)
+    sim = _sim(cfg)
+    augf, augi, npairs = sim.drift(seg.contiguous())
+    aug = o.drift(cfg, {k: got[i] for i, k in enumerate(gen.SEG_FIELDS)})
+    np.testing.assert_array_equal(augi.cpu().numpy()[:6], np.concatenate([aug["lo"].T, aug["hi"].T]))
