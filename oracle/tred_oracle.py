@@ -405,3 +405,66 @@ def split_steps(par, steps) -> dict:
     out["q"] = (ne[parent] / n).astype(np.float32)
     out["t0"] = steps["t0"][parent].astype(np.float32)
     return dict(segs=out, parent=parent, count=count)
+
+
+# ---------------------------------------------------------------------------
+# N3: trigger-reset pixel readout -- PAPER.md:L185, L189 (Fig. 4), noise
+# terms PAPER.md:L262.  Reading G23 of DESIGN.md (the paper gives the scheme in words only):
+# per channel, tick by tick, in the kernel's precision (fp32 running sum, because the
+# crossing tick is an integer decided by a floating-point comparison):
+#   WAIT   q += I[t]; when q >= threshold + d_thr[h] the discriminator fires at tick tc = t;
+#   INTEG  q += I[t] for the next n_integ ticks; at ts = tc + n_integ the record
+#          (ts, q + d_adc[h]) is written (hits whose ts falls outside the window are lost);
+#   RESET  q = d_base[h]; the n_reset ticks after ts are dead (their charge is dropped);
+# d_thr, d_adc, d_base are the discriminator, preamplifier and baseline noise draws of hit h
+# (inputs; zeros if absent).  adc_lsb_e > 0 rounds the record to that many electrons.
+# ---------------------------------------------------------------------------
+def readout(par, wave, noise=None):
+    """wave [npix][nticks] float32 (electrons per tick) -> (nhit [npix] int32,
+    tick [npix][max_hits] int32 (-1 where unused), adc [npix][max_hits] float32)."""
+    wave = np.asarray(wave, dtype=np.float32)
+    npix, nticks = wave.shape
+    mh = int(par["max_hits"])
+    nhit = np.zeros(npix, np.int32)
+    tick = np.full((npix, mh), -1, np.int32)
+    adc = np.zeros((npix, mh), np.float32)
+    thr0 = np.float32(par["threshold_e"])
+    lsb = np.float32(par.get("adc_lsb_e", 0.0))
+    for p in range(npix):
+        q = np.float32(0.0)
+        h = 0
+        state, left = 0, 0                                # 0 WAIT, 1 INTEG, 2 DEAD
+        nz = (lambda k: np.float32(noise[p, h, k])) if noise is not None else (lambda k: np.float32(0.0))
+        thr = np.float32(thr0 + nz(0)) if h < mh else thr0
+        row = wave[p]
+        for t in range(nticks):
+            if h >= mh:
+                break
+            if state == 2:
+                left -= 1
+                if left == 0:
+                    state = 0
+                continue
+            q = np.float32(q + row[t])
+            fire = False
+            if state == 0:
+                if q >= thr:
+                    if par["n_integ"] == 0:
+                        fire = True
+                    else:
+                        state, left = 1, int(par["n_integ"])
+            else:
+                left -= 1
+                fire = left == 0
+            if fire:
+                v = np.float32(q + nz(1))
+                if lsb > 0:
+                    v = np.float32(np.floor(np.float32(v / lsb) + np.float32(0.5)) * lsb)
+                tick[p, h], adc[p, h] = t, v
+                q = nz(2)
+                h += 1
+                nhit[p] = h
+                if h < mh:
+                    thr = np.float32(thr0 + nz(0))
+                state, left = (2, int(par["n_reset"])) if par["n_reset"] > 0 else (0, 0)
+    return nhit, tick, adc
