@@ -291,6 +291,33 @@ int tred_steps(const tred_steps_config* cfg, int64_t nstep, const float* d_step,
                void* stream);
 
 /*
+ * tred_readout -- trigger-reset pixel readout (Fig. 4; noise terms
+ * PAPER.md:L262; reading G23).  Per channel, tick by tick: the charge on the
+ * preamplifier is the running fp32 sum of the current; when it reaches threshold_e (+ the
+ * discriminator noise draw of this hit) the channel integrates n_integ more ticks and records
+ * (tick of digitisation, charge + preamplifier noise draw); it is then reset to the baseline
+ * draw and dead for n_reset ticks.  A hit whose digitisation tick falls outside the window
+ * is lost; at most max_hits records per channel.
+ *   d_wave     [npix][nticks] float32 current in electrons per tick (rows of d_dense of
+ *              tred_gather_waveforms)
+ *   d_noise    [npix][max_hits][3] float32 draws (discriminator, preamplifier, baseline) in
+ *              electrons for every possible hit, or NULL for none: random numbers are inputs
+ *   d_nhit     [npix] int32 out; d_hit_tick [npix][max_hits] int32 out (-1 = unused);
+ *   d_hit_adc  [npix][max_hits] float32 out (rounded to adc_lsb_e electrons if > 0)
+ */
+typedef struct tred_readout_config {
+  double  threshold_e;           /* discriminator threshold, electrons                      */
+  int32_t n_integ;               /* fixed integration after the crossing, ticks             */
+  int32_t n_reset;               /* dead ticks after the digitisation                        */
+  int32_t max_hits;              /* capacity of the per-channel record list                 */
+  double  adc_lsb_e;             /* 0: keep the charge as it is; > 0: round to this step     */
+} tred_readout_config;
+
+int tred_readout(const tred_readout_config* cfg, int64_t npix, int32_t nticks, const float* d_wave,
+                 const float* d_noise, int32_t* d_nhit, int32_t* d_hit_tick, float* d_hit_adc,
+                 void* stream);
+
+/*
  * Stage profiling (the paper's "profiler-guided optimization", Fig. 10).
  * tred_profile_begin clears the counters; with record_events != 0 every stage of the
  * following calls is bracketed by CUDA events on the launching stream.

@@ -16,7 +16,7 @@ import os
 
 from . import build as _build
 
-__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS", "split_steps", "TredStepsConfig"]
+__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS", "split_steps", "TredStepsConfig", "readout", "TredReadoutConfig"]
 
 _c_i64 = C.c_int64
 _c_p = C.c_void_p
@@ -53,6 +53,12 @@ class TredStepsConfig(C.Structure):
                 ("box_alpha", C.c_double), ("box_beta", C.c_double)]
 
 
+class TredReadoutConfig(C.Structure):
+    """Mirror of `tred_readout_config` (include/tred.h)."""
+    _fields_ = [("threshold_e", C.c_double), ("n_integ", C.c_int32), ("n_reset", C.c_int32),
+                ("max_hits", C.c_int32), ("adc_lsb_e", C.c_double)]
+
+
 # name -> (restype, argtypes); every symbol include/tred.h declares
 EXPORTS = {
     "tred_get_dims": (C.c_int, [C.POINTER(TredConfig), C.POINTER(TredDims)]),
@@ -86,6 +92,7 @@ EXPORTS = {
     "tred_steps_work_bytes": (C.c_size_t, [_c_i64]),
     "tred_steps": (C.c_int, [C.POINTER(TredStepsConfig), _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
                              C.c_size_t, _c_p]),
+    "tred_readout": (C.c_int, [C.POINTER(TredReadoutConfig), _c_i64, C.c_int32, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p]),
     "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
     "tred_profile_end": (C.c_int, [_c_p, C.c_int, _c_p, _c_p]),
     "tred_stage_count": (C.c_int, []),
@@ -154,6 +161,29 @@ def get_dims(cfg) -> TredDims:
 
 def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def readout(wave, params: dict, noise=None):
+    """tred_readout: waveforms [npix][nticks] (float32 CUDA tensor) -> (nhit, hit_tick, hit_adc)."""
+    import torch
+    if not wave.is_cuda:
+        raise TredError("tred_readout needs CUDA tensors: the TRED path has no CPU fallback")
+    assert wave.dtype == torch.float32 and wave.is_contiguous() and wave.dim() == 2
+    c = TredReadoutConfig()
+    for k, _ in TredReadoutConfig._fields_:
+        setattr(c, k, params.get(k, 0))
+    npix, nticks = wave.shape
+    mh = int(c.max_hits)
+    dev = wave.device
+    if noise is not None:
+        assert noise.is_cuda and noise.dtype == torch.float32 and noise.is_contiguous()
+        assert tuple(noise.shape) == (npix, mh, 3)
+    nhit = torch.empty((max(npix, 1),), dtype=torch.int32, device=dev)
+    tick = torch.empty((max(npix, 1), max(mh, 1)), dtype=torch.int32, device=dev)
+    adc = torch.empty((max(npix, 1), max(mh, 1)), dtype=torch.float32, device=dev)
+    _check(lib().tred_readout(C.byref(c), npix, nticks, _ptr(wave), _ptr(noise), _ptr(nhit), _ptr(tick), _ptr(adc),
+                              C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)), "tred_readout")
+    return nhit[:npix], tick[:npix, :mh], adc[:npix, :mh]
 
 
 def split_steps(steps, params: dict, cap_seg: int | None = None):

@@ -461,3 +461,32 @@ def test_steps_parity(model):
     augf, augi, npairs = sim.drift(seg.contiguous())
     aug = o.drift(cfg, {k: got[i] for i, k in enumerate(gen.SEG_FIELDS)})
     np.testing.assert_array_equal(augi.cpu().numpy()[:6], np.concatenate([aug["lo"].T, aug["hi"].T]))
+
+
+# ------------------------------------------------------------------ N3: trigger-reset readout
+@pytest.mark.parametrize("with_noise", [False, True])
+def test_readout_parity(with_noise):
+    """tred_readout on the waveforms of the path (config 1) vs the oracle on the same fp32
+    waveforms: hit counts, digitisation ticks and ADC words bit-exact (same fp32 running sum)."""
+    torch = _torch()
+    from paper_2602_12052_b200 import readout
+    cfg, segs = _small(1)
+    R = gen.make_response(cfg, 2001)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    pix = torch.arange(0, cfg.npix_x * cfg.npix_y, 3, dtype=torch.int32).cuda()
+    wave = sim.simulate(_seg_tensor(segs), rhat, pix_ids=pix)["dense"]
+    par = dict(threshold_e=3000.0, n_integ=16, n_reset=8, max_hits=12, adc_lsb_e=250.0 if with_noise else 0.0)
+    noise = None
+    if with_noise:      # PAPER.md:L262: discriminator 650 e, preamplifier 500 e, baseline 900 e
+        rng = np.random.default_rng(99)
+        noise = (rng.standard_normal((pix.numel(), par["max_hits"], 3)) * [650.0, 500.0, 900.0]).astype(np.float32)
+    nh, tk, adc = readout(wave, par, None if noise is None else torch.from_numpy(noise).cuda())
+    rn, rt, ra = o.readout(par, wave.cpu().numpy(), noise)
+    assert rn.sum() > 20 and rn.max() >= 2                     # the track is seen, some pixels fire repeatedly
+    np.testing.assert_array_equal(nh.cpu().numpy(), rn)
+    np.testing.assert_array_equal(tk.cpu().numpy(), rt)
+    np.testing.assert_array_equal(adc.cpu().numpy(), ra)
+    # empty input and zero capacity
+    z = torch.zeros((5, 64), dtype=torch.float32).cuda()
+    assert int(readout(z, par)[0].sum()) == 0
