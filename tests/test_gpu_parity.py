@@ -490,3 +490,48 @@ def test_readout_parity(with_noise):
     # empty input and zero capacity
     z = torch.zeros((5, 64), dtype=torch.float32).cuda()
     assert int(readout(z, par)[0].sum()) == 0
+
+
+# ------------------------------------------------------------------ full size (config 3)
+def test_full_size_config3_sampled_pixels():
+    """BASELINE config 3 at full size, in the configuration bench.py times: all integer outputs
+    (block keys, output tile keys) bit-exact in full; waveforms and effective charge on sampled
+    pixels, which the oracle can compute one neighbourhood at a time (only the blocks within
+    the response's reach of a pixel contribute to it)."""
+    torch = _torch()
+    cfg, segs = gen.make_segments(3)
+    R = gen.make_response(cfg, 2003)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    tiles = o.out_tiles(cfg, keys)
+    g = o.grid_of(cfg)
+    npy, S, H = cfg.npix_y, cfg.sub, cfg.resp_half
+    rng = np.random.default_rng(33)
+    act = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
+    centres = rng.choice(act[(act // npy > 8) & (act // npy < cfg.npix_x - 8) &
+                             (act % npy > 8) & (act % npy < npy - 8)], 2, replace=False)
+    groups = [np.array([c, c + 1, c + npy], dtype=np.int64) for c in centres]
+    pix_all = np.concatenate(groups)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    out = sim.simulate(_seg_tensor(segs), rhat, torch.from_numpy(pix_all.astype(np.int32)).cuda(), keep=True)
+    assert out["nblocks"] == len(keys)
+    gk = out["keys"].cpu().numpy()
+    np.testing.assert_array_equal(gk, keys)
+    np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
+    dense = out["dense"].cpu().numpy().astype(np.float64)
+    bx, by, bt = o.key_to_bxyz(g, keys)
+    Bx, By = cfg.block[0], cfg.block[1]
+    for gi, grp in enumerate(groups):
+        px, py = grp // npy, grp % npy
+        # blocks whose pixel span reaches any pixel of the group through the (2H+1)^2 response
+        m = ((Bx * bx + Bx - 1) // S >= px.min() - H) & ((Bx * bx) // S <= px.max() + H) & \
+            ((By * by + By - 1) // S >= py.min() - H) & ((By * by) // S <= py.max() + H)
+        kk = keys[m]
+        sel = o.segments_touching(cfg, aug, kk)
+        payload = o.effq(cfg, aug, kk, sel)
+        ref = o.conv_fft(cfg, kk, payload, R, grp)
+        _wave_checks(dense[3 * gi: 3 * gi + 3], ref)
+        # effective charge of the same blocks
+        got_q = out["payload"][torch.from_numpy(np.flatnonzero(m)).cuda()].cpu().numpy().astype(np.float64)
+        assert np.abs(got_q - payload).max() <= TOL_QEFF * np.abs(payload).max()
