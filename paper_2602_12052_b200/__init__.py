@@ -432,6 +432,27 @@ class Tred:
                        sp_keys=sp_keys[:nsp], sp_data=sp_data[:nsp], sp_off=sp_off)
         return out
 
+    # -- truth attribution ---------------------------
+    def attribute(self, seg, rhat, group, pix_ids, ngroups: int | None = None):
+        """On-demand waveform attribution "by re-convolving selected contributions"
+        (PAPER.md:L356): the path is linear in the segment charges, so the waveform a group of
+        segments (a track, a particle, a vertex) leaves on the requested pixels is the path run
+        on that group alone.  `group` [nseg] int tensor (group id of every segment, < 0: none).
+        Returns dense [ngroups][npix][nticks]; summed over the groups it equals the waveform
+        of all grouped segments up to fp32 rounding."""
+        t = self.torch
+        assert group.shape[0] == seg.shape[1]
+        if ngroups is None:
+            ngroups = int(group.max().item()) + 1 if group.numel() else 0
+        out = t.zeros((max(ngroups, 1), pix_ids.numel(), self.cfg.nticks), dtype=t.float32, device=self.device)
+        for gid in range(ngroups):
+            idx = t.nonzero(group == gid).flatten()
+            if idx.numel() == 0:
+                continue
+            sub = seg.index_select(1, idx).contiguous()          # selecting rows: marshalling, no arithmetic
+            out[gid] = self.simulate(sub, rhat, pix_ids=pix_ids)["dense"]
+        return out[:ngroups]
+
     # -- whole path in bounded-memory chunks of occupied blocks (BASELINE config 4) --------
     def simulate_chunked(self, seg, rhat, pix_ids=None, payload_budget_bytes: int = 8 << 30):
         """Same result as `simulate`, bit for bit, with the block payload, the convolution

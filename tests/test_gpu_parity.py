@@ -535,3 +535,33 @@ def test_full_size_config3_sampled_pixels():
         # effective charge of the same blocks
         got_q = out["payload"][torch.from_numpy(np.flatnonzero(m)).cuda()].cpu().numpy().astype(np.float64)
         assert np.abs(got_q - payload).max() <= TOL_QEFF * np.abs(payload).max()
+
+
+# ------------------------------------------------------------------ N4: truth attribution
+def test_attribution_by_reconvolution():
+    """waveform-level truth attribution re-convolves selected contributions.
+    Per-group waveforms match the oracle run on that group alone, and add up to the whole."""
+    torch = _torch()
+    cfg, segs = _small(2)
+    n = len(segs["q"])
+    R = gen.make_response(cfg, 2002)
+    group = (np.arange(n) * 3 // n).astype(np.int64)           # three "tracks": consecutive thirds
+    group[::17] = -1                                            # some segments without a label
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    seg = _seg_tensor(segs)
+    aug = o.drift(cfg, segs)
+    tiles = o.out_tiles(cfg, o.blocks(cfg, aug))
+    act = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
+    pix = act[:: max(1, len(act) // 10)][:10]
+    pix_d = torch.from_numpy(pix.astype(np.int32)).cuda()
+    per = sim.attribute(seg, rhat, torch.from_numpy(group).cuda(), pix_d).cpu().numpy().astype(np.float64)
+    assert per.shape == (3, len(pix), cfg.nticks)
+    for gid in range(3):
+        sub = {k: v[group == gid] for k, v in segs.items()}
+        ref = o.simulate(cfg, sub, R, pix=pix, fft=True)["wave"]
+        scale = max(np.abs(ref).max(), 1e-30)
+        assert np.abs(per[gid] - ref).max() <= TOL_WAVE * scale
+    labelled = {k: v[group >= 0] for k, v in segs.items()}
+    whole = sim.simulate(_seg_tensor(labelled), rhat, pix_ids=pix_d)["dense"].cpu().numpy().astype(np.float64)
+    assert np.abs(per.sum(0) - whole).max() <= 5e-6 * np.abs(whole).max()
