@@ -430,9 +430,9 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   constexpr int LOGB = tred_log2(B);
   static_assert(NT % B == 0, "step 1 keeps one b per thread");
   extern __shared__ float2 buf[];           // step 1 -> 2: [col][ka][b (+1)]; then Z: [col][k (+1)]
-  __shared__ long long colbase[CG];
-  __shared__ long long colbase2[SYM ? CG : 1];        // SYM: the mirror column
-  const int row = blockIdx.x / NGRP, grp = blockIdx.x - row * NGRP;
+  __shared__ long long colbase_all[NGRP * CG];
+  __shared__ long long colbase2_all[SYM ? NGRP * CG : 1];   // SYM: the mirror column
+  const int row = blockIdx.x;                               // one CTA per row, its 5 column groups in turn
   int px, py, bt;
   if (!row_pixel(rs, row, g, px, py, bt)) return;
   auto column_base = [&](int jx, int jy) {
@@ -443,19 +443,23 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
     if (slot >= 0) base = (((long long)slot * g.Bx + (i - bx * g.Bx)) * g.By + (j - by * g.By)) * g.Bt;
     return base;
   };
-  if (threadIdx.x < CG) {
+  for (int t = threadIdx.x; t < NGRP * CG; t += NT) {
+    const int gq = t / CG, cq = t - gq * CG;
     if (SYM) {
-      const int pl = threadIdx.x % S;                      // pair p = (jx = grp, jy = pl), mirror (S-1-grp, S-1-pl)
-      long long b1 = column_base(grp, pl), b2 = column_base(S - 1 - grp, S - 1 - pl);
-      if (b1 < 0 && b2 < 0) b2 = -2;                       // both empty: a zero column
-      colbase[threadIdx.x] = b1;
-      colbase2[threadIdx.x] = b2;
+      const int pl = cq % S;                               // pair p = (jx = gq, jy = pl), mirror (S-1-gq, S-1-pl)
+      colbase_all[t] = column_base(gq, pl);
+      colbase2_all[t] = column_base(S - 1 - gq, S - 1 - pl);
     } else {
-      colbase[threadIdx.x] = column_base(grp * JG + threadIdx.x / S, threadIdx.x % S);
+      colbase_all[t] = column_base(gq * JG + cq / S, cq % S);
     }
   }
   __syncthreads();
   const int hb = g.Bt >> 1;
+  const int64_t fstride = (int64_t)rp * NPH;
+#pragma unroll 1
+  for (int grp = 0; grp < NGRP; ++grp) {
+  const long long* colbase = colbase_all + grp * CG;
+  const long long* colbase2 = SYM ? colbase2_all + grp * CG : colbase2_all;
   // ---- step 1 (NT is a multiple of B: a thread keeps the same b for all its columns; all
   // global loads are issued before the arithmetic)
   {
@@ -532,30 +536,38 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
     }
   }
   __syncthreads();
-  // ---- real-FFT post-processing on pairs (k, M - k); slot 0 packs (DC, Nyquist)
-  // SYM: column c = (pl, sd) goes to float2 slot sd * 50 + 10 grp + pl of the row
-  float2* out = qhat + (int64_t)row * NPH + (SYM ? grp * S : grp * CG);
-  const int64_t fstride = (int64_t)rp * NPH;
-  constexpr int NPAIR = M / 2 + 1;
-#pragma unroll 4
-  for (int it = threadIdx.x; it < NPAIR * CG; it += NT) {
-    const int k = it / CG, c = it - k * CG;
+  // ---- real-FFT post-processing on pairs (k, M - k); slot 0 packs (DC, Nyquist).
+  // Thread (kr, c): column c, pairs k = 1 + kr, 1 + kr + KR, ...; the two output pointers
+  // advance by a constant, no index arithmetic in the loop.
+  {
+    constexpr int KR = NT / CG;                                    // pair rows per sweep
+    const int c = threadIdx.x % CG, kr = threadIdx.x / CG;
     const int cm = SYM ? (c < S ? c : c - S + NPH / 2) : c;
+    float2* out = qhat + (int64_t)row * NPH + (SYM ? grp * S : grp * CG) + cm;
     const float2* Z = buf + c * ZP;
-    if (k == 0) {
-      const float2 z0 = Z[0];
-      out[cm] = make_float2(z0.x + z0.y, z0.x - z0.y);
-    } else if (2 * k == M) {
-      const float2 z = Z[k];                                // X[M/2] = conj(Z[M/2])
-      out[k * fstride + cm] = make_float2(z.x, -z.y);
-    } else {
-      const float2 pz = Z[k], qz = Z[M - k];
-      const float2 e = make_float2(0.5f * (pz.x + qz.x), 0.5f * (pz.y - qz.y));
-      const float2 o = make_float2(0.5f * (pz.x - qz.x), 0.5f * (pz.y + qz.y));
-      const float2 wo = cmulf(__ldg(gtw + k), o);
-      out[k * fstride + cm] = make_float2(e.x + wo.y, e.y - wo.x);              // X[k]
-      out[(M - k) * fstride + cm] = make_float2(e.x - wo.y, -e.y - wo.x);       // X[M-k]
+    if (kr < KR) {
+      if (kr == 0) {
+        const float2 z0 = Z[0];
+        out[0] = make_float2(z0.x + z0.y, z0.x - z0.y);
+      } else if (kr == 1) {
+        const float2 z = Z[M / 2];                                  // X[M/2] = conj(Z[M/2])
+        out[(M / 2) * fstride] = make_float2(z.x, -z.y);
+      }
+      float2* o1 = out + (int64_t)(1 + kr) * fstride;
+      float2* o2 = out + (int64_t)(M - 1 - kr) * fstride;
+      const int64_t step = (int64_t)KR * fstride;
+#pragma unroll 4
+      for (int k = 1 + kr; k < M / 2; k += KR, o1 += step, o2 -= step) {
+        const float2 pz = Z[k], qz = Z[M - k];
+        const float2 e = make_float2(0.5f * (pz.x + qz.x), 0.5f * (pz.y - qz.y));
+        const float2 o = make_float2(0.5f * (pz.x - qz.x), 0.5f * (pz.y + qz.y));
+        const float2 wo = cmulf(__ldg(gtw + k), o);
+        *o1 = make_float2(e.x + wo.y, e.y - wo.x);                 // X[k]
+        *o2 = make_float2(e.x - wo.y, -e.y - wo.x);                // X[M-k]
+      }
     }
+  }
+  __syncthreads();                                                 // buf is rewritten by the next group
   }
 }
 
@@ -943,7 +955,7 @@ static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const flo
     TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA, SYM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     set = true;
   }
-  k_fft_fwd_2s<MM, BB, NZA, SYM><<<(unsigned)(nr * 5), NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);
+  k_fft_fwd_2s<MM, BB, NZA, SYM><<<(unsigned)nr, NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);
   return 1;
 }
 
