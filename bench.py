@@ -198,7 +198,7 @@ def run_cuda(args):
 
     # config 4: device-memory-bounded chunks of occupied blocks (peak <= 40 GB)
     if args.config == 4:
-        sim.conv_work_bytes = (args.work_gb or 8) << 30
+        sim.conv_work_bytes = (args.work_gb or 5) << 30
 
         def simulate(s):
             return sim.simulate_chunked(s, rhat, payload_budget_bytes=args.budget_gb << 30)
@@ -494,7 +494,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--ref-segments", type=int, default=0, help="oracle sample size (0 = per config)")
     ap.add_argument("--work-gb", type=int, default=0, help="tred_convolve workspace cap (GiB), 0 = default")
-    ap.add_argument("--budget-gb", type=int, default=10, help="config 4: block payload per chunk (GiB)")
+    ap.add_argument("--budget-gb", type=int, default=7, help="config 4: block payload per chunk (GiB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
