@@ -565,3 +565,30 @@ def test_attribution_by_reconvolution():
     labelled = {k: v[group >= 0] for k, v in segs.items()}
     whole = sim.simulate(_seg_tensor(labelled), rhat, pix_ids=pix_d)["dense"].cpu().numpy().astype(np.float64)
     assert np.abs(per.sum(0) - whole).max() <= 5e-6 * np.abs(whole).max()
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_empty_and_out_of_window_inputs():
+    """No segments, and segments whose charge falls entirely outside the grid / time window
+    (clip-and-drop, reading G13): no blocks, no tiles, zero waveforms, no error."""
+    torch = _torch()
+    cfg, segs = _small(1)
+    R = gen.make_response(cfg, 2001)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    pix = torch.arange(0, 16, dtype=torch.int32).cuda()
+    empty = torch.empty((8, 0), dtype=torch.float32).cuda()
+    out = sim.simulate(empty, rhat, pix_ids=pix)
+    assert out["nblocks"] == 0 and out["ntiles"] == 0 and float(out["dense"].abs().max()) == 0.0
+    far = {k: v[:50].copy() for k, v in segs.items()}
+    far["x0"] += 1.0e4; far["x1"] += 1.0e4                    # 10 m off the pixel plane
+    out = sim.simulate(_seg_tensor(far), rhat, pix_ids=pix)
+    assert out["nblocks"] == 0 and out["ntiles"] == 0 and float(out["dense"].abs().max()) == 0.0
+    assert len(o.blocks(cfg, o.drift(cfg, far))) == 0
+    late = {k: v[:50].copy() for k, v in segs.items()}
+    late["t0"] += 1.0e4                                        # arrives after the window
+    out = sim.simulate(_seg_tensor(late), rhat, pix_ids=pix)
+    assert out["nblocks"] == len(o.blocks(cfg, o.drift(cfg, late))) == 0
+    # chunked driver on an empty event
+    out = sim.simulate_chunked(empty, rhat, pix_ids=pix)
+    assert out["ntiles"] == 0 and float(out["dense"].abs().max()) == 0.0
