@@ -318,6 +318,24 @@ int tred_readout(const tred_readout_config* cfg, int64_t npix, int32_t nticks, c
                  void* stream);
 
 /*
+ * tred_truth -- truth record ("segment-id -> charge per (channel, short time
+ * slice)"; reading G24): the effective charge of every segment summed over the grid
+ * points of each pixel and each time tile (Bt ticks) of its clipped footprint.  One entry per
+ * (pixel, tile) the footprint reaches, ordered by segment, then by key.
+ *   d_augf, d_augi  from tred_drift
+ *   d_rec_seg [cap_rec] int32 out, d_rec_key [cap_rec] int64 out ((tile * npix_x + px) * npix_y + py,
+ *             the key of tred_convolve_plan's tiles), d_rec_q [cap_rec] float32 out (electrons)
+ *   d_nrec    int64 out: number of entries (TRED_ECAP semantics: may exceed cap_rec, nothing
+ *             beyond the capacity is written)
+ *   d_work    at least tred_truth_work_bytes(nseg) bytes
+ * A segment reaching more than 16 pixels or tiles along one axis is truncated to 16.
+ */
+size_t tred_truth_work_bytes(const tred_ctx* ctx, int64_t nseg);
+int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, const int32_t* d_augi, int64_t cap_rec,
+               int32_t* d_rec_seg, int64_t* d_rec_key, float* d_rec_q, int64_t* d_nrec, void* d_work,
+               size_t work_bytes, void* stream);
+
+/*
  * Stage profiling (the paper's "profiler-guided optimization", Fig. 10).
  * tred_profile_begin clears the counters; with record_events != 0 every stage of the
  * following calls is bracketed by CUDA events on the launching stream.

@@ -468,3 +468,50 @@ def readout(par, wave, noise=None):
                     thr = np.float32(thr0 + nz(0))
                 state, left = (2, int(par["n_reset"])) if par["n_reset"] > 0 else (0, 0)
     return nhit, tick, adc
+
+
+# ---------------------------------------------------------------------------
+# N4: truth record -- PAPER.md:L352-354 ("segment-id -> charge per
+# (channel, short time slice)").  Reading G24 of DESIGN.md: the record of segment s is its
+# effective charge (Eq. (9)) summed over the grid points of every pixel and every time tile
+# of Bt ticks it reaches, one entry per (pixel, tile) of the clipped integer footprint
+# [lo - e, hi + e] (entries at the rim of the footprint may hold tiny values), ordered by
+# segment, then by the tile key (tb * npix_x + px) * npix_y + py.
+# ---------------------------------------------------------------------------
+def truth_record(cfg, aug, segs_sel=None):
+    """Returns (seg [n] int32, key [n] int64, charge [n] float64)."""
+    g = grid_of(cfg)
+    e = 1 if cfg.gl_n > 1 else 0
+    S, Bt = cfg.sub, cfg.block[2]
+    nseg = len(aug["Qp"]) if "Qp" in aug else aug["lo"].shape[0]
+    sel = range(nseg) if segs_sel is None else segs_sel
+    rs, rk, rq = [], [], []
+    all_keys = None
+    for s in sel:
+        lo = np.maximum(aug["lo"][s] - e, 0)
+        hi = np.minimum(aug["hi"][s] + e, np.array(g.NG) - 1)
+        if np.any(lo > hi):
+            continue
+        # this segment alone, on the blocks it touches
+        sub = {k: (v[s:s + 1] if hasattr(v, "shape") and v.shape[:1] == (nseg,) else v) for k, v in aug.items()}
+        keys_s = blocks(cfg, sub)
+        pay = effq(cfg, sub, keys_s)
+        bx, by, bt = key_to_bxyz(g, keys_s)
+        Bx, By = cfg.block[0], cfg.block[1]
+        acc = {}
+        for b in range(len(keys_s)):
+            i = Bx * bx[b] + np.arange(Bx)
+            j = By * by[b] + np.arange(By)
+            k = Bt * bt[b] + np.arange(Bt)
+            for px in np.unique(i // S):
+                mi = (i // S == px) & (i >= lo[0]) & (i <= hi[0])
+                for py in np.unique(j // S):
+                    mj = (j // S == py) & (j >= lo[1]) & (j <= hi[1])
+                    mk = (k >= lo[2]) & (k <= hi[2])
+                    if not (mi.any() and mj.any() and mk.any()) or px >= cfg.npix_x or py >= cfg.npix_y:
+                        continue
+                    key = (int(bt[b]) * cfg.npix_x + int(px)) * cfg.npix_y + int(py)
+                    acc[key] = acc.get(key, 0.0) + float(pay[b][np.ix_(mi, mj, mk)].sum())
+        for key in sorted(acc):
+            rs.append(s); rk.append(key); rq.append(acc[key])
+    return np.asarray(rs, np.int32), np.asarray(rk, np.int64), np.asarray(rq, np.float64)

@@ -93,6 +93,8 @@ EXPORTS = {
     "tred_steps": (C.c_int, [C.POINTER(TredStepsConfig), _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
                              C.c_size_t, _c_p]),
     "tred_readout": (C.c_int, [C.POINTER(TredReadoutConfig), _c_i64, C.c_int32, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p]),
+    "tred_truth_work_bytes": (C.c_size_t, [_c_p, _c_i64]),
+    "tred_truth": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
     "tred_profile_end": (C.c_int, [_c_p, C.c_int, _c_p, _c_p]),
     "tred_stage_count": (C.c_int, []),
@@ -432,7 +434,25 @@ class Tred:
                        sp_keys=sp_keys[:nsp], sp_data=sp_data[:nsp], sp_off=sp_off)
         return out
 
-    # -- truth attribution ---------------------------
+    # -- truth record --------------------------------
+    def truth(self, augf, augi, cap_rec: int | None = None):
+        """Charge of every segment per (pixel, time tile): (rec_seg, rec_key, rec_q, nrec)."""
+        t = self.torch
+        nseg = augf.shape[1]
+        work = self._workbuf("truth", self.L.tred_truth_work_bytes(self.h, nseg))
+        nrec = self._empty((1,), t.int64)
+        if cap_rec is None:                         # counting pass
+            _check(self.L.tred_truth(self.h, nseg, _ptr(augf), _ptr(augi), 0, None, None, None, _ptr(nrec),
+                                     _ptr(work), work.numel(), self._stream()), "tred_truth")
+            cap_rec = int(nrec.item())
+        rs = self._empty((max(cap_rec, 1),), t.int32)
+        rk = self._empty((max(cap_rec, 1),), t.int64)
+        rq = self._empty((max(cap_rec, 1),), t.float32)
+        _check(self.L.tred_truth(self.h, nseg, _ptr(augf), _ptr(augi), cap_rec, _ptr(rs), _ptr(rk), _ptr(rq),
+                                 _ptr(nrec), _ptr(work), work.numel(), self._stream()), "tred_truth")
+        return rs[:cap_rec], rk[:cap_rec], rq[:cap_rec], nrec
+
+    # -- truth attribution (SURVEY.md Sec. 8(f) N4; PAPER.md:L356) ---------------------------------
     def attribute(self, seg, rhat, group, pix_ids, ngroups: int | None = None):
         """On-demand waveform attribution "by re-convolving selected contributions"
         (PAPER.md:L356): the path is linear in the segment charges, so the waveform a group of

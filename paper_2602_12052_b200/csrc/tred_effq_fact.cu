@@ -441,6 +441,116 @@ int tred_effq_init_tables(void) {
   return TRED_OK;
 }
 
+// ------------------------------------------------------------------ N4: truth record
+// "segment-id -> charge per (channel, short time slice)".  Reading G24:
+// the effective charge of segment s summed over the grid points of every pixel and time tile
+// (Bt ticks) its clipped footprint [lo - e, hi + e] reaches.  With the factored form of the
+// charge the sum over a pixel x tile box factors too:
+//   Q[s][px][py][tb] = sum_m (K W_m sum_{i in px} GX_m[i]) (sum_{j in py} GY_m[j]) (sum_{k in tb} GT_m[k]).
+constexpr int TR_MAXG = 16;          // pixel / tile groups per axis a segment may reach
+
+struct TruthBox { int lo[3], hi[3], g0[3], ng[3]; };
+
+__device__ __forceinline__ bool truth_box(const int32_t* __restrict__ augi, int64_t nseg, int64_t s, const TredGrid& g,
+                                          int E, TruthBox& b) {
+  const int NG[3] = {g.NGx, g.NGy, g.NGt}, div[3] = {g.S, g.S, g.Bt};
+  bool ok = true;
+  for (int a = 0; a < 3; ++a) {
+    b.lo[a] = max(augi[a * nseg + s] - E, 0);
+    b.hi[a] = min(augi[(3 + a) * nseg + s] + E, NG[a] - 1);
+    ok = ok && b.lo[a] <= b.hi[a];
+    b.g0[a] = b.lo[a] / div[a];
+    b.ng[a] = ok ? min(b.hi[a] / div[a] - b.g0[a] + 1, TR_MAXG) : 0;
+  }
+  return ok;
+}
+
+template <int N>
+__global__ void __launch_bounds__(256)
+k_truth_count(int64_t nseg, const int32_t* __restrict__ augi, TredGrid g, int32_t* __restrict__ cnt) {
+  const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s > nseg) return;
+  int c = 0;
+  if (s < nseg) {
+    TruthBox b;
+    if (truth_box(augi, nseg, s, g, N > 1 ? 1 : 0, b)) c = b.ng[0] * b.ng[1] * b.ng[2];
+  }
+  cnt[s] = c;
+}
+
+// one warp per segment
+template <int N>
+__global__ void __launch_bounds__(128)
+k_truth_fill(int64_t nseg, const float* __restrict__ augf, const int32_t* __restrict__ augi,
+             const int32_t* __restrict__ first, TredGrid g, int64_t cap, int32_t* __restrict__ rec_seg,
+             int64_t* __restrict__ rec_key, float* __restrict__ rec_q, int64_t* __restrict__ d_nrec) {
+  __shared__ float sums[4][3 * TR_MAXG][MMAX];
+  const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t s = (int64_t)blockIdx.x * 4 + wid;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *d_nrec = first[nseg];
+  if (s >= nseg) return;
+  constexpr int E = N > 1 ? 1 : 0;
+  constexpr float LOG2E_HALF = 0.72134752044448170f;
+  TruthBox b;
+  if (!truth_box(augi, nseg, s, g, E, b)) return;
+  const int nrec = b.ng[0] * b.ng[1] * b.ng[2];
+  const int64_t f0 = first[s];
+  const int lo3[3] = {augi[0 * nseg + s], augi[1 * nseg + s], augi[2 * nseg + s]};
+  const int hi3[3] = {augi[3 * nseg + s], augi[4 * nseg + s], augi[5 * nseg + s]};
+  const int flag = augi[6 * nseg + s];
+  const float p0[3] = {augf[0 * nseg + s], augf[1 * nseg + s], augf[2 * nseg + s]};
+  const float d3[3] = {augf[3 * nseg + s] - p0[0], augf[4 * nseg + s] - p0[1], augf[5 * nseg + s] - p0[2]};
+  const float sg[3] = {augf[6 * nseg + s], augf[7 * nseg + s], augf[8 * nseg + s]};
+  const float Qp = augf[9 * nseg + s];
+  const float k2[3] = {LOG2E_HALF / (sg[0] * sg[0]), LOG2E_HALF / (sg[1] * sg[1]), LOG2E_HALF / (sg[2] * sg[2])};
+  const float K = Qp * 0.063493635934240969f / (sg[0] * sg[1] * sg[2]) * 0.125f;
+  const SegQuad q = seg_quad(flag, d3[0], d3[1], d3[2], sg[0], sg[1], sg[2]);
+  const int m = q.m, goff = m * (m - 1) / 2;
+  const float inv_np = 1.0f / (float)q.npiece;
+  const int div[3] = {g.S, g.S, g.Bt};
+  float (*S)[MMAX] = sums[wid];
+  float acc = 0.0f;                                       // record `lane` (+ 32, ... handled below)
+  const int ngt = b.ng[0] + b.ng[1] + b.ng[2];
+  for (int r0 = 0; r0 < nrec; r0 += 32) {                 // 32 records at a time (usually one round)
+    acc = 0.0f;
+    for (int pc = 0; pc < q.npiece; ++pc) {
+      __syncwarp();
+      // group sums: lane -> (group, mi), grid points of the group summed in ascending order
+      for (int e = lane; e < ngt * m; e += 32) {
+        const int gi = e / m, mi = e - gi * m;
+        const int a = gi < b.ng[0] ? 0 : gi < b.ng[0] + b.ng[1] ? 1 : 2;
+        const int gl = gi - (a == 0 ? 0 : a == 1 ? b.ng[0] : b.ng[0] + b.ng[1]);
+        float sk, wk;
+        if (flag) { sk = 0.5f; wk = mi == 0 ? 1.0f : 0.0f; }
+        else { sk = ((float)pc + c_gl_s[goff + mi]) * inv_np; wk = c_gl_w[goff + mi] * inv_np; }
+        const float c = fmaf(sk, d3[a], p0[a]);
+        const int i0 = max((b.g0[a] + gl) * div[a], b.lo[a]), i1 = min((b.g0[a] + gl + 1) * div[a] - 1, b.hi[a]);
+        float v = 0.0f;
+        for (int i = i0; i <= i1; ++i) v += axis_entry<N>(i, lo3[a], hi3[a], c, k2[a]);
+        S[gi][mi] = a == 0 ? v * (K * wk) : v;
+      }
+      __syncwarp();
+      const int rr = r0 + lane;
+      if (rr < nrec) {
+        const int gy = rr % b.ng[1], gx = (rr / b.ng[1]) % b.ng[0], gt = rr / (b.ng[1] * b.ng[0]);
+        const float* sx = S[gx];
+        const float* sy = S[b.ng[0] + gy];
+        const float* stt = S[b.ng[0] + b.ng[1] + gt];
+        float v = 0.0f;
+        for (int mi = 0; mi < m; ++mi) v = fmaf(sx[mi] * sy[mi], stt[mi], v);
+        acc += v;
+      }
+    }
+    const int rr = r0 + lane;
+    if (rr < nrec && f0 + rr < cap) {
+      const int gy = rr % b.ng[1], gx = (rr / b.ng[1]) % b.ng[0], gt = rr / (b.ng[1] * b.ng[0]);
+      rec_seg[f0 + rr] = (int32_t)s;
+      rec_key[f0 + rr] = ((int64_t)(b.g0[2] + gt) * g.npx + (b.g0[0] + gx)) * g.npy + (b.g0[1] + gy);
+      rec_q[f0 + rr] = acc;
+    }
+  }
+}
+
 struct EffqWork { int32_t* slot; int32_t* tabslot; int32_t* seglist; void* scan; float* tab; int cap; size_t total; };
 
 static EffqWork carve_effq(void* base, int64_t nseg, size_t work_bytes) {
@@ -531,5 +641,44 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
 #undef LAUNCH
   }
   TRED_LAUNCH_CHECK("k_effq_fact");
+  return TRED_OK;
+}
+
+
+extern "C" size_t tred_truth_work_bytes(const tred_ctx* ctx, int64_t nseg) {
+  if (!ctx || nseg < 0) return 0;
+  return align_up((size_t)(nseg + 1) * 4, 256) + tred_scan_work_bytes(nseg + 1);
+}
+
+extern "C" int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, const int32_t* d_augi, int64_t cap_rec,
+                          int32_t* d_rec_seg, int64_t* d_rec_key, float* d_rec_q, int64_t* d_nrec, void* d_work,
+                          size_t work_bytes, void* stream) {
+  if (!ctx || nseg < 0 || cap_rec < 0 || !d_nrec) return TRED_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (nseg == 0) { TRED_CUDA(cudaMemsetAsync(d_nrec, 0, sizeof(int64_t), st)); return TRED_OK; }
+  if (!d_augf || !d_augi || !d_work) return TRED_EINVAL;
+  if (work_bytes < tred_truth_work_bytes(ctx, nseg)) return TRED_ECAP;
+  if (cap_rec > 0 && (!d_rec_seg || !d_rec_key || !d_rec_q)) return TRED_EINVAL;
+  const TredGrid g = make_grid(ctx);
+  int32_t* first = (int32_t*)d_work;
+  void* scan = (char*)d_work + align_up((size_t)(nseg + 1) * 4, 256);
+#define TRUTH(NN)                                                                                          \
+  do {                                                                                                     \
+    k_truth_count<NN><<<cdiv(nseg + 1, 256), 256, 0, st>>>(nseg, d_augi, g, first);                        \
+    int rc = tred_exclusive_scan_i32(first, first, nseg + 1, nullptr, scan, st);                           \
+    if (rc != TRED_OK) return rc;                                                                          \
+    k_truth_fill<NN><<<cdiv(nseg, 4), 128, 0, st>>>(nseg, d_augf, d_augi, first, g, cap_rec, d_rec_seg,     \
+                                                    d_rec_key, d_rec_q, d_nrec);                           \
+  } while (0)
+  switch (g.gl_n) {
+    case 1: TRUTH(1); break;
+    case 2: TRUTH(2); break;
+    case 3: TRUTH(3); break;
+    case 4: TRUTH(4); break;
+    default: return TRED_EINVAL;
+  }
+#undef TRUTH
+  TRED_COUNT_LAUNCH(2);
+  TRED_LAUNCH_CHECK("tred_truth");
   return TRED_OK;
 }

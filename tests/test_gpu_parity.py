@@ -592,3 +592,29 @@ def test_empty_and_out_of_window_inputs():
     # chunked driver on an empty event
     out = sim.simulate_chunked(empty, rhat, pix_ids=pix)
     assert out["ntiles"] == 0 and float(out["dense"].abs().max()) == 0.0
+
+
+# ------------------------------------------------------------------ N4: truth record
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_truth_record_parity(cfg_id):
+    """tred_truth vs the oracle: (segment, key) lists bit-exact, charges within the
+    effective-charge tolerance; capacity semantics."""
+    torch = _torch()
+    cfg, segs = _small(cfg_id)
+    segs = {k: v[:60] for k, v in segs.items()}
+    aug = o.drift(cfg, segs)
+    rs, rk, rq = o.truth_record(cfg, aug)
+    sim = _sim(cfg)
+    augf, augi, _ = sim.drift(_seg_tensor(segs))
+    gs, gk, gq, nrec = sim.truth(augf, augi)
+    assert int(nrec.item()) == len(rs)
+    np.testing.assert_array_equal(gs.cpu().numpy(), rs)
+    np.testing.assert_array_equal(gk.cpu().numpy(), rk)
+    got = gq.cpu().numpy().astype(np.float64)
+    assert np.abs(got - rq).max() <= TOL_QEFF * np.abs(rq).max()
+    tot_g = np.bincount(rs, weights=got, minlength=60)
+    tot_r = np.bincount(rs, weights=rq, minlength=60)
+    assert np.allclose(tot_g, tot_r, rtol=1e-5)
+    gs2, gk2, gq2, nrec2 = sim.truth(augf, augi, cap_rec=7)
+    assert int(nrec2.item()) == len(rs) and gs2.numel() == 7
+    np.testing.assert_array_equal(gk2.cpu().numpy(), rk[:7])
