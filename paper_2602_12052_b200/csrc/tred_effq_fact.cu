@@ -253,7 +253,7 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
   // Segment records of the block are staged in shared memory SB at a time (one pass of
   // coalesced loads instead of two dependent global loads per segment and thread).
   constexpr int SB = 32, NF = 18;                      // 7 int fields (bbox, flag), 10 floats, table slot
-  constexpr int NX = 6;                                // derived: k2x, k2y, k2t, K, npiece, m
+  constexpr int NX = 20;    // derived once per segment: k2x, k2y, k2t, K, npiece, m, clipped box, work split
   __shared__ int32_t s_rec[SB][NF + NX + 1];
   __shared__ int s_list[SB];
   __shared__ int s_cnt;
@@ -290,6 +290,21 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
         rec[NF + 3] = __float_as_int(__int_as_float(rec[16]) * 0.063493635934240969f / (sx * sy * st) * 0.125f);
         rec[NF + 4] = q.npiece;
         rec[NF + 5] = q.m;
+        // clipped footprint and the phase-B work split (ncol columns x nsplit tick chunks); item / ncolp,
+        // col / ny and entry / m by multiplication: exact for arguments < 2048 and divisors <= 1024
+        const int ix0 = max(rec[0] - E, I0), ix1 = min(min(rec[3] + E, I0 + g.Bx - 1), g.NGx - 1);
+        const int iy0 = max(rec[1] - E, J0), iy1 = min(min(rec[4] + E, J0 + g.By - 1), g.NGy - 1);
+        const int kt0 = max(rec[2] - E, K0), kt1 = min(min(rec[5] + E, K0 + P.TS - 1), g.NGt - 1);
+        const int nx = ix1 - ix0 + 1, ny = iy1 - iy0 + 1, nt = kt1 - kt0 + 1;
+        const int ncol = nx * ny, ncolp = (ncol + 31) & ~31;
+        const int nsplit = ncolp < NT ? NT / ncolp : 1;
+        rec[NF + 6] = ix0; rec[NF + 7] = nx; rec[NF + 8] = iy0; rec[NF + 9] = ny;
+        rec[NF + 10] = kt0; rec[NF + 11] = nt;
+        rec[NF + 12] = ncolp; rec[NF + 13] = nsplit; rec[NF + 14] = (nt + nsplit - 1) / nsplit;
+        rec[NF + 15] = (65536 + ncolp - 1) / ncolp; rec[NF + 16] = (65536 + ny - 1) / ny;
+        rec[NF + 17] = (65536 + q.m - 1) / q.m;
+        rec[NF + 18] = q.m * (q.m - 1) / 2;
+        rec[NF + 19] = __float_as_int(1.0f / (float)q.npiece);
       }
     }
     const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
@@ -302,11 +317,6 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
     const int32_t* rec = s_rec[s_list[sl]];
     const int lox = rec[0], loy = rec[1], lot = rec[2];
     const int hix = rec[3], hiy = rec[4], hit = rec[5];
-    // grid points of the segment's footprint inside this tile (and the grid)
-    const int ix0 = max(lox - E, I0), ix1 = min(min(hix + E, I0 + g.Bx - 1), g.NGx - 1);
-    const int iy0 = max(loy - E, J0), iy1 = min(min(hiy + E, J0 + g.By - 1), g.NGy - 1);
-    const int kt0 = max(lot - E, K0), kt1 = min(min(hit + E, K0 + P.TS - 1), g.NGt - 1);
-    const int nx = ix1 - ix0 + 1, ny = iy1 - iy0 + 1, nt = kt1 - kt0 + 1;
     const int flag = rec[6];
     const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
     const float dx = __int_as_float(rec[10]) - p0x, dy = __int_as_float(rec[11]) - p0y,
@@ -315,15 +325,12 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
                 k2t = __int_as_float(rec[NF + 2]), K = __int_as_float(rec[NF + 3]);
     const int npiece = rec[NF + 4], m = rec[NF + 5];
     const int slot = rec[17];
-    const int goff = m * (m - 1) / 2;
-    const float inv_np = 1.0f / (float)npiece;
-    // phase-B work split: ncol columns x nsplit tick chunks
-    const int ncol = nx * ny;
-    const int ncolp = (ncol + 31) & ~31;
-    const int nsplit = ncolp < NT ? NT / ncolp : 1;
-    const int chunk = (nt + nsplit - 1) / nsplit;
-    // item / ncolp and col / ny by multiplication: exact for item, col < 2048 and divisors <= 1024
-    const int inv_ncolp = (65536 + ncolp - 1) / ncolp, inv_ny = (65536 + ny - 1) / ny;
+    // clipped footprint and work split, computed once per segment by the batch prologue
+    const int ix0 = rec[NF + 6], nx = rec[NF + 7], iy0 = rec[NF + 8], ny = rec[NF + 9];
+    const int kt0 = rec[NF + 10], nt = rec[NF + 11];
+    const int ncol = nx * ny, ncolp = rec[NF + 12], nsplit = rec[NF + 13], chunk = rec[NF + 14];
+    const int inv_ncolp = rec[NF + 15], inv_ny = rec[NF + 16], inv_m = rec[NF + 17], goff = rec[NF + 18];
+    const float inv_np = __int_as_float(rec[NF + 19]);
 
     for (int pc = 0; pc < npiece; ++pc, ++it) {
       float* GX = tabs + (it & 1) * tabn;             // [Bx][MP]
@@ -347,7 +354,7 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
         }
       } else
       for (int e = threadIdx.x; e < nent; e += NT) {
-        const int r = e / m, mi = e - r * m;
+        const int r = (e * inv_m) >> 16, mi = e - r * m;      // e / m
         float sk, wk;
         if (flag) { sk = 0.5f; wk = mi == 0 ? 1.0f : 0.0f; }      // point-like: midpoint Gaussian
         else { sk = ((float)pc + c_gl_s[goff + mi]) * inv_np; wk = c_gl_w[goff + mi] * inv_np; }
