@@ -66,6 +66,27 @@ struct FactParams {
 
 // One table entry: grid point gi of one axis, quadrature centre c (grid units relative to
 // lo), k2 = log2(e) / (2 sigma^2).
+// Contributions of the n nodes of dual cell gi (between grid points gi and gi + 1) to the
+// table entries of gi (coefficient 1 - s) and of gi + 1 (coefficient s): the same n
+// exponentials serve both, so a row of entries costs n, not 2n, exponentials per entry
+// (entry(gi) = own(gi) + up(gi - 1)); same arithmetic per term as axis_entry.
+template <int N>
+__device__ __forceinline__ void axis_cell(int gi, int lo, int hi, float c, float k2, float& own, float& up) {
+  own = 0.0f; up = 0.0f;
+  const float base = (float)(gi - lo) + 0.5f;
+#pragma unroll
+  for (int q = 0; q < N; ++q) {
+    const float sq = DualGL<N>::s(q), wq = DualGL<N>::w(q);
+    const int cub = gi + DualGL<N>::side(q);
+    const float z = (base + sq) - c;
+    const float e = ex2_approx(-z * z * k2);
+    if (cub >= lo && cub <= hi) {
+      own = fmaf(wq * (1.0f - sq), e, own);
+      if (sq != 0.0f) up = fmaf(wq * sq, e, up);
+    }
+  }
+}
+
 template <int N>
 __device__ __forceinline__ float axis_entry(int gi, int lo, int hi, float c, float k2) {
   float v = 0.0f;
@@ -253,7 +274,7 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
   // Segment records of the block are staged in shared memory SB at a time (one pass of
   // coalesced loads instead of two dependent global loads per segment and thread).
   constexpr int SB = 32, NF = 18;                      // 7 int fields (bbox, flag), 10 floats, table slot
-  constexpr int NX = 20;    // derived once per segment: k2x, k2y, k2t, K, npiece, m, clipped box, work split
+  constexpr int NX = 21;    // derived once per segment: k2x, k2y, k2t, K, npiece, m, clipped box, work split
   __shared__ int32_t s_rec[SB][NF + NX + 1];
   __shared__ int s_list[SB];
   __shared__ int s_cnt;
@@ -305,6 +326,7 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
         rec[NF + 17] = (65536 + q.m - 1) / q.m;
         rec[NF + 18] = q.m * (q.m - 1) / 2;
         rec[NF + 19] = __float_as_int(1.0f / (float)q.npiece);
+        rec[NF + 20] = (65536 + (nx + ny + nt) - 1) / (nx + ny + nt);
       }
     }
     const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
@@ -329,8 +351,9 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
     const int ix0 = rec[NF + 6], nx = rec[NF + 7], iy0 = rec[NF + 8], ny = rec[NF + 9];
     const int kt0 = rec[NF + 10], nt = rec[NF + 11];
     const int ncol = nx * ny, ncolp = rec[NF + 12], nsplit = rec[NF + 13], chunk = rec[NF + 14];
-    const int inv_ncolp = rec[NF + 15], inv_ny = rec[NF + 16], inv_m = rec[NF + 17], goff = rec[NF + 18];
+    const int inv_ncolp = rec[NF + 15], inv_ny = rec[NF + 16], goff = rec[NF + 18];
     const float inv_np = __int_as_float(rec[NF + 19]);
+    const int nr = nx + ny + nt, inv_nr = rec[NF + 20];
 
     for (int pc = 0; pc < npiece; ++pc, ++it) {
       float* GX = tabs + (it & 1) * tabn;             // [Bx][MP]
@@ -353,21 +376,36 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
               __ldg(reinterpret_cast<const float4*>(T + src * TAB_M) + c4);
         }
       } else
-      for (int e = threadIdx.x; e < nent; e += NT) {
-        const int r = (e * inv_m) >> 16, mi = e - r * m;      // e / m
+      // entry e = (quadrature point mi, row r of the concatenated x | y | t rows), rows along the
+      // lanes: a lane evaluates the n exponentials of dual cell gi once, for its own entry and
+      // for the entry of gi + 1, which the next lane picks up by a shuffle (the first row of an
+      // axis and lane 0 evaluate the cell below themselves)
+      for (int e = threadIdx.x; e - (int)(threadIdx.x & 31) < nent; e += NT) {
+        const bool act = e < nent;
+        const int ee = act ? e : nent - 1;
+        const int mi = (ee * inv_nr) >> 16, r = ee - mi * nr;     // ee / nr
         float sk, wk;
         if (flag) { sk = 0.5f; wk = mi == 0 ? 1.0f : 0.0f; }      // point-like: midpoint Gaussian
         else { sk = ((float)pc + c_gl_s[goff + mi]) * inv_np; wk = c_gl_w[goff + mi] * inv_np; }
+        int gi, lo_a, hi_a, rr; float c, k2a, scale; float* dstp;
         if (r < nx) {
-          const float v = axis_entry<N>(ix0 + r, lox, hix, fmaf(sk, dx, p0x), k2x);
-          GX[r * MP + mi] = v * (K * wk);
+          rr = r; gi = ix0 + rr; lo_a = lox; hi_a = hix; c = fmaf(sk, dx, p0x); k2a = k2x; scale = K * wk;
+          dstp = GX + rr * MP + mi;
         } else if (r < nx + ny) {
-          const int rr = r - nx;
-          GY[rr * MP + mi] = axis_entry<N>(iy0 + rr, loy, hiy, fmaf(sk, dy, p0y), k2y);
+          rr = r - nx; gi = iy0 + rr; lo_a = loy; hi_a = hiy; c = fmaf(sk, dy, p0y); k2a = k2y; scale = 1.0f;
+          dstp = GY + rr * MP + mi;
         } else {
-          const int rr = r - nx - ny;
-          GT[rr * MP + mi] = axis_entry<N>(kt0 + rr, lot, hit, fmaf(sk, dt, p0t), k2t);
+          rr = r - nx - ny; gi = kt0 + rr; lo_a = lot; hi_a = hit; c = fmaf(sk, dt, p0t); k2a = k2t; scale = 1.0f;
+          dstp = GT + rr * MP + mi;
         }
+        float own, up;
+        axis_cell<N>(gi, lo_a, hi_a, c, k2a, own, up);
+        float below = __shfl_up_sync(0xffffffffu, up, 1);
+        if (N > 1 && (rr == 0 || (threadIdx.x & 31) == 0)) {       // no lane holds cell gi - 1 of this axis
+          float o2;
+          axis_cell<N>(gi - 1, lo_a, hi_a, c, k2a, o2, below);
+        }
+        if (act) *dstp = (N > 1 ? own + below : own) * scale;
       }
       __syncthreads();
       // ---- phase B: tile[k][i][j] += sum_mi GX[i][mi] GY[j][mi] GT[k][mi]
