@@ -138,7 +138,7 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           float4 h, l;
           h.x = tf32_hi(v.x); h.y = tf32_hi(v.y); h.z = tf32_hi(v.z); h.w = tf32_hi(v.w);
           l.x = tf32_hi(v.x - h.x); l.y = tf32_hi(v.y - h.y); l.z = tf32_hi(v.z - h.z); l.w = tf32_hi(v.w - h.w);
-          a[tc + 128 * i] = h;
+          // A_hi stays as loaded: kind::tf32 reads only the upper 19 bits of an operand (h is what it sees)
           lo[tc + 128 * i] = l;
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor core reads
