@@ -193,8 +193,8 @@ k_fill_blockmap(int64_t nblocks, const int64_t* __restrict__ keys, int32_t* __re
 
 // ------------------------------------------------------------------ row tiles
 // The tensor-core path orders the charge pixels of a slab by (strip = px / 8, py, px % 8)
-// and cuts every (slab, strip) sequence into row tiles of at most RT_ROWS rows made of
-// whole py-lines, at most RT_PY - 2H lines tall.  The outputs of a row tile then fall in
+// and cuts every (slab, strip) sequence into row tiles of at most RT_ROWS consecutive rows,
+// at most RT_PY - 2H lines tall (a py-line may be split between two tiles).  The outputs of a row tile then fall in
 // the patch [8 strip - H, 8 strip + 7 + H] x [py0 - H, py0 + ny - 1 + H], small enough to
 // be summed over the offsets in shared memory by the GEMM epilogue.
 struct RtGeom { int nstrip, ngrp, capy; int64_t nmap2, cap_rt; };
@@ -249,17 +249,21 @@ k_rt_tiles(int ngrp, int npy, int capy, const int32_t* __restrict__ ridx, int32_
   if (grp >= ngrp) return;
   const int32_t* line = ridx + (int64_t)grp * npy * RT_SW;      // line[py * 8] = first row of the line
   int t = WRITE ? off[grp] : 0;
-  int py = 0;
+  int py = 0, used = 0;                 // used: rows of line py already given to a tile
   while (py < npy) {
-    if (line[(py + 1) * RT_SW] == line[py * RT_SW]) { ++py; continue; }
-    const int py0 = py, row0 = line[py * RT_SW];
+    if (line[(py + 1) * RT_SW] - line[py * RT_SW] - used == 0) { ++py; used = 0; continue; }
+    // a tile takes rows in order until it holds RT_ROWS (a line may be split between two tiles:
+    // every row carries its own pixel, the patch only has to cover the lines of its rows)
+    const int py0 = py, row0 = line[py * RT_SW] + used;
     int rows = 0, last = py;
     while (py < npy && py - py0 < capy) {
-      const int c = line[(py + 1) * RT_SW] - line[py * RT_SW];
-      if (rows + c > RT_ROWS) break;
-      if (c > 0) last = py;
-      rows += c;
-      ++py;
+      const int c = line[(py + 1) * RT_SW] - line[py * RT_SW] - used;
+      const int take = min(c, RT_ROWS - rows);
+      if (take > 0) last = py;
+      rows += take;
+      if (take < c) { used += take; break; }             // full inside this line
+      ++py; used = 0;
+      if (rows == RT_ROWS) break;
     }
     if (WRITE && t < cap_rt) desc[t] = make_int4(row0, rows, py0, last - py0 + 1);
     ++t;
@@ -712,7 +716,7 @@ k_accum(const float2* __restrict__ T, const int64_t* __restrict__ sp_keys, int s
 // tile order onto the running value of ohat, so the sequence of additions is the same for
 // any chunking.  One CTA per 32 consecutive slab pixels; reads are coalesced over the
 // pixels, the ohat update over the frequencies (transposed through shared memory).
-constexpr int ACC_MAXE = 8;
+constexpr int ACC_MAXE = 12;
 
 __global__ void __launch_bounds__(256)
 k_accum_tiles(const float2* __restrict__ opart, const int64_t* __restrict__ sp_keys, int s0, int ns,
