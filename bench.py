@@ -183,6 +183,8 @@ def run_cuda(args):
         dist.init_process_group("nccl", device_id=dev)
 
     cfg, segs, seg_h, R = workload(args.config, rank)
+    if args.mac_mode:
+        cfg = cfg.with_(mac_mode=args.mac_mode)
     nseg = seg_h.shape[1]
     sim = Tred(cfg, device=dev, conv_work_bytes=args.work_gb << 30 if args.work_gb else None)
     rhat = sim.prepare_response(torch.from_numpy(R).to(dev))       # once per response
@@ -322,8 +324,9 @@ def run_cuda(args):
         pk = {"hbm": (hbm, "GB/s", 1e9, hbm_src),
               "alu": (alu_peak, "TFLOP/s", 1e12, "derived: 148 SM x 128 lanes x 2 x sm_max_mhz (DESIGN.md)"),
               "tensor": (tf32_peak, "TFLOP/s", 1e12,
-                         "tf32 dense = measured bf16_tflops x 1/2 (nominal ratio); the kernel executes "
-                         "3 tf32 products per algorithmic fp32 product (3xTF32), so 1/3 is its ceiling")}
+                         "tf32 dense = measured bf16_tflops x 1/2 (nominal ratio); the kernel executes one tf32 "
+                         "and two bf16 products per algorithmic fp32 product (2 tf32-equivalents), so 1/2 "
+                         "is its ceiling")}
         nlaunch = {k: v[1] for k, v in stage_prof_last.items()}
         traffic = _load_traffic(cfg.name)
         stage_roof = {}
@@ -339,9 +342,11 @@ def run_cuda(args):
                              "work_per_launch": w / nl, "peak_source": src,
                              "traffic": (tr / nl) if tr else None}
         if "mac" in stage_roof and stage_roof["mac"]["bound"] == "tensor":
-            # what the tensor cores execute: 3 tf32 products per fp32 product, row tiles of 128
-            # rows (partly filled), 2 x 128 output columns for 2 x 121 offsets
-            ex = 3.0 * 2.0 * info["nrt"] * 128 * (2 * d.n_off_pad) * (2 * d.n_phase) * nf
+            # what the tensor cores execute: 3 products per fp32 product (tf32-equivalent: the two
+            # bf16 correction products of the default mode run at twice the tf32 rate and count
+            # half), row tiles of 128 rows (partly filled), 2 x 128 output columns for 2 x 121 offsets
+            nprod = 3.0 if sim.cfg.mac_mode in (2, 3, 4, 5) else 2.0
+            ex = nprod * 2.0 * info["nrt"] * 128 * (2 * d.n_off_pad) * (2 * d.n_phase) * nf
             stage_roof["mac"]["executed_tflops"] = ex / (stage_ms["mac"] * 1e-3) / 1e12
             stage_roof["mac"]["executed_frac"] = stage_roof["mac"]["executed_tflops"] / tf32_peak
         dom = max(stage_roof, key=lambda k: stage_ms[k])
@@ -495,6 +500,7 @@ def main():
     ap.add_argument("--ref-segments", type=int, default=0, help="oracle sample size (0 = per config)")
     ap.add_argument("--work-gb", type=int, default=0, help="tred_convolve workspace cap (GiB), 0 = default")
     ap.add_argument("--budget-gb", type=int, default=7, help="config 4: block payload per chunk (GiB)")
+    ap.add_argument("--mac-mode", type=int, default=0, help="tred_config.mac_mode (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

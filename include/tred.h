@@ -68,10 +68,12 @@ typedef struct tred_config {
                                     0 = factored line integral (default, see tred_effq),
                                     1 = closed form with erf per Gauss-Legendre node          */
   int32_t mac_mode;              /* spectrum multiply-accumulate of tred_convolve:
-                                    0 = default: tensor cores (3xTF32) over row tiles with
-                                        the sum over the offsets fused into the epilogue, on
-                                        CTA pairs (tcgen05 cta_group::2) if supported, else
-                                        as 3, else as 2, else as 1,
+                                    0 = default: tensor cores over row tiles with the sum over
+                                        the offsets fused into the epilogue, on CTA pairs
+                                        (tcgen05 cta_group::2); operands split x = hi + lo, the
+                                        main product hi*hi in tf32, the two corrections lo*hi,
+                                        hi*lo (2^-11 of it) in bf16; if unsupported as 3, 2, 1,
+                                    5 = as 0 with all three products in tf32 (3xTF32),
                                     3 = as 0 on single CTAs,
                                     4 = as 0 with the mirror symmetry of the response
                                         (MPCP) spent on the product: sums and

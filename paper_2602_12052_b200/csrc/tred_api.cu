@@ -97,7 +97,7 @@ extern "C" int tred_get_dims(const tred_config* c, tred_dims* d) {
   if (c->npix_x <= 0 || c->npix_y <= 0 || c->sub <= 0 || c->nticks <= 0) return TRED_EINVAL;
   if (c->gl_n < 1 || c->gl_n > 4) return TRED_EINVAL;
   if (c->resp_half < 0 || c->resp_nticks <= 0) return TRED_EINVAL;
-  if (c->effq_mode < 0 || c->effq_mode > 1 || c->mac_mode < 0 || c->mac_mode > 4) return TRED_EINVAL;
+  if (c->effq_mode < 0 || c->effq_mode > 1 || c->mac_mode < 0 || c->mac_mode > 5) return TRED_EINVAL;
   if (!(c->pitch_mm > 0) || !(c->tick_us > 0) || !(c->v_mm_us > 0) || !(c->lifetime_us > 0))
     return TRED_EINVAL;
   if (!(c->nsigma > 0) || !(c->sigma_min_xy_mm > 0) || !(c->sigma_min_t_us > 0)) return TRED_EINVAL;

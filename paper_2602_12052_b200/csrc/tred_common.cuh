@@ -85,8 +85,9 @@ static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 // ---- layout of the response-spectrum buffer d_rhat (tred_prepare_response) ---------------
 // [W: fp32 complex [f][phase][kp]] [B_hi][B_lo: [f][2 kp][2 nph] tf32 parts]
 // [Bs_hi][Bs_lo][Bd_hi][Bd_lo: [f][SYM_N][nph] mirror-symmetric halves, see tred_conv.cu] [flag]
+// [B_hi, B_lo rounded to bf16, same shape as B_hi: operands of the bf16 correction products]
 constexpr int SYM_N = 128;           // rows of the symmetric matrices: 2 x (noff + 1) / 2 padded
-struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, total; };
+struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, bhb, blb, total; };
 static inline RhatLayout rhat_layout(const tred_dims& d) {
   RhatLayout L;
   const int64_t rb = (int64_t)d.n_freq * d.n_phase * d.n_off_pad;
@@ -94,7 +95,9 @@ static inline RhatLayout rhat_layout(const tred_dims& d) {
   L.w = 0; L.bhi = 2 * rb; L.blo = 6 * rb;
   L.bs_hi = 10 * rb; L.bs_lo = L.bs_hi + sb; L.bd_hi = L.bs_lo + sb; L.bd_lo = L.bd_hi + sb;
   L.flag = L.bd_lo + sb;
-  L.total = L.flag + 8;
+  L.bhb = L.flag + 8;                 // bf16 copies of B_hi and B_lo, [f][2 kp][2 nph] bf16 = 2 rb floats each
+  L.blb = L.bhb + 2 * rb;
+  L.total = L.blb + 2 * rb;
   return L;
 }
 

@@ -15,6 +15,7 @@
 //   (d) one inverse real FFT per slab pixel                               (k_ifft)
 //   (e) overlap-add of the slab outputs into tiles (pixel, Bt ticks)      (k_gather_*)
 // Spectra hold L/2 complex numbers: slot 0 packs (DC, Nyquist), both real.
+#include <cuda_bf16.h>
 #include "tred_common.cuh"
 #include "tred_fft.cuh"
 
@@ -38,7 +39,8 @@ __device__ __forceinline__ float tf32_trunc(float x) {
 
 __global__ void __launch_bounds__(256)
 k_resp_dft64(const float* __restrict__ resp, float2* __restrict__ W, float* __restrict__ Bhi,
-             float* __restrict__ Blo, int Tr, int L, int noff, int kp, int nph) {
+             float* __restrict__ Blo, __nv_bfloat16* __restrict__ Bhb, __nv_bfloat16* __restrict__ Blb,
+             int Tr, int L, int noff, int kp, int nph) {
   extern __shared__ double smd[];
   double2* tw = reinterpret_cast<double2*>(smd);       // [L]  exp(-2 pi i k / L)
   double* r = smd + 2 * L;                              // [Tr]
@@ -62,10 +64,14 @@ k_resp_dft64(const float* __restrict__ resp, float2* __restrict__ W, float* __re
     const float fre = (float)re, fim = (float)im;
     float* bh = Bhi + (int64_t)(f == nf ? 0 : f) * bplane;
     float* bl = Blo + (int64_t)(f == nf ? 0 : f) * bplane;
+    __nv_bfloat16* bhb = Bhb + (int64_t)(f == nf ? 0 : f) * bplane;
+    __nv_bfloat16* blb = Blb + (int64_t)(f == nf ? 0 : f) * bplane;
     auto put = [&](int n, int kk, float v) {
       const float h = tf32_trunc(v);
       bh[(int64_t)n * (2 * nph) + kk] = h;
       bl[(int64_t)n * (2 * nph) + kk] = tf32_trunc(v - h);
+      bhb[(int64_t)n * (2 * nph) + kk] = __float2bfloat16_rn(h);        // operands of the bf16 corrections
+      blb[(int64_t)n * (2 * nph) + kk] = __float2bfloat16_rn(v - h);
     };
     if (f == 0) {                       // DC: real lane of slot 0
       W[(int64_t)phase * kp + off].x = fre;
@@ -1103,8 +1109,9 @@ int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const 
 
 // the same on CTA pairs (tred_mac_tc2.cu)
 bool tred_mac_tc2_supported(const tred_ctx* ctx);
-int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
-                 int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
+int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, const void* Bhb,
+                 const void* Blb, float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2,
+                 cudaStream_t st);
 
 // mirror-symmetric response (tred_mac_tc2s.cu)
 bool tred_mac_tc2s_supported(const tred_ctx* ctx);
@@ -1199,8 +1206,10 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
                              d_rhat + rl.bd_lo, (float*)w.opart, nt, t0, pw.rt_desc, pw.row_m2, st);
           if (rc != TRED_OK) return rc;
         } else if (ctx->cfg.mac_mode != 3 && tred_mac_tc2_supported(ctx))
-          rc = tred_mac_tc2(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.opart, nt, t0,
-                            pw.rt_desc, pw.row_m2, st);
+          rc = tred_mac_tc2(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl,
+                            ctx->cfg.mac_mode != 5 ? (const void*)(d_rhat + rl.bhb) : nullptr,
+                            ctx->cfg.mac_mode != 5 ? (const void*)(d_rhat + rl.blb) : nullptr, (float*)w.opart, nt,
+                            t0, pw.rt_desc, pw.row_m2, st);
         if (rc == TRED_EUNSUPPORTED)
           rc = tred_mac_tc_fused(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.opart, nt,
                                  t0, pw.rt_desc, pw.row_m2, st);
@@ -1251,6 +1260,8 @@ extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* 
     TredProfScope ps(ctx, ST_RESP, st);
     TRED_CUDA(cudaMemsetAsync(d_rhat, 0, (size_t)ctx->dims.rhat_floats * 4, st));
     k_resp_dft64<<<nrows, 256, smem, st>>>(d_resp, (float2*)d_rhat, d_rhat + wfl, d_rhat + wfl + bfl,
+                                           reinterpret_cast<__nv_bfloat16*>(d_rhat + rl.bhb),
+                                           reinterpret_cast<__nv_bfloat16*>(d_rhat + rl.blb),
                                            g.Tr, g.L, g.noff, g.kp, g.nph);
     TRED_COUNT_LAUNCH(1);
   }

@@ -18,10 +18,43 @@
 
 namespace {
 
-template <int KC>
+// BF: the two correction products A_lo B_hi and A_hi B_lo (2^-11 of the main product) run as
+// bf16 MMAs (kind::f16, K = 16 per instruction, twice the tf32 rate): the stage then holds
+// A fp32 | A_hi bf16 | A_lo bf16 | B_hi tf32 | B_hi bf16 | B_lo bf16 (the bf16 tiles in 32-byte
+// swizzled rows), and tmBl / tmBl2 are the maps of the bf16 copies of B_hi / B_lo.
+struct T2Maps { CUtensorMap a, bh, bl, bl2; };
+
+__device__ __forceinline__ void tc_mma_bf16_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                                 uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// K-major operand tile of 32-byte swizzled rows (8 rows = one 256-byte swizzle atom)
+__device__ __forceinline__ uint64_t make_desc_sw32(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3ffff) >> 4);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(256 >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)6 << 61;                           // SWIZZLE_32B
+  return d;
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {      // round to nearest even
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+
+template <int KC, bool BF>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1)
-k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmBh,
-          const __grid_constant__ CUtensorMap tmBl, T2Params p) {
+k_mac_tc2(const __grid_constant__ T2Maps tm, T2Params p) {
+  const CUtensorMap& tmA = tm.a;
+  const CUtensorMap& tmBh = tm.bh;
+  const CUtensorMap& tmBl = tm.bl;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;                  // identical in both CTAs of the pair
@@ -72,6 +105,7 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     // ------------------------------------------------------------ TMA producer (each CTA)
     if (lane == 0) {
       const int nh = p.N >> 1;
+      // tf32: B_hi + B_lo rows of 64 bytes; bf16: B_hi 64-byte rows + two bf16 copies of 32-byte rows
       const uint32_t tx = (uint32_t)(T2_A_BYTES + 2 * nh * T2_KC * 4);
       int stage = 0, phase = 0;
       for (int item = cid; item < nitems; item += ncl) {
@@ -90,6 +124,7 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           tma_load_3d(sA(stage), &tmA, kc * T2_KC, mt * T2_M, f, full_bar(stage));
           tma_load_3d(sBh(stage), &tmBh, kc * T2_KC, (int)rank * nh, f, full_bar(stage));
           tma_load_3d(sBl(stage), &tmBl, kc * T2_KC, (int)rank * nh, f, full_bar(stage));
+          if (BF) tma_load_3d(sBl(stage) + T2_BH_BYTES / 2, &tm.bl2, kc * T2_KC, (int)rank * nh, f, full_bar(stage));
           if (++stage == T2_STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -108,13 +143,23 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           mbar_wait(conv_bar(stage), phase);                       // both CTAs: loaded and split
           tc_fence_after();
           const int nks = min(T2_KC, p.K2 - kc * T2_KC) >> 3;
-          const uint64_t da = make_desc_sw64(sA(stage)), dl = make_desc_sw64(sAlo(stage));
-          const uint64_t dbh = make_desc_sw64(sBh(stage)), dbl = make_desc_sw64(sBl(stage));
-          for (int ks = 0; ks < nks; ++ks) {
-            const uint64_t adv = (uint64_t)(ks * 2);
-            tc_mma_tf32_pair(d_tmem, da + adv, dbh + adv, idesc, (kc | ks) != 0);
-            tc_mma_tf32_pair(d_tmem, dl + adv, dbh + adv, idesc, 1);
-            tc_mma_tf32_pair(d_tmem, da + adv, dbl + adv, idesc, 1);
+          const uint64_t da = make_desc_sw64(sA(stage)), dbh = make_desc_sw64(sBh(stage));
+          if (BF) {
+            // bf16 tiles: A_hi | A_lo at sAlo, B_hi | B_lo copies at sBl (32-byte swizzled rows, K = 16)
+            const uint32_t idesc_b = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(p.N >> 3) << 17) |
+                                     ((uint32_t)(256 >> 4) << 24);
+            for (int ks = 0; ks < nks; ++ks)
+              tc_mma_tf32_pair(d_tmem, da + (uint64_t)(ks * 2), dbh + (uint64_t)(ks * 2), idesc, (kc | ks) != 0);
+            tc_mma_bf16_pair(d_tmem, make_desc_sw32(sAlo(stage) + T2_A_BYTES / 2), make_desc_sw32(sBl(stage)), idesc_b, 1);
+            tc_mma_bf16_pair(d_tmem, make_desc_sw32(sAlo(stage)), make_desc_sw32(sBl(stage) + T2_BH_BYTES / 2), idesc_b, 1);
+          } else {
+            const uint64_t dl = make_desc_sw64(sAlo(stage)), dbl = make_desc_sw64(sBl(stage));
+            for (int ks = 0; ks < nks; ++ks) {
+              const uint64_t adv = (uint64_t)(ks * 2);
+              tc_mma_tf32_pair(d_tmem, da + adv, dbh + adv, idesc, (kc | ks) != 0);
+              tc_mma_tf32_pair(d_tmem, dl + adv, dbh + adv, idesc, 1);
+              tc_mma_tf32_pair(d_tmem, da + adv, dbl + adv, idesc, 1);
+            }
           }
           tc_commit_pair(empty_bar(stage));                        // frees the stage in both CTAs
           if (++stage == T2_STAGES) { stage = 0; phase ^= 1; }
@@ -134,12 +179,25 @@ k_mac_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         float4* lo = reinterpret_cast<float4*>(base_ptr + stage * T2_STAGE_BYTES + T2_A_BYTES);
 #pragma unroll
         for (int i = 0; i < T2_A_BYTES / 16 / 128; ++i) {
-          const float4 v = a[tc + 128 * i];
+          const int j = tc + 128 * i;
+          const float4 v = a[j];
           float4 h, l;
           h.x = tf32_hi(v.x); h.y = tf32_hi(v.y); h.z = tf32_hi(v.z); h.w = tf32_hi(v.w);
-          l.x = tf32_hi(v.x - h.x); l.y = tf32_hi(v.y - h.y); l.z = tf32_hi(v.z - h.z); l.w = tf32_hi(v.w - h.w);
           // A_hi stays as loaded: kind::tf32 reads only the upper 19 bits of an operand (h is what it sees)
-          lo[tc + 128 * i] = l;
+          if (BF) {
+            // float4 j of the 64-byte swizzled fp32 tile is row j / 4, logical 16-byte chunk
+            // (j % 4) ^ ((row >> 1) & 3), i.e. floats k0 .. k0 + 3; in a 32-byte swizzled bf16 tile
+            // they are 8 bytes of row `row`, 16-byte chunk (k0 / 8) ^ ((row >> 2) & 1)
+            const int row = j >> 2, k0 = 4 * ((j & 3) ^ ((row >> 1) & 3));
+            const int ob = row * 32 + (((k0 >> 3) ^ ((row >> 2) & 1)) << 4) + ((k0 & 7) << 1);
+            uint8_t* tb = base_ptr + stage * T2_STAGE_BYTES + T2_A_BYTES;
+            *reinterpret_cast<uint2*>(tb + ob) = make_uint2(pack_bf16(h.x, h.y), pack_bf16(h.z, h.w));
+            *reinterpret_cast<uint2*>(tb + T2_A_BYTES / 2 + ob) =
+                make_uint2(pack_bf16(v.x - h.x, v.y - h.y), pack_bf16(v.z - h.z, v.w - h.w));
+          } else {
+            l.x = tf32_hi(v.x - h.x); l.y = tf32_hi(v.y - h.y); l.z = tf32_hi(v.z - h.z); l.w = tf32_hi(v.w - h.w);
+            lo[j] = l;
+          }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes -> tensor core reads
         asm volatile("bar.sync 2, 128;" ::: "memory");
@@ -331,23 +389,48 @@ bool tred_mac_tc2_supported(const tred_ctx* ctx) {
          ctx->cfg.resp_half <= RT_MAXH && ctx->num_sms >= 2 && get_encode_fn2() != nullptr;
 }
 
-// Same contract as tred_mac_tc_fused (tred_mac_tc.cu), on CTA pairs.
-int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, float* opart,
-                 int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st) {
+// [nslot][rows][k2] bf16, K contiguous; box = 16 elements (32 bytes) x box_rows rows, 32-byte swizzle
+static bool make_map2_bf16(PFN_encodeTiled2 enc, CUtensorMap* tm, const void* base, int k2, int64_t rows, int nslot,
+                           int box_rows) {
+  const cuuint64_t dims[3] = {(cuuint64_t)k2, (cuuint64_t)rows, (cuuint64_t)nslot};
+  const cuuint64_t strides[2] = {(cuuint64_t)k2 * 2, (cuuint64_t)k2 * 2 * (cuuint64_t)rows};
+  const cuuint32_t box[3] = {(cuuint32_t)T2_KC, (cuuint32_t)box_rows, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, (void*)base, dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Same contract as tred_mac_tc_fused (tred_mac_tc.cu), on CTA pairs.  Bhb / Blb: the bf16
+// copies of B_hi / B_lo; non-NULL selects the variant whose two correction products are bf16.
+int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, const void* Bhb,
+                 const void* Blb, float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2,
+                 cudaStream_t st) {
   const tred_dims& d = ctx->dims;
   const int N = 2 * d.n_off_pad, K2 = 2 * d.n_phase;
+  const bool bf = Bhb && Blb;
   if (ntile < 1 || !tred_mac_tc2_supported(ctx)) return TRED_EUNSUPPORTED;
-  if ((((uintptr_t)qhat) | ((uintptr_t)Bhi) | ((uintptr_t)Blo)) & 15) return TRED_EUNSUPPORTED;
+  if ((((uintptr_t)qhat) | ((uintptr_t)Bhi) | ((uintptr_t)Blo) | ((uintptr_t)Bhb) | ((uintptr_t)Blb)) & 15)
+    return TRED_EUNSUPPORTED;
   PFN_encodeTiled2 enc = get_encode_fn2();
   const int rp = ntile * T2_M;
-  CUtensorMap tmA, tmBh, tmBl;
-  if (!make_map2(enc, &tmA, qhat, K2, rp, d.n_freq, T2_M) || !make_map2(enc, &tmBh, Bhi, K2, N, d.n_freq, N / 2) ||
-      !make_map2(enc, &tmBl, Blo, K2, N, d.n_freq, N / 2))
+  T2Maps tm;
+  if (!make_map2(enc, &tm.a, qhat, K2, rp, d.n_freq, T2_M) || !make_map2(enc, &tm.bh, Bhi, K2, N, d.n_freq, N / 2))
     return TRED_EUNSUPPORTED;
+  if (bf) {
+    if (!make_map2_bf16(enc, &tm.bl, Bhb, K2, N, d.n_freq, N / 2) ||
+        !make_map2_bf16(enc, &tm.bl2, Blb, K2, N, d.n_freq, N / 2))
+      return TRED_EUNSUPPORTED;
+  } else {
+    if (!make_map2(enc, &tm.bl, Blo, K2, N, d.n_freq, N / 2)) return TRED_EUNSUPPORTED;
+    tm.bl2 = tm.bl;
+  }
   static bool attr_set = false;
   if (!attr_set) {
-    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
-    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<11, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
+    TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<11, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
     attr_set = true;
   }
   T2Params p;
@@ -359,10 +442,13 @@ int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float
   int64_t ncl = ctx->num_sms / 2;
   if (ncl > items) ncl = items;
   const int grid = (int)(2 * ncl);
-  if (p.K == 11)
-    k_mac_tc2<11><<<grid, T2_THREADS, T2_SMEM, st>>>(tmA, tmBh, tmBl, p);
-  else
-    k_mac_tc2<0><<<grid, T2_THREADS, T2_SMEM, st>>>(tmA, tmBh, tmBl, p);
+  if (p.K == 11) {
+    if (bf) k_mac_tc2<11, true><<<grid, T2_THREADS, T2_SMEM, st>>>(tm, p);
+    else k_mac_tc2<11, false><<<grid, T2_THREADS, T2_SMEM, st>>>(tm, p);
+  } else {
+    if (bf) k_mac_tc2<0, true><<<grid, T2_THREADS, T2_SMEM, st>>>(tm, p);
+    else k_mac_tc2<0, false><<<grid, T2_THREADS, T2_SMEM, st>>>(tm, p);
+  }
   TRED_LAUNCH_CHECK("k_mac_tc2");
   return TRED_OK;
 }

@@ -55,7 +55,7 @@ def test_dims_host_logic(cfg_id, L, nover, ppb):
     assert list(d.NB) == [-(-d.NG[a] // cfg.block[a]) for a in range(3)]
     assert (d.n_phase, d.n_off, d.n_off_pad) == (100, 121, 128)
     # fp32 spectrum + tf32 hi/lo matrices + the four mirror-symmetric half matrices + flag
-    assert d.rhat_floats == 10 * (L // 2) * 100 * 128 + 4 * (L // 2) * 128 * 100 + 8
+    assert d.rhat_floats == 14 * (L // 2) * 100 * 128 + 4 * (L // 2) * 128 * 100 + 8
     assert d.conv_row_bytes == (L // 2) * (100 + 128) * 8
 
 
