@@ -219,11 +219,12 @@ int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
  * the time axis: real FFT along time of the S*S fine columns of every charge pixel
  * (zero where no block is occupied); per frequency, the product of the [charge pixels x
  * phases] spectra with the [phases x offsets] response spectrum (one batched complex
- * GEMM: fp32 FMA, or tensor cores with 3xTF32 split operands, see tred_config.mac_mode);
- * sum over the (2H+1)^2 offsets onto the output pixels in the frequency domain (sum
- * before the inverse FFT, Eq. (14)), in a fixed order; one inverse FFT per slab pixel.
- * Charge pixels are processed in chunks that fit the workspace; results do not depend on
- * the chunking (bit-identical).
+ * GEMM: tensor cores with split operands by default, fp32 FMA on request, see
+ * tred_config.mac_mode); sum over the (2H+1)^2 offsets onto the output pixels in the
+ * frequency domain (sum before the inverse FFT, Eq. (14)), in a fixed order -- in the default
+ * mode inside the GEMM epilogue, per row tile, so the products never reach memory; one
+ * inverse FFT per slab pixel.  Charge pixels are processed in chunks that fit the workspace;
+ * results do not depend on the chunking (bit-identical).  No unordered float atomics.
  *   h_cp_off   [NBt+1] HOST copy of tred_convolve_plan's d_cp_off
  *   h_sp_off   [NBt+1] HOST copy of d_sp_off
  *   h_rt_off   [NBt+1] HOST copy of d_rt_off
