@@ -313,18 +313,20 @@ class Tred:
                                     _ptr(work), work.numel(), self._stream()), "tred_blockbin")
         return keys, blk_off, pair_seg, slab_off, nblocks
 
-    def effq(self, nblocks: int, keys, blk_off, pair_seg, augf, augi, payload=None):
+    def effq(self, nblocks: int, keys, blk_off, pair_seg, augf, augi, payload=None, work_bytes: int | None = None):
         t = self.torch
         nseg = augf.shape[1]
         if payload is None:
             payload = self._empty((max(nblocks, 1), self.cfg.block[0], self.cfg.block[1], self.cfg.block[2]),
                                   t.float32)
-        work = None                                   # default: every CTA builds the tables of its segments
-        if os.environ.get("TRED_EFFQ_TABLES", "0") == "1":   # measured slower at config 3 (46.9 vs 39.6 ms)
-            work = self._workbuf("effq", self.L.tred_effq_work_bytes(self.h, nseg))
+        # workspace for the per-segment tables (less is allowed: same values, slower)
+        wb = self.L.tred_effq_work_bytes(self.h, nseg)
+        if work_bytes is not None:
+            wb = min(wb, int(work_bytes))
+        work = self._workbuf("effq", wb) if wb > 0 else None
         _check(self.L.tred_effq(self.h, nseg, nblocks, _ptr(keys), _ptr(blk_off), _ptr(pair_seg),
                                 _ptr(augf), _ptr(augi), _ptr(payload), _ptr(work),
-                                work.numel() if work is not None else 0, self._stream()), "tred_effq")
+                                wb if work is not None else 0, self._stream()), "tred_effq")
         return payload
 
     def convolve_plan(self, nblocks: int, keys, cap_cp: int | None = None, cap_sp: int | None = None,
@@ -474,7 +476,8 @@ class Tred:
         return out[:ngroups]
 
     # -- whole path in bounded-memory chunks of occupied blocks (BASELINE config 4) --------
-    def simulate_chunked(self, seg, rhat, pix_ids=None, payload_budget_bytes: int = 8 << 30):
+    def simulate_chunked(self, seg, rhat, pix_ids=None, payload_budget_bytes: int = 8 << 30,
+                         effq_work_bytes: int = 1 << 30):
         """Same result as `simulate`, bit for bit, with the block payload, the convolution
         workspace and the slab outputs held for one range of time slabs at a time
         (chunks bounded by device memory).  The occupied blocks are
@@ -517,7 +520,7 @@ class Tred:
                 payload = None
                 payload = self._empty((nb, self.cfg.block[0], self.cfg.block[1], Bt), t.float32)
             kc = keys[k0:k1]
-            self.effq(nb, kc, blk_off[k0:k1 + 1], pair_seg, augf, augi, payload=payload)
+            self.effq(nb, kc, blk_off[k0:k1 + 1], pair_seg, augf, augi, payload=payload, work_bytes=effq_work_bytes)
             plan = self.convolve_plan(nb, kc)
             counts = t.cat([plan["ncp"], plan["nsp"], plan["cp_off"].to(t.int64), plan["sp_off"].to(t.int64),
                             plan["rt_off"].to(t.int64)]).cpu().numpy()

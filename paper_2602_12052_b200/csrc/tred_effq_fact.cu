@@ -13,18 +13,25 @@
 // Same nodes, weights, coefficients and bounding box as the closed-form kernel
 // (tred_effq.cu); only the order of summation and the evaluation of q differ.
 //
-// One CTA per block tile (all of Bx x By, TS ticks) staged in shared memory.  Per segment
-// of the block: phase A builds the three tables (double-buffered), one __syncthreads,
-// phase B adds the rank-m product into the tile, one thread per (column, tick chunk).
-// No atomics; the summation order is fixed (segments ascending), so results are
-// deterministic.
+// Kernel k_effq_blk: one CTA per (block, sub-tile of TS ticks); the tile [column][tick] lives
+// in shared memory and every thread OWNS a column (and a range of its ticks) for the whole
+// CTA, so the tile needs no synchronisation between segments, no atomics, and the order of
+// the additions is fixed (segments ascending, quadrature points ascending): deterministic.
+// The segments of the block are taken 32 records at a time; their quadrature points are cut
+// into passes of <= 12 points, and EB_GP passes form a group:
+//   phase A (warp per (pass, round of 31 table rows)): the three per-axis tables of the pass,
+//            rows along the lanes, the n exponentials of a dual cell shared by the two grid
+//            points it touches through a shuffle; everything that depends on the row is a
+//            per-lane constant of the loop over the quadrature points;
+//   phase B (thread per column): rank-m update of the thread's own tile cells, four ticks
+//            per step (LDS.128 of the tile and of the broadcast t-table rows).
+// Two __syncthreads per group.
 #include <math.h>
 #include "tred_common.cuh"
 
 namespace {
 
-constexpr int MMAX = 24;            // quadrature points per pass
-constexpr int MP = MMAX + 4;        // table row pitch (floats): conflict-free LDS.128
+constexpr int MMAX = 24;            // quadrature points of the largest rule
 constexpr int NGL = MMAX * (MMAX + 1) / 2;
 
 __constant__ float c_gl_s[NGL];     // nodes mapped to [0,1], rule m at offset m(m-1)/2
@@ -58,35 +65,8 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
-struct FactParams {
-  int TS;        // ticks per CTA tile
-  int nsub;      // Bt / TS
-  int plane;     // Bx*By + 1
-};
-
-// One table entry: grid point gi of one axis, quadrature centre c (grid units relative to
-// lo), k2 = log2(e) / (2 sigma^2).
-// Contributions of the n nodes of dual cell gi (between grid points gi and gi + 1) to the
-// table entries of gi (coefficient 1 - s) and of gi + 1 (coefficient s): the same n
-// exponentials serve both, so a row of entries costs n, not 2n, exponentials per entry
-// (entry(gi) = own(gi) + up(gi - 1)); same arithmetic per term as axis_entry.
-template <int N>
-__device__ __forceinline__ void axis_cell(int gi, int lo, int hi, float c, float k2, float& own, float& up) {
-  own = 0.0f; up = 0.0f;
-  const float base = (float)(gi - lo) + 0.5f;
-#pragma unroll
-  for (int q = 0; q < N; ++q) {
-    const float sq = DualGL<N>::s(q), wq = DualGL<N>::w(q);
-    const int cub = gi + DualGL<N>::side(q);
-    const float z = (base + sq) - c;
-    const float e = ex2_approx(-z * z * k2);
-    if (cub >= lo && cub <= hi) {
-      own = fmaf(wq * (1.0f - sq), e, own);
-      if (sq != 0.0f) up = fmaf(wq * sq, e, up);
-    }
-  }
-}
-
+// One table entry (used by the truth record below): grid point gi of one axis, quadrature
+// centre c (grid units relative to lo), k2 = log2(e) / (2 sigma^2).
 template <int N>
 __device__ __forceinline__ float axis_entry(int gi, int lo, int hi, float c, float k2) {
   float v = 0.0f;
@@ -110,154 +90,253 @@ __device__ __forceinline__ float axis_entry(int gi, int lo, int hi, float c, flo
   return v;
 }
 
-// ------------------------------------------------------------------ tables built once
-// A segment meets ~4 blocks x 2 tick sub-tiles, and every such CTA would rebuild the same
-// three per-axis tables (8 ex2 per entry for n = 4): ncu showed the tile kernel issue-bound
-// on exactly that.  So the tables of the segments a range of blocks refers to are built once
-// (k_effq_tables) into a slot of TAB_ROWS x TAB_M floats and the tile kernel copies the rows
-// it needs.  Segments that do not fit a slot (more than TAB_M quadrature points, several
-// pieces, a bounding box of more than TAB_ROWS grid rows in total, or no free slot) are
-// evaluated in the tile kernel as before.
-constexpr int TAB_M = 12;
-constexpr int TAB_ROWS = 96;
-constexpr int TAB_FLOATS = TAB_ROWS * TAB_M;
-constexpr int64_t EFFQ_MAX_SLOTS = 1 << 18;          // 262144 slots = 1.2 GB of tables at most
-constexpr int EFFQ_RANGE_BLOCKS = 8192;              // blocks per pass of (mark, tables, tiles)
-
-// Quadrature of a segment record: number of pieces and points per piece from its length
-// in sigmas (same arithmetic wherever it is needed).
+// Quadrature of a segment record: number of pieces and points per piece from its length W
+// in sigmas (same arithmetic wherever it is needed).  The m-point Gauss-Legendre rule of
+// int_0^1 N(x - s W) ds has a relative error (of the maximum over x) below 1.5e-7 for
+// W <= 1.13, 1.83, 2.58, 3.35, 4.11 (m = 4..8) and then ~0.75 more per extra point up to
+// 16.1 at m = 24 (computed against the erf closed form); the thresholds below are 0.95 of that.
 struct SegQuad { int npiece, m; };
 __device__ __forceinline__ SegQuad seg_quad(int flag, float dx, float dy, float dt, float sx, float sy, float st) {
   SegQuad q;
   q.npiece = 1; q.m = 4;
   if (!flag) {
     const float W = sqrtf((dx / sx) * (dx / sx) + (dy / sy) * (dy / sy) + (dt / st) * (dt / st));
-    q.npiece = (int)ceilf(W * (1.0f / 15.5f));
+    q.npiece = (int)ceilf(W * (1.0f / 15.3f));
     if (q.npiece < 1) q.npiece = 1;
     const float Wp = W / (float)q.npiece;
-    q.m = Wp <= 1.0f ? 4 : Wp <= 3.9f ? 8 : Wp <= 6.9f ? 12 : Wp <= 9.9f ? 16 : Wp <= 12.8f ? 20 : 24;
+    if (Wp <= 3.18f) q.m = Wp <= 1.07f ? 4 : Wp <= 1.74f ? 5 : Wp <= 2.45f ? 6 : 7;
+    else {
+      q.m = 8 + (int)ceilf((Wp - 3.9f) * (1.0f / 0.7125f));
+      q.m = q.m < 8 ? 8 : q.m > MMAX ? MMAX : q.m;
+    }
   }
   return q;
 }
 
-// marks the segments the blocks [k0, k0 + nb) refer to (idempotent plain stores)
+// ------------------------------------------------------------------ table rows
+// Entries of the per-axis tables for the dual cells one lane each (lane = cell gi between
+// grid points gi and gi + 1, of the axis with bbox [lo_a, hi_a], segment end p0a, extent da,
+// nk2 = -log2(e)/(2 sigma^2)), for the quadrature points [g0, g0 + cnt) of the segment: the n
+// exponentials of a cell serve the entry of gi (coefficient 1 - s) and, through a shuffle, the
+// entry of gi + 1 (coefficient s) held by the next lane, so lane 0 and the first cell of an axis
+// only provide.  Kx = K for the x axis (K W_k is folded into the x table), 1 otherwise.
+struct QuadRule { int m, flag, goff; float inv_np; };
+
+template <int N>
+__device__ __forceinline__ void effq_cells(int gi, int lo_a, int hi_a, float p0a, float da, float nk2, float Kx,
+                                           bool scale_w, bool wr, bool zero, float* __restrict__ dst, int stride,
+                                           const QuadRule& qr, int g0, int cnt) {
+  const float base = (float)(gi - lo_a) + 0.5f;
+  float wo[N], wu[N];
+#pragma unroll
+  for (int q = 0; q < N; ++q) {
+    const int cub = gi + DualGL<N>::side(q);
+    const bool ok = cub >= lo_a && cub <= hi_a;
+    wo[q] = ok ? DualGL<N>::w(q) * (1.0f - DualGL<N>::s(q)) : 0.0f;
+    wu[q] = ok ? DualGL<N>::w(q) * DualGL<N>::s(q) : 0.0f;
+  }
+  int pc = g0 / qr.m, mi = g0 - pc * qr.m;
+  for (int pt = 0; pt < cnt; ++pt, dst += stride) {
+    float sk, wk;
+    if (qr.flag) { sk = 0.5f; wk = (g0 + pt) == 0 ? 1.0f : 0.0f; }      // point-like: midpoint Gaussian
+    else { sk = ((float)pc + c_gl_s[qr.goff + mi]) * qr.inv_np; wk = c_gl_w[qr.goff + mi] * qr.inv_np; }
+    const float zb = base - fmaf(sk, da, p0a);
+    float own = 0.0f, up = 0.0f;
+#pragma unroll
+    for (int q = 0; q < N; ++q) {
+      const float z = zb + DualGL<N>::s(q);
+      const float e = ex2_approx(z * z * nk2);
+      own = fmaf(wo[q], e, own);
+      if (DualGL<N>::s(q) != 0.0f) up = fmaf(wu[q], e, up);
+    }
+    const float below = __shfl_up_sync(0xffffffffu, up, 1);
+    float val = N > 1 ? own + below : own;
+    if (scale_w) val *= Kx * wk;
+    if (zero) val = 0.0f;
+    if (wr) *dst = val;
+    if (++mi == qr.m) { mi = 0; ++pc; }
+  }
+}
+
+// ------------------------------------------------------------------ tables built once per segment
+// A segment meets ~4 blocks x 1.5 tick tiles, and every such CTA needs the same three per-axis
+// tables.  With a workspace, tred_effq builds them once per segment (k_effq_tables, one warp per
+// segment, whole bounding box) and the tile CTAs copy the rows they need with cp.async; without
+// one (or for segments whose tables do not fit it) the tile CTAs compute the rows themselves with
+// the same code (effq_cells): same values either way.
+// Table of segment s at tab + 4 * off[s] floats: [point][rs], rs = align4(nxf + nyf) + ntfp;
+// x rows (grid points lox-E .. hix+E), y rows, then the t rows from the 4-aligned tick tb =
+// align_down(lot - E, 4), ntfp = align_up(hit + E + 1 - tb, 4) of them.  Entries of grid points
+// outside the grid are zero (clip and drop, reading G13).
+struct TabGeom { int nxf, nyf, tb, ntfp, toff, rs; };
+__device__ __forceinline__ TabGeom tab_geom(int lox, int loy, int lot, int hix, int hiy, int hit, int E) {
+  TabGeom t;
+  t.nxf = hix - lox + 1 + 2 * E;
+  t.nyf = hiy - loy + 1 + 2 * E;
+  t.tb = (lot - E) & ~3;
+  t.ntfp = ((hit + E + 1 - t.tb) + 3) & ~3;
+  t.toff = (t.nxf + t.nyf + 3) & ~3;
+  t.rs = t.toff + t.ntfp;
+  return t;
+}
+
+// marks the segments the blocks [0, nb) of this call refer to (idempotent plain stores)
 __global__ void __launch_bounds__(256)
-k_effq_mark(int nb, int k0, const int32_t* __restrict__ blk_off, const int32_t* __restrict__ pair_seg,
+k_effq_mark(int64_t nb, const int32_t* __restrict__ blk_off, const int32_t* __restrict__ pair_seg,
             int32_t* __restrict__ mark) {
-  const int warp = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
   if (warp >= nb) return;
-  const int p0 = blk_off[k0 + warp], p1 = blk_off[k0 + warp + 1];
+  const int p0 = blk_off[warp], p1 = blk_off[warp + 1];
   for (int p = p0 + lane; p < p1; p += 32) mark[pair_seg[p]] = 1;
 }
 
-// slot[] = exclusive scan of the marks; lists the marked segments and resets tabslot
+// mark[s] = size of the table of a marked segment in 16-byte units (0 if not marked)
+template <int N>
 __global__ void __launch_bounds__(256)
-k_effq_list(int64_t nseg, const int32_t* __restrict__ slot, int32_t* __restrict__ seglist, int cap,
-            int32_t* __restrict__ tabslot) {
+k_effq_sizes(int64_t nseg, const float* __restrict__ augf, const int32_t* __restrict__ augi,
+             int32_t* __restrict__ mark) {
   const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= nseg) return;
-  const int sl = slot[s];
-  const bool marked = slot[s + 1] != sl;
-  if (marked && sl < cap) seglist[sl] = (int32_t)s;
-  tabslot[s] = -1;
+  if (s > nseg) return;
+  int v = 0;
+  if (s < nseg && mark[s]) {
+    constexpr int E = N > 1 ? 1 : 0;
+    const TabGeom t = tab_geom(augi[0 * nseg + s], augi[1 * nseg + s], augi[2 * nseg + s], augi[3 * nseg + s],
+                               augi[4 * nseg + s], augi[5 * nseg + s], E);
+    const float p0x = augf[0 * nseg + s], p0y = augf[1 * nseg + s], p0t = augf[2 * nseg + s];
+    const SegQuad q = seg_quad(augi[6 * nseg + s], augf[3 * nseg + s] - p0x, augf[4 * nseg + s] - p0y,
+                               augf[5 * nseg + s] - p0t, augf[6 * nseg + s], augf[7 * nseg + s], augf[8 * nseg + s]);
+    const int64_t sz = (int64_t)q.npiece * q.m * (t.rs >> 2);
+    v = sz < (1 << 24) ? (int)sz : (1 << 24);           // absurdly large boxes: no table (never fits)
+  }
+  mark[s] = v;
 }
 
-// One warp per listed segment: the three tables of its bounding box (grid points
-// lo - E .. hi + E per axis), rows of TAB_M floats, X rows first (with K W_k folded in),
-// then Y, then T.
+// one warp per 32 consecutive segments; the marked ones among them one after the other
 template <int N>
 __global__ void __launch_bounds__(128)
-k_effq_tables(int64_t nseg, const int32_t* __restrict__ slot, const int32_t* __restrict__ seglist, int cap,
-              const float* __restrict__ augf, const int32_t* __restrict__ augi, float* __restrict__ tab,
-              int32_t* __restrict__ tabslot) {
-  const int sl = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  const int total = min(slot[nseg], cap);
-  if (sl >= total) return;
-  const int64_t s = seglist[sl];
+k_effq_tables(int64_t nseg, const int32_t* __restrict__ off, int64_t cap16, const float* __restrict__ augf,
+              const int32_t* __restrict__ augi, float* __restrict__ tab, TredGrid g) {
+  const int64_t w = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  const int64_t s_l = w * 32 + lane;
+  bool mine = false;
+  if (s_l < nseg) { const int o0 = off[s_l], o1 = off[s_l + 1]; mine = o1 > o0 && (int64_t)o1 <= cap16; }
+  uint32_t todo = __ballot_sync(0xffffffffu, mine);
   constexpr int E = N > 1 ? 1 : 0;
   constexpr float LOG2E_HALF = 0.72134752044448170f;
-  const int lox = augi[0 * nseg + s], loy = augi[1 * nseg + s], lot = augi[2 * nseg + s];
-  const int hix = augi[3 * nseg + s], hiy = augi[4 * nseg + s], hit = augi[5 * nseg + s];
-  const int flag = augi[6 * nseg + s];
-  const float p0x = augf[0 * nseg + s], p0y = augf[1 * nseg + s], p0t = augf[2 * nseg + s];
-  const float p1x = augf[3 * nseg + s], p1y = augf[4 * nseg + s], p1t = augf[5 * nseg + s];
-  const float sx = augf[6 * nseg + s], sy = augf[7 * nseg + s], st = augf[8 * nseg + s];
-  const float Qp = augf[9 * nseg + s];
-  const float dx = p1x - p0x, dy = p1y - p0y, dt = p1t - p0t;
-  const SegQuad q = seg_quad(flag, dx, dy, dt, sx, sy, st);
-  const int nxf = hix - lox + 1 + 2 * E, nyf = hiy - loy + 1 + 2 * E, ntf = hit - lot + 1 + 2 * E;
-  if (q.npiece != 1 || q.m > TAB_M || nxf + nyf + ntf > TAB_ROWS) return;      // tile kernel evaluates it
-  const float k2x = LOG2E_HALF / (sx * sx), k2y = LOG2E_HALF / (sy * sy), k2t = LOG2E_HALF / (st * st);
-  const float K = Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f;
-  const int m = q.m, goff = m * (m - 1) / 2;
-  float* T = tab + (int64_t)sl * TAB_FLOATS;
-  const int nent = (nxf + nyf + ntf) * TAB_M;
-  for (int e = lane; e < nent; e += 32) {
-    const int r = e / TAB_M, mi = e - r * TAB_M;
-    float v = 0.0f;
-    if (mi < m) {
-      float sk, wk;
-      if (flag) { sk = 0.5f; wk = mi == 0 ? 1.0f : 0.0f; }
-      else { sk = c_gl_s[goff + mi]; wk = c_gl_w[goff + mi]; }
-      if (r < nxf) v = axis_entry<N>(lox - E + r, lox, hix, fmaf(sk, dx, p0x), k2x) * (K * wk);
-      else if (r < nxf + nyf) v = axis_entry<N>(loy - E + (r - nxf), loy, hiy, fmaf(sk, dy, p0y), k2y);
-      else v = axis_entry<N>(lot - E + (r - nxf - nyf), lot, hit, fmaf(sk, dt, p0t), k2t);
+  while (todo) {
+    const int b = __ffs(todo) - 1;
+    todo &= todo - 1;
+    const int64_t s = w * 32 + b;
+    const int lo[3] = {augi[0 * nseg + s], augi[1 * nseg + s], augi[2 * nseg + s]};
+    const int hi[3] = {augi[3 * nseg + s], augi[4 * nseg + s], augi[5 * nseg + s]};
+    const float p0[3] = {augf[0 * nseg + s], augf[1 * nseg + s], augf[2 * nseg + s]};
+    const float d3[3] = {augf[3 * nseg + s] - p0[0], augf[4 * nseg + s] - p0[1], augf[5 * nseg + s] - p0[2]};
+    const float sg[3] = {augf[6 * nseg + s], augf[7 * nseg + s], augf[8 * nseg + s]};
+    const float K = augf[9 * nseg + s] * 0.063493635934240969f / (sg[0] * sg[1] * sg[2]) * 0.125f;
+    const int flag = augi[6 * nseg + s];
+    const SegQuad q = seg_quad(flag, d3[0], d3[1], d3[2], sg[0], sg[1], sg[2]);
+    const QuadRule qr{q.m, flag, q.m * (q.m - 1) / 2, 1.0f / (float)q.npiece};
+    const int ptot = q.npiece * q.m;
+    const TabGeom t = tab_geom(lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], E);
+    float* T = tab + 4 * (int64_t)off[s];
+    // cells: one leading cell per axis, then one per row
+    const int ncell = t.nxf + t.nyf + t.ntfp + 3;
+    for (int r0 = 0; r0 < ncell - 1; r0 += 31) {
+      const int p = r0 + lane;
+      int a, q0, first, rowb, NGa;
+      if (p < t.nxf + 1) { a = 0; q0 = p; first = lo[0] - E; rowb = 0; NGa = g.NGx; }
+      else if (p < t.nxf + t.nyf + 2) { a = 1; q0 = p - (t.nxf + 1); first = lo[1] - E; rowb = t.nxf; NGa = g.NGy; }
+      else { a = 2; q0 = p - (t.nxf + t.nyf + 2); first = t.tb; rowb = t.toff; NGa = g.NGt; }
+      const int gi = first - 1 + q0;
+      const bool wr = lane >= 1 && q0 >= 1 && p < ncell;
+      effq_cells<N>(gi, lo[a], hi[a], p0[a], d3[a], -LOG2E_HALF / (sg[a] * sg[a]), K, a == 0, wr,
+                    gi < 0 || gi >= NGa, T + rowb + q0 - 1, t.rs, qr, 0, ptot);
     }
-    T[e] = v;
+    // the padding between the y rows and the t rows is never read
   }
-  if (lane == 0) tabslot[s] = sl;
 }
 
-// Phase B of one (segment, piece): tile[k][i][j] += sum_mi GX[i][mi] GY[j][mi] GT[k][mi] over
-// the clipped footprint.  A thread owns one column (and one tick chunk of it); the products
-// GX GY of its column stay in registers (MQ = m / 4 float4), every tile value is read and
-// written once per piece.
-template <int MQ>
-__device__ __forceinline__ void effq_phase_b(float* __restrict__ tp, int plane, const float* __restrict__ GXr,
-                                             const float* __restrict__ GYr, const float* __restrict__ GT,
-                                             int ka, int kb) {
-  float4 ab[MQ];
+// ------------------------------------------------------------------ the tile kernel
+constexpr int EB_SB = 32;           // segment records staged per batch
+constexpr int EB_MQ = 12;           // quadrature points per pass (table columns)
+constexpr int EB_GP = 8;            // passes per group = table sets in shared memory
+constexpr int EB_NREC = 36;         // int32 words per staged record
+// staged record (after the batch prologue):
+//   0..5 lo, hi (x, y, t)   6 flag   7 m (points per piece)
+//   8..10 p0 (x, y, t)      11 K = Q' (2 pi)^-3/2 / (sx sy st) / 8
+//   12..14 d = p1 - p0      15 1 / npiece
+//   16..18 -log2(e)/(2 sigma^2) (x, y, t)     19 offset of rule m in c_gl_s / c_gl_w
+//   20..23 clipped footprint in the tile: x first, nx, y first, ny          (tile-relative)
+//   24..27 t first, t last (tile-relative), first / count of the 4-aligned tick range
+//   28 quadrature points in total (npiece m)   29 passes
+//   30 offset of the segment's table in 16-byte units (-1: none)   31 its row stride
+//   32 x row, 33 y row, 34 t row of the table that holds the first x / y / aligned t entry of the tile
+enum { ER_M = 7, ER_P0 = 8, ER_K = 11, ER_D = 12, ER_INVNP = 15, ER_NK2 = 16, ER_GOFF = 19, ER_FX = 20, ER_FT = 24,
+       ER_PTOT = 28, ER_NPASS = 29, ER_TOFF = 30, ER_TRS = 31, ER_TROW = 32 };
+
+struct BlkParams {
+  int TS, nsub;      // ticks per CTA tile, tiles per block
+  int ncol;          // Bx * By columns
+  int by_shift;      // log2(By)
+  int ts_shift;      // log2(TS)
+  int CS;            // column stride of the tile in floats (TS + 4: conflict-free LDS.128)
+  int RS;            // rows of one table set = Bx + By + TS
+  // what a warp owns for the whole CTA: wi rows x wj columns-in-a-row (wi * wj = 32 or 16) x wt ticks
+  int wi, wj, wt;
+  int nwj, nwi;      // warps along j, along i (warp -> (tick range, i range, j range))
+  int64_t cap16;     // 16-byte units of table workspace (0: no tables)
+};
+
+__device__ __forceinline__ void cp_async4(float* dst, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async16(float* dst, const float* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src)
+               : "memory");
+}
+
+// Phase B of one pass for one lane: tile[col][k] += sum_pt GX[pt][i] GY[pt][j] GT[pt][k] for the
+// tick quads k = k0, k0 + kstep, ... < k1 of column col.
+template <int CNT>
+__device__ __forceinline__ void effq_blk_update(float* __restrict__ tcol, const float* __restrict__ T, int RS,
+                                                int xrow, int yrow, int trow0, int k0, int k1, int kstep) {
+  float ab[CNT];
 #pragma unroll
-  for (int q = 0; q < MQ; ++q) {
-    const float4 a = *reinterpret_cast<const float4*>(GXr + 4 * q);
-    const float4 b = *reinterpret_cast<const float4*>(GYr + 4 * q);
-    ab[q] = make_float4(a.x * b.x, a.y * b.y, a.z * b.z, a.w * b.w);
-  }
+  for (int pt = 0; pt < CNT; ++pt) ab[pt] = T[pt * RS + xrow] * T[pt * RS + yrow];
+  const int rs4 = RS >> 2;
 #pragma unroll 2
-  for (int k = ka; k < kb; ++k) {
-    float v = tp[k * plane];
+  for (int k = k0; k < k1; k += kstep) {
+    float4* tp = reinterpret_cast<float4*>(tcol + k);
+    const float4* gt = reinterpret_cast<const float4*>(T + trow0 + k);
+    float4 v = *tp;
 #pragma unroll
-    for (int q = 0; q < MQ; ++q) {
-      const float4 c = *reinterpret_cast<const float4*>(GT + k * MP + 4 * q);
-      v = fmaf(ab[q].x, c.x, v); v = fmaf(ab[q].y, c.y, v);
-      v = fmaf(ab[q].z, c.z, v); v = fmaf(ab[q].w, c.w, v);
+    for (int pt = 0; pt < CNT; ++pt) {
+      const float4 gq = gt[pt * rs4];
+      v.x = fmaf(ab[pt], gq.x, v.x); v.y = fmaf(ab[pt], gq.y, v.y);
+      v.z = fmaf(ab[pt], gq.z, v.z); v.w = fmaf(ab[pt], gq.w, v.w);
     }
-    tp[k * plane] = v;
+    *tp = v;
   }
 }
 
-#ifndef TRED_EFFQ_MINB
-#define TRED_EFFQ_MINB 4            // resident CTAs per SM the register allocation aims at
-#endif
-#ifndef TRED_EFFQ_TILE_KB
-#define TRED_EFFQ_TILE_KB 64        // largest tile (floats x 4) a CTA stages
-#endif
-
-#ifndef TRED_EFFQ_THREADS
-#define TRED_EFFQ_THREADS 256       // largest CTA
-#endif
-
-template <int N>
-__global__ void __launch_bounds__(TRED_EFFQ_THREADS, TRED_EFFQ_MINB)
-k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict__ blk_off,
-            const int32_t* __restrict__ pair_seg, const float* __restrict__ augf,
-            const int32_t* __restrict__ augi, const int32_t* __restrict__ tabslot,
-            const float* __restrict__ tab, float* __restrict__ payload, TredGrid g, FactParams P) {
-  extern __shared__ float smf[];
-  float* tile = smf;                                   // [TS][plane]
-  const int tabn = (g.Bx + g.By + P.TS) * MP;          // floats of one table set
-  float* tabs = smf + (((size_t)P.TS * P.plane + 3) & ~(size_t)3);   // 2 sets, 16-byte aligned
+template <int N, int MAXT>
+__global__ void __launch_bounds__(MAXT, MAXT >= 1024 ? 1 : 2)
+k_effq_blk(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict__ blk_off,
+           const int32_t* __restrict__ pair_seg, const float* __restrict__ augf,
+           const int32_t* __restrict__ augi, const int32_t* __restrict__ tabofs, const float* __restrict__ gtab,
+           float* __restrict__ payload, TredGrid g, BlkParams P) {
+  extern __shared__ __align__(16) float smf[];
+  float* tile = smf;                                          // [ncol][CS]
+  float* tab = smf + (size_t)P.ncol * P.CS;                   // [EB_GP][EB_MQ][RS]
+  int32_t (*s_rec)[EB_NREC] = reinterpret_cast<int32_t (*)[EB_NREC]>(tab + (size_t)EB_GP * EB_MQ * P.RS);
+  __shared__ int s_list[EB_SB];
+  __shared__ int s_pfx[EB_SB + 1];
+  __shared__ int s_cnt;
   const int NT = blockDim.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = NT >> 5;
   const int blk = blockIdx.x / P.nsub;
   const int sub = blockIdx.x - blk * P.nsub;
   const int64_t key = keys[blk];
@@ -266,187 +345,204 @@ k_effq_fact(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __res
   const int bt = (int)(key / ((int64_t)g.NBy * g.NBx));
   const int I0 = bx * g.Bx, J0 = by * g.By, K0 = bt * g.Bt + sub * P.TS;
   constexpr int E = N > 1 ? 1 : 0;
-  constexpr float LOG2E_HALF = 0.72134752044448170f;   // log2(e) / 2
+  constexpr float LOG2E_HALF = 0.72134752044448170f;          // log2(e) / 2
 
-  for (int i = threadIdx.x; i < P.TS * P.plane; i += NT) tile[i] = 0.0f;
-  // the first __syncthreads of the segment loop (or the one after it) orders this
+  // what this warp owns: rows [wi0, wi0 + wi) x columns-in-a-row [wj0, wj0 + wj) x ticks [wt0, wt0 + wt)
+  const int wjj = warp % P.nwj, wrest = warp / P.nwj;
+  const int wii = wrest % P.nwi, wtt = wrest / P.nwi;
+  const int wi0 = wii * P.wi, wj0 = wjj * P.wj, wt0 = wtt * P.wt;
 
-  // Segment records of the block are staged in shared memory SB at a time (one pass of
-  // coalesced loads instead of two dependent global loads per segment and thread).
-  constexpr int SB = 32, NF = 18;                      // 7 int fields (bbox, flag), 10 floats, table slot
-  constexpr int NX = 21;    // derived once per segment: k2x, k2y, k2t, K, npiece, m, clipped box, work split
-  __shared__ int32_t s_rec[SB][NF + NX + 1];
-  __shared__ int s_list[SB];
-  __shared__ int s_cnt;
+  {
+    float4* t4 = reinterpret_cast<float4*>(tile);
+    const int n4 = (P.ncol * P.CS) >> 2;
+    for (int i = threadIdx.x; i < n4; i += NT) t4[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+
   const int s_beg = blk_off[blk], s_end = blk_off[blk + 1];
-  int it = 0;
-  for (int b0 = s_beg; b0 < s_end; b0 += SB) {
-  const int nbatch = min(SB, s_end - b0);
-  __syncthreads();                                     // the previous batch's records are no longer read
-  for (int e = threadIdx.x; e < nbatch * NF; e += NT) {
-    const int j = e / NF, f = e - j * NF;
-    const int64_t s = pair_seg[b0 + j];
-    s_rec[j][f] = f < 7 ? augi[f * nseg + s]
-                : f < 17 ? __float_as_int(augf[(f - 7) * nseg + s]) : (tabslot ? tabslot[s] : -1);
-  }
-  __syncthreads();
-  // one lane per record: does the footprint meet this tile? per-segment constants once
-  if (threadIdx.x < 32) {
-    const int j = threadIdx.x;
-    bool hit_tile = false;
-    if (j < nbatch) {
-      int32_t* rec = s_rec[j];
-      hit_tile = max(rec[0] - E, I0) <= min(min(rec[3] + E, I0 + g.Bx - 1), g.NGx - 1) &&
-                 max(rec[1] - E, J0) <= min(min(rec[4] + E, J0 + g.By - 1), g.NGy - 1) &&
-                 max(rec[2] - E, K0) <= min(min(rec[5] + E, K0 + P.TS - 1), g.NGt - 1);
-      if (hit_tile) {
-        const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
-        const float dx = __int_as_float(rec[10]) - __int_as_float(rec[7]);
-        const float dy = __int_as_float(rec[11]) - __int_as_float(rec[8]);
-        const float dt = __int_as_float(rec[12]) - __int_as_float(rec[9]);
-        const SegQuad q = seg_quad(rec[6], dx, dy, dt, sx, sy, st);
-        rec[NF + 0] = __float_as_int(LOG2E_HALF / (sx * sx));
-        rec[NF + 1] = __float_as_int(LOG2E_HALF / (sy * sy));
-        rec[NF + 2] = __float_as_int(LOG2E_HALF / (st * st));
-        rec[NF + 3] = __float_as_int(__int_as_float(rec[16]) * 0.063493635934240969f / (sx * sy * st) * 0.125f);
-        rec[NF + 4] = q.npiece;
-        rec[NF + 5] = q.m;
-        // clipped footprint and the phase-B work split (ncol columns x nsplit tick chunks); item / ncolp,
-        // col / ny and entry / m by multiplication: exact for arguments < 2048 and divisors <= 1024
-        const int ix0 = max(rec[0] - E, I0), ix1 = min(min(rec[3] + E, I0 + g.Bx - 1), g.NGx - 1);
-        const int iy0 = max(rec[1] - E, J0), iy1 = min(min(rec[4] + E, J0 + g.By - 1), g.NGy - 1);
-        const int kt0 = max(rec[2] - E, K0), kt1 = min(min(rec[5] + E, K0 + P.TS - 1), g.NGt - 1);
-        const int nx = ix1 - ix0 + 1, ny = iy1 - iy0 + 1, nt = kt1 - kt0 + 1;
-        const int ncol = nx * ny, ncolp = (ncol + 31) & ~31;
-        const int nsplit = ncolp < NT ? NT / ncolp : 1;
-        rec[NF + 6] = ix0; rec[NF + 7] = nx; rec[NF + 8] = iy0; rec[NF + 9] = ny;
-        rec[NF + 10] = kt0; rec[NF + 11] = nt;
-        rec[NF + 12] = ncolp; rec[NF + 13] = nsplit; rec[NF + 14] = (nt + nsplit - 1) / nsplit;
-        rec[NF + 15] = (65536 + ncolp - 1) / ncolp; rec[NF + 16] = (65536 + ny - 1) / ny;
-        rec[NF + 17] = (65536 + q.m - 1) / q.m;
-        rec[NF + 18] = q.m * (q.m - 1) / 2;
-        rec[NF + 19] = __float_as_int(1.0f / (float)q.npiece);
-        rec[NF + 20] = (65536 + (nx + ny + nt) - 1) / (nx + ny + nt);
-      }
+  for (int b0 = s_beg; b0 < s_end; b0 += EB_SB) {
+    const int nbatch = min(EB_SB, s_end - b0);
+    __syncthreads();                                   // previous batch's records and tables are no longer read
+    // raw records: words 0..6 = bbox, flag; 7..16 = p0, p1, sigma, Q'; 17, 18 = table offsets of s, s + 1
+    for (int e = threadIdx.x; e < nbatch * 19; e += NT) {
+      const int j = e / 19, f = e - j * 19;
+      const int64_t s = pair_seg[b0 + j];
+      s_rec[j][f] = f < 7 ? augi[f * nseg + s]
+                  : f < 17 ? __float_as_int(augf[(f - 7) * nseg + s]) : (tabofs ? tabofs[s + (f - 17)] : 0);
     }
-    const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
-    if (hit_tile) s_list[__popc(bal & ((1u << j) - 1u))] = j;
-    if (j == 0) s_cnt = __popc(bal);
-  }
-  __syncthreads();
-  const int nlist = s_cnt;
-  for (int sl = 0; sl < nlist; ++sl) {
-    const int32_t* rec = s_rec[s_list[sl]];
-    const int lox = rec[0], loy = rec[1], lot = rec[2];
-    const int hix = rec[3], hiy = rec[4], hit = rec[5];
-    const int flag = rec[6];
-    const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
-    const float dx = __int_as_float(rec[10]) - p0x, dy = __int_as_float(rec[11]) - p0y,
-                dt = __int_as_float(rec[12]) - p0t;
-    const float k2x = __int_as_float(rec[NF + 0]), k2y = __int_as_float(rec[NF + 1]),
-                k2t = __int_as_float(rec[NF + 2]), K = __int_as_float(rec[NF + 3]);
-    const int npiece = rec[NF + 4], m = rec[NF + 5];
-    const int slot = rec[17];
-    // clipped footprint and work split, computed once per segment by the batch prologue
-    const int ix0 = rec[NF + 6], nx = rec[NF + 7], iy0 = rec[NF + 8], ny = rec[NF + 9];
-    const int kt0 = rec[NF + 10], nt = rec[NF + 11];
-    const int ncol = nx * ny, ncolp = rec[NF + 12], nsplit = rec[NF + 13], chunk = rec[NF + 14];
-    const int inv_ncolp = rec[NF + 15], inv_ny = rec[NF + 16], goff = rec[NF + 18];
-    const float inv_np = __int_as_float(rec[NF + 19]);
-    const int nr = nx + ny + nt, inv_nr = rec[NF + 20];
-
-    for (int pc = 0; pc < npiece; ++pc, ++it) {
-      float* GX = tabs + (it & 1) * tabn;             // [Bx][MP]
-      float* GY = GX + g.Bx * MP;                     // [By][MP]
-      float* GT = GY + g.By * MP;                     // [TS][MP]
-      // ---- phase A: tables (copied from the segment's slot if it has one)
-      const int nent = (nx + ny + nt) * m;
-      if (slot >= 0) {
-        const float* T = tab + (int64_t)slot * TAB_FLOATS;
-        const int nxf = hix - lox + 1 + 2 * E, nyf = hiy - loy + 1 + 2 * E;
-        const int rx = ix0 - (lox - E), ry = nxf + iy0 - (loy - E), rt = nxf + nyf + kt0 - (lot - E);
-        constexpr int Q = TAB_M / 4;                   // float4 per table row
-        for (int e = threadIdx.x; e < (nx + ny + nt) * Q; e += NT) {
-          const int r = e / Q, c4 = e - r * Q;
-          int src, dst;
-          if (r < nx) { src = rx + r; dst = r * MP; }
-          else if (r < nx + ny) { src = ry + (r - nx); dst = (g.Bx + (r - nx)) * MP; }
-          else { src = rt + (r - nx - ny); dst = (g.Bx + g.By + (r - nx - ny)) * MP; }
-          *reinterpret_cast<float4*>(GX + dst + 4 * c4) =
-              __ldg(reinterpret_cast<const float4*>(T + src * TAB_M) + c4);
+    __syncthreads();
+    // one lane per record: does the footprint meet this tile?  constants of the segment, once
+    if (warp == 0) {
+      const int j = lane;
+      bool hit_tile = false;
+      int npass = 0;
+      if (j < nbatch) {
+        int32_t* rec = s_rec[j];
+        const int lox = rec[0], loy = rec[1], lot = rec[2], hix = rec[3], hiy = rec[4], hit = rec[5];
+        const int ix0 = max(lox - E, I0), ix1 = min(min(hix + E, I0 + g.Bx - 1), g.NGx - 1);
+        const int iy0 = max(loy - E, J0), iy1 = min(min(hiy + E, J0 + g.By - 1), g.NGy - 1);
+        const int kt0 = max(lot - E, K0), kt1 = min(min(hit + E, K0 + P.TS - 1), g.NGt - 1);
+        hit_tile = ix0 <= ix1 && iy0 <= iy1 && kt0 <= kt1;
+        if (hit_tile) {
+          const int flag = rec[6];
+          const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
+          const float dx = __int_as_float(rec[10]) - p0x, dy = __int_as_float(rec[11]) - p0y,
+                      dt = __int_as_float(rec[12]) - p0t;
+          const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
+          const float Qp = __int_as_float(rec[16]);
+          const int o0 = rec[17], o1 = rec[18];
+          const SegQuad q = seg_quad(flag, dx, dy, dt, sx, sy, st);
+          const int ptot = q.npiece * q.m;
+          npass = (ptot + EB_MQ - 1) / EB_MQ;
+          rec[ER_M] = q.m;
+          rec[ER_P0 + 0] = __float_as_int(p0x); rec[ER_P0 + 1] = __float_as_int(p0y); rec[ER_P0 + 2] = __float_as_int(p0t);
+          rec[ER_K] = __float_as_int(Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f);
+          rec[ER_D + 0] = __float_as_int(dx); rec[ER_D + 1] = __float_as_int(dy); rec[ER_D + 2] = __float_as_int(dt);
+          rec[ER_INVNP] = __float_as_int(1.0f / (float)q.npiece);
+          rec[ER_NK2 + 0] = __float_as_int(-LOG2E_HALF / (sx * sx));
+          rec[ER_NK2 + 1] = __float_as_int(-LOG2E_HALF / (sy * sy));
+          rec[ER_NK2 + 2] = __float_as_int(-LOG2E_HALF / (st * st));
+          rec[ER_GOFF] = q.m * (q.m - 1) / 2;
+          rec[ER_FX + 0] = ix0 - I0; rec[ER_FX + 1] = ix1 - ix0 + 1;
+          rec[ER_FX + 2] = iy0 - J0; rec[ER_FX + 3] = iy1 - iy0 + 1;
+          const int a0 = (kt0 - K0) & ~3, a1 = ((kt1 - K0) | 3) + 1;
+          rec[ER_FT + 0] = kt0 - K0; rec[ER_FT + 1] = kt1 - K0; rec[ER_FT + 2] = a0; rec[ER_FT + 3] = a1 - a0;
+          rec[ER_PTOT] = ptot; rec[ER_NPASS] = npass;
+          const TabGeom t = tab_geom(lox, loy, lot, hix, hiy, hit, E);
+          const bool has = o1 > o0 && (int64_t)o1 <= P.cap16;
+          rec[ER_TOFF] = has ? o0 : -1;
+          rec[ER_TRS] = t.rs;
+          rec[ER_TROW + 0] = ix0 - (lox - E);
+          rec[ER_TROW + 1] = t.nxf + iy0 - (loy - E);
+          rec[ER_TROW + 2] = t.toff + (K0 + a0 - t.tb);
         }
-      } else
-      // entry e = (quadrature point mi, row r of the concatenated x | y | t rows), rows along the
-      // lanes: a lane evaluates the n exponentials of dual cell gi once, for its own entry and
-      // for the entry of gi + 1, which the next lane picks up by a shuffle (the first row of an
-      // axis and lane 0 evaluate the cell below themselves)
-      for (int e = threadIdx.x; e - (int)(threadIdx.x & 31) < nent; e += NT) {
-        const bool act = e < nent;
-        const int ee = act ? e : nent - 1;
-        const int mi = (ee * inv_nr) >> 16, r = ee - mi * nr;     // ee / nr
-        float sk, wk;
-        if (flag) { sk = 0.5f; wk = mi == 0 ? 1.0f : 0.0f; }      // point-like: midpoint Gaussian
-        else { sk = ((float)pc + c_gl_s[goff + mi]) * inv_np; wk = c_gl_w[goff + mi] * inv_np; }
-        int gi, lo_a, hi_a, rr; float c, k2a, scale; float* dstp;
-        if (r < nx) {
-          rr = r; gi = ix0 + rr; lo_a = lox; hi_a = hix; c = fmaf(sk, dx, p0x); k2a = k2x; scale = K * wk;
-          dstp = GX + rr * MP + mi;
-        } else if (r < nx + ny) {
-          rr = r - nx; gi = iy0 + rr; lo_a = loy; hi_a = hiy; c = fmaf(sk, dy, p0y); k2a = k2y; scale = 1.0f;
-          dstp = GY + rr * MP + mi;
-        } else {
-          rr = r - nx - ny; gi = kt0 + rr; lo_a = lot; hi_a = hit; c = fmaf(sk, dt, p0t); k2a = k2t; scale = 1.0f;
-          dstp = GT + rr * MP + mi;
+      }
+      const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
+      const int pos = __popc(bal & ((1u << j) - 1u));
+      if (hit_tile) s_list[pos] = j;
+      // exclusive prefix of the pass counts over the compacted list
+      int incl = npass;                               // 0 for records that do not hit
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      if (hit_tile) s_pfx[pos] = incl - npass;
+      if (lane == 31) { s_pfx[__popc(bal)] = incl; s_cnt = __popc(bal); }
+    }
+    __syncthreads();
+    const int nlist = s_cnt;
+    const int npass_all = s_pfx[nlist];
+    for (int gp0 = 0; gp0 < npass_all; gp0 += EB_GP) {
+      const int npg = min(EB_GP, npass_all - gp0);
+      if (gp0 > 0) __syncthreads();                    // phase B of the previous group is done with the tables
+      // record and local pass index of the first pass of the group (uniform)
+      const uint32_t bal0 = __ballot_sync(0xffffffffu, lane < nlist && s_pfx[lane] <= gp0);
+      const int l0 = 31 - __clz(bal0), lp0 = gp0 - s_pfx[l0];
+      // ---- phase A: the tables of the passes of the group
+      {
+        int l = l0, lp = lp0;
+        for (int pl = 0; pl < npg; ++pl) {
+          const int32_t* rec = s_rec[s_list[l]];
+          const int4 fx = *reinterpret_cast<const int4*>(rec + ER_FX);
+          const int4 ft = *reinterpret_cast<const int4*>(rec + ER_FT);
+          const int nx = fx.y, ny = fx.w, nta = ft.w;
+          const int g0 = lp * EB_MQ;
+          const int cnt = min(EB_MQ, rec[ER_PTOT] - g0);
+          float* Ts = tab + (size_t)(pl * EB_MQ) * P.RS;
+          const int toff = rec[ER_TOFF];
+          if (toff >= 0) {
+            // copy: warp = quadrature point, lanes = x entries, y entries, 16-byte groups of t entries
+            const int trs = rec[ER_TRS];
+            const int ne = nx + ny + (nta >> 2);
+            for (int pt = warp; pt < cnt; pt += nwarps) {
+              const float* G = gtab + 4 * (int64_t)toff + (int64_t)(g0 + pt) * trs;
+              float* D = Ts + pt * P.RS;
+              for (int e = lane; e < ne; e += 32) {
+                if (e < nx) cp_async4(D + fx.x + e, G + rec[ER_TROW + 0] + e);
+                else if (e < nx + ny) cp_async4(D + g.Bx + fx.z + (e - nx), G + rec[ER_TROW + 1] + (e - nx));
+                else cp_async16(D + g.Bx + g.By + ft.z + 4 * (e - nx - ny), G + rec[ER_TROW + 2] + 4 * (e - nx - ny));
+              }
+            }
+          } else {
+            // compute: warp = round of 31 cells (one leading cell per axis)
+            const int ncell = nx + ny + nta + 3;
+            const QuadRule qr{rec[ER_M], rec[6], rec[ER_GOFF], __int_as_float(rec[ER_INVNP])};
+            for (int r0 = 31 * warp; r0 < ncell - 1; r0 += 31 * nwarps) {
+              const int p = r0 + lane;
+              int a, q0, first, rowb;
+              if (p < nx + 1) { a = 0; q0 = p; first = I0 + fx.x; rowb = fx.x; }
+              else if (p < nx + ny + 2) { a = 1; q0 = p - (nx + 1); first = J0 + fx.z; rowb = g.Bx + fx.z; }
+              else { a = 2; q0 = p - (nx + ny + 2); first = K0 + ft.z; rowb = g.Bx + g.By + ft.z; }
+              const int gi = first - 1 + q0;           // dual cell between grid points gi and gi + 1
+              const bool wr = lane >= 1 && q0 >= 1 && p < ncell;
+              // the 4-aligned tick range may reach beyond the clipped footprint: zeros there
+              const bool zero = a == 2 && (gi < K0 + ft.x || gi > K0 + ft.y);
+              effq_cells<N>(gi, rec[a], rec[3 + a], __int_as_float(rec[ER_P0 + a]), __int_as_float(rec[ER_D + a]),
+                            __int_as_float(rec[ER_NK2 + a]), __int_as_float(rec[ER_K]), a == 0, wr, zero,
+                            Ts + rowb + q0 - 1, P.RS, qr, g0, cnt);
+            }
+          }
+          if (++lp == rec[ER_NPASS]) { lp = 0; ++l; }
         }
-        float own, up;
-        axis_cell<N>(gi, lo_a, hi_a, c, k2a, own, up);
-        float below = __shfl_up_sync(0xffffffffu, up, 1);
-        if (N > 1 && (rr == 0 || (threadIdx.x & 31) == 0)) {       // no lane holds cell gi - 1 of this axis
-          float o2;
-          axis_cell<N>(gi - 1, lo_a, hi_a, c, k2a, o2, below);
-        }
-        if (act) *dstp = (N > 1 ? own + below : own) * scale;
+        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
       }
       __syncthreads();
-      // ---- phase B: tile[k][i][j] += sum_mi GX[i][mi] GY[j][mi] GT[k][mi]
-      for (int item = threadIdx.x; item < ncolp * nsplit; item += NT) {
-        const int sp = (item * inv_ncolp) >> 16, col = item - sp * ncolp;      // item / ncolp, exact here
-        if (col >= ncol) continue;
-        const int cx = (col * inv_ny) >> 16, cy = col - cx * ny;               // col / ny
-        const int ka = sp * chunk, kb = min(ka + chunk, nt);
-        float* tp = tile + (size_t)(kt0 - K0) * P.plane + (ix0 - I0 + cx) * g.By + (iy0 - J0 + cy);
-        const float* GXr = GX + cx * MP;
-        const float* GYr = GY + cy * MP;
-        switch (m >> 2) {
-          case 1: effq_phase_b<1>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
-          case 2: effq_phase_b<2>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
-          case 3: effq_phase_b<3>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
-          case 4: effq_phase_b<4>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
-          case 5: effq_phase_b<5>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
-          default: effq_phase_b<6>(tp, P.plane, GXr, GYr, GT, ka, kb); break;
+      // ---- phase B: every warp adds the passes of the group to the cells it owns, in order;
+      // within a pass the lanes share out the columns of the footprint that fall in the warp's
+      // rectangle (and, when those are fewer than 16, its tick quads)
+      {
+        int l = l0, lp = lp0;
+        for (int pl = 0; pl < npg; ++pl) {
+          const int32_t* rec = s_rec[s_list[l]];
+          const int4 fx = *reinterpret_cast<const int4*>(rec + ER_FX);
+          const int4 ft = *reinterpret_cast<const int4*>(rec + ER_FT);
+          const int cnt = min(EB_MQ, rec[ER_PTOT] - lp * EB_MQ);
+          const int ia = max(fx.x, wi0), ib = min(fx.x + fx.y, wi0 + P.wi);
+          const int ja = max(fx.z, wj0), jb = min(fx.z + fx.w, wj0 + P.wj);
+          const int ka = max(ft.z, wt0), kb = min(ft.z + ft.w, wt0 + P.wt);
+          if (ia < ib && ja < jb && ka < kb) {
+            const int nj = jb - ja, nc = (ib - ia) * nj;
+            const int G = 32 / nc;                                   // lane groups: tick quads are dealt round-robin
+            const int grp = (int)(((float)lane + 0.5f) * __frcp_rn((float)nc));
+            const int c = lane - grp * nc;
+            const int ii = (int)(((float)c + 0.5f) * __frcp_rn((float)nj));
+            const int jj = c - ii * nj;
+            if (grp < G) {
+              const int ci = ia + ii, cj = ja + jj;
+              float* tcol = tile + (size_t)((ci << P.by_shift) + cj) * P.CS;
+              const float* T = tab + (size_t)(pl * EB_MQ) * P.RS;
+              const int trow0 = g.Bx + g.By, k0 = ka + 4 * grp, ks = 4 * G;
+              switch (cnt) {
+                case 1: effq_blk_update<1>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 2: effq_blk_update<2>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 3: effq_blk_update<3>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 4: effq_blk_update<4>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 5: effq_blk_update<5>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 6: effq_blk_update<6>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 7: effq_blk_update<7>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 8: effq_blk_update<8>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 9: effq_blk_update<9>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 10: effq_blk_update<10>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                case 11: effq_blk_update<11>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+                default: effq_blk_update<12>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
+              }
+            }
+            __syncwarp();                              // the next pass deals the cells to other lanes
+          }
+          if (++lp == rec[ER_NPASS]) { lp = 0; ++l; }
         }
       }
-      // no barrier here: the next phase A writes the other table set, and its barrier
-      // orders this phase B before the next one
     }
-  }
   }
   __syncthreads();
-  // tile -> payload[blk][i][j][k], k contiguous: a thread writes 4 consecutive ticks
-  float* out = payload + (int64_t)blk * g.Bx * g.By * g.Bt + sub * P.TS;
-  const int nij = g.Bx * g.By;
-  if ((P.TS & 3) == 0) {
-    const int q4 = P.TS >> 2;                           // float4 per column
-    for (int idx = threadIdx.x; idx < nij * q4; idx += NT) {
-      const int ij = idx / q4, k = (idx - ij * q4) << 2;
-      const float* t = tile + k * P.plane + ij;
-      *reinterpret_cast<float4*>(out + (int64_t)ij * g.Bt + k) =
-          make_float4(t[0], t[P.plane], t[2 * P.plane], t[3 * P.plane]);
-    }
-  } else {
-    for (int idx = threadIdx.x; idx < nij * P.TS; idx += NT) {
-      const int k = idx % P.TS, ij = idx / P.TS;
-      out[(int64_t)ij * g.Bt + k] = tile[k * P.plane + ij];
+  // tile -> payload[blk][col][sub * TS + k]: float4 copies, 4 TS bytes contiguous per column
+  {
+    float* out = payload + (int64_t)blk * P.ncol * g.Bt + sub * P.TS;
+    const int qs = P.ts_shift - 2, cs4 = P.CS >> 2;
+    const float4* t4 = reinterpret_cast<const float4*>(tile);
+    for (int idx = threadIdx.x; idx < (P.ncol << qs); idx += NT) {
+      const int c = idx >> qs, kq = idx & ((1 << qs) - 1);
+      *reinterpret_cast<float4*>(out + (int64_t)c * g.Bt + 4 * kq) = t4[c * cs4 + kq];
     }
   }
 }
@@ -596,34 +692,96 @@ k_truth_fill(int64_t nseg, const float* __restrict__ augf, const int32_t* __rest
   }
 }
 
-struct EffqWork { int32_t* slot; int32_t* tabslot; int32_t* seglist; void* scan; float* tab; int cap; size_t total; };
+
+
+struct EffqWork { int32_t* off; void* scan; float* tab; int64_t cap16; size_t fixed; };
 
 static EffqWork carve_effq(void* base, int64_t nseg, size_t work_bytes) {
   EffqWork w;
   size_t o = 0; char* b = (char*)base;
   auto take = [&](size_t bytes) { void* p = b ? b + o : nullptr; o += align_up(bytes, 256); return p; };
-  w.slot = (int32_t*)take((size_t)(nseg + 1) * 4);
-  w.tabslot = (int32_t*)take((size_t)(nseg > 0 ? nseg : 1) * 4);
+  w.off = (int32_t*)take((size_t)(nseg + 1) * 4);
   w.scan = take(tred_scan_work_bytes(nseg + 1));
-  const size_t fixed = o;
-  int64_t cap = nseg < EFFQ_MAX_SLOTS ? nseg : EFFQ_MAX_SLOTS;
-  if (work_bytes) {                                  // what the given workspace holds
-    const size_t per = (size_t)TAB_FLOATS * 4 + 4;
-    cap = work_bytes > fixed + 4096 ? (int64_t)((work_bytes - fixed - 4096) / per) : 0;
-    if (cap > nseg) cap = nseg;
-    if (cap > EFFQ_MAX_SLOTS) cap = EFFQ_MAX_SLOTS;
-  }
-  if (cap < 0) cap = 0;
-  w.cap = (int)cap;
-  w.seglist = (int32_t*)take((size_t)(cap > 0 ? cap : 1) * 4);
-  w.tab = (float*)take((size_t)(cap > 0 ? cap : 1) * TAB_FLOATS * 4);
-  w.total = o;
+  w.fixed = o;
+  w.tab = (float*)(b ? b + o : nullptr);
+  w.cap16 = work_bytes > o ? (int64_t)((work_bytes - o) / 16) : 0;
+  if (w.cap16 > 0x7fffffff) w.cap16 = 0x7fffffff;              // offsets are int32, in 16-byte units
   return w;
 }
 
+// Workspace for the per-segment tables: the fixed part plus ~2 KB per segment (a segment of the
+// paper's workloads needs 1-1.5 KB), at most 4 GiB.  Less is allowed: segments whose tables do not
+// fit are evaluated by the tile CTAs themselves.
 extern "C" size_t tred_effq_work_bytes(const tred_ctx* ctx, int64_t nseg) {
   if (!ctx || nseg < 0) return 0;
-  return carve_effq(nullptr, nseg, 0).total;
+  size_t t = (size_t)nseg * 2048;
+  if (t > ((size_t)4 << 30)) t = (size_t)4 << 30;
+  return carve_effq(nullptr, nseg, 0).fixed + t;
+}
+
+// shape of the tile kernel for this configuration; false if the block shape is outside what it
+// supports (then the closed-form kernel runs)
+static bool effq_blk_shape(const tred_ctx* ctx, const TredGrid& g, BlkParams& P, int& threads, size_t& smem) {
+  const int ncol = g.Bx * g.By;
+  if (ncol < 16 || ncol > 1024 || g.Bt < 4 || ((g.Bx + g.By) & 3)) return false;
+  P.ncol = ncol;
+  P.by_shift = 0;
+  while ((1 << P.by_shift) < g.By) ++P.by_shift;
+  // 1024-column blocks run one CTA of 1024 threads per SM and may use most of its shared memory
+  const size_t budget = ncol >= 1024 ? 150 * 1024 : 72 * 1024;
+  int TS = g.Bt;
+  while (TS > 4 && (size_t)ncol * (TS + 4) * sizeof(float) > budget) TS /= 2;
+  P.TS = TS; P.nsub = g.Bt / TS;
+  P.ts_shift = 0;
+  while ((1 << P.ts_shift) < TS) ++P.ts_shift;
+  P.CS = TS + 4;
+  P.RS = g.Bx + g.By + TS;
+  // warps: 32 (16 for a 4x4 block) columns each, as wi rows x wj columns of a row
+  const int wcols = ncol >= 32 ? 32 : ncol;
+  P.wj = g.By < wcols ? g.By : wcols;
+  P.wi = wcols / P.wj;
+  P.nwj = g.By / P.wj;
+  P.nwi = g.Bx / P.wi;
+  int nwarps = P.nwj * P.nwi;                       // one tick range
+  int nparts = 1;
+  while (nwarps * nparts * 2 <= 8 && TS / (nparts * 2) >= 4) nparts *= 2;
+  P.wt = TS / nparts;
+  threads = nwarps * nparts * 32;
+  if (threads > 1024) return false;
+  smem = ((size_t)ncol * P.CS + (size_t)EB_GP * EB_MQ * P.RS) * sizeof(float) + (size_t)EB_SB * EB_NREC * 4;
+  return smem <= (size_t)ctx->smem_optin;
+}
+
+template <int N>
+static int effq_launch(tred_ctx* ctx, const TredGrid& g, BlkParams P, int threads, size_t smem, int64_t nseg,
+                       int64_t nblocks, const int64_t* d_keys, const int32_t* d_blk_off, const int32_t* d_pair_seg,
+                       const float* d_augf, const int32_t* d_augi, float* d_payload, void* d_work, size_t work_bytes,
+                       cudaStream_t st) {
+  EffqWork w = carve_effq(d_work, nseg, work_bytes);
+  const bool tables = d_work && w.cap16 >= 4096 && nseg > 0;
+  P.cap16 = tables ? w.cap16 : 0;
+  if (tables) {
+    TRED_CUDA(cudaMemsetAsync(w.off, 0, (size_t)(nseg + 1) * 4, st));
+    k_effq_mark<<<cdiv(nblocks * 32, 256), 256, 0, st>>>(nblocks, d_blk_off, d_pair_seg, w.off);
+    k_effq_sizes<N><<<cdiv(nseg + 1, 256), 256, 0, st>>>(nseg, d_augf, d_augi, w.off);
+    int rc = tred_exclusive_scan_i32(w.off, w.off, nseg + 1, nullptr, w.scan, st);
+    if (rc != TRED_OK) return rc;
+    k_effq_tables<N><<<cdiv(nseg, 128), 128, 0, st>>>(nseg, w.off, w.cap16, d_augf, d_augi, w.tab, g);
+    TRED_COUNT_LAUNCH(5);
+  }
+  const int32_t* tabofs = tables ? w.off : nullptr;
+  if (threads > 256) {
+    TRED_CUDA(cudaFuncSetAttribute(k_effq_blk<N, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_effq_blk<N, 1024><<<(unsigned)(nblocks * P.nsub), threads, smem, st>>>(
+        nseg, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi, tabofs, w.tab, d_payload, g, P);
+  } else {
+    TRED_CUDA(cudaFuncSetAttribute(k_effq_blk<N, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_effq_blk<N, 256><<<(unsigned)(nblocks * P.nsub), threads, smem, st>>>(
+        nseg, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi, tabofs, w.tab, d_payload, g, P);
+  }
+  TRED_COUNT_LAUNCH(1);
+  TRED_LAUNCH_CHECK("k_effq_blk");
+  return TRED_OK;
 }
 
 extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
@@ -634,61 +792,28 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
   if (nblocks == 0) return TRED_OK;
   if (!d_keys || !d_blk_off || !d_pair_seg || !d_augf || !d_augi || !d_payload) return TRED_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
-  if (ctx->cfg.effq_mode == 1)
+  if (ctx->cfg.effq_mode != 0 && ctx->cfg.effq_mode != 1) return TRED_EINVAL;
+  const TredGrid g = make_grid(ctx);
+  BlkParams P;
+  int threads = 0;
+  size_t smem = 0;
+  if (ctx->cfg.effq_mode == 1 || !effq_blk_shape(ctx, g, P, threads, smem))
     return tred_effq_closed_form(ctx, nseg, nblocks, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi,
                                  d_payload, st);
-  if (ctx->cfg.effq_mode != 0) return TRED_EINVAL;
-  const TredGrid g = make_grid(ctx);
-  FactParams P;
-  P.plane = g.Bx * g.By + 1;
-  // largest TS (power of two, <= Bt) whose tile fits ~64 KB
-  int TS = g.Bt;
-  while (TS > 4 && (size_t)TS * P.plane * sizeof(float) > TRED_EFFQ_TILE_KB * 1024) TS /= 2;
-  P.TS = TS; P.nsub = g.Bt / TS;
-  const size_t tile_floats = ((size_t)TS * P.plane + 3) & ~(size_t)3;
-  const size_t smem = (tile_floats + 2 * (size_t)(g.Bx + g.By + TS) * MP) * sizeof(float);
-  if (smem > (size_t)ctx->smem_optin) return TRED_EUNSUPPORTED;
-  int threads = g.Bx * g.By * 4;
-  threads = threads < 64 ? 64 : threads > TRED_EFFQ_THREADS ? TRED_EFFQ_THREADS : threads;
   if (nblocks * P.nsub >= (1ll << 31)) return TRED_EUNSUPPORTED;
-  EffqWork w = carve_effq(d_work, nseg, work_bytes);
-  const bool tables = d_work && w.total <= work_bytes && w.cap >= 1024;
   TredProfScope ps(ctx, ST_EFFQ, st);
-  for (int64_t k0 = 0; k0 < nblocks; k0 += tables ? EFFQ_RANGE_BLOCKS : nblocks) {
-    const int nb = (int)(tables ? (nblocks - k0 < EFFQ_RANGE_BLOCKS ? nblocks - k0 : EFFQ_RANGE_BLOCKS) : nblocks);
-    if (tables) {
-      TRED_CUDA(cudaMemsetAsync(w.slot, 0, (size_t)(nseg + 1) * 4, st));
-      k_effq_mark<<<cdiv((int64_t)nb * 32, 256), 256, 0, st>>>(nb, (int)k0, d_blk_off, d_pair_seg, w.slot);
-      int rc = tred_exclusive_scan_i32(w.slot, w.slot, nseg + 1, nullptr, w.scan, st);
-      if (rc != TRED_OK) return rc;
-      k_effq_list<<<cdiv(nseg, 256), 256, 0, st>>>(nseg, w.slot, w.seglist, w.cap, w.tabslot);
-      TRED_COUNT_LAUNCH(4);
-    }
-#define LAUNCH(NN)                                                                                     \
-  do {                                                                                                 \
-    if (tables)                                                                                        \
-      k_effq_tables<NN><<<cdiv(w.cap, 4), 128, 0, st>>>(nseg, w.slot, w.seglist, w.cap, d_augf, d_augi, \
-                                                        w.tab, w.tabslot);                             \
-    TRED_CUDA(cudaFuncSetAttribute(k_effq_fact<NN>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                                   (int)smem));                                                        \
-    k_effq_fact<NN><<<(unsigned)((int64_t)nb * P.nsub), threads, smem, st>>>(                          \
-        nseg, d_keys + k0, d_blk_off + k0, d_pair_seg, d_augf, d_augi, tables ? w.tabslot : nullptr,   \
-        w.tab, d_payload + k0 * g.Bx * g.By * g.Bt, g, P);                                             \
-  } while (0)
-    TRED_COUNT_LAUNCH(tables ? 2 : 1);
-    switch (g.gl_n) {
-      case 1: LAUNCH(1); break;
-      case 2: LAUNCH(2); break;
-      case 3: LAUNCH(3); break;
-      case 4: LAUNCH(4); break;
-      default: return TRED_EINVAL;
-    }
-#undef LAUNCH
+  switch (g.gl_n) {
+    case 1: return effq_launch<1>(ctx, g, P, threads, smem, nseg, nblocks, d_keys, d_blk_off, d_pair_seg, d_augf,
+                                  d_augi, d_payload, d_work, work_bytes, st);
+    case 2: return effq_launch<2>(ctx, g, P, threads, smem, nseg, nblocks, d_keys, d_blk_off, d_pair_seg, d_augf,
+                                  d_augi, d_payload, d_work, work_bytes, st);
+    case 3: return effq_launch<3>(ctx, g, P, threads, smem, nseg, nblocks, d_keys, d_blk_off, d_pair_seg, d_augf,
+                                  d_augi, d_payload, d_work, work_bytes, st);
+    case 4: return effq_launch<4>(ctx, g, P, threads, smem, nseg, nblocks, d_keys, d_blk_off, d_pair_seg, d_augf,
+                                  d_augi, d_payload, d_work, work_bytes, st);
+    default: return TRED_EINVAL;
   }
-  TRED_LAUNCH_CHECK("k_effq_fact");
-  return TRED_OK;
 }
-
 
 extern "C" size_t tred_truth_work_bytes(const tred_ctx* ctx, int64_t nseg) {
   if (!ctx || nseg < 0) return 0;
