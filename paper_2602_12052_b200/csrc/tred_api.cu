@@ -159,6 +159,8 @@ extern "C" int tred_create(const tred_config* cfg, tred_ctx** out) {
   c->dims = d;
   TRED_CUDA(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
   TRED_CUDA(cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  TRED_CUDA(cudaDeviceGetAttribute(&c->smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+  c->device = dev;
   rc = tred_effq_init_tables();
   if (rc != TRED_OK) { free(c); return rc; }
   *out = c;

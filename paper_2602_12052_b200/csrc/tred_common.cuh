@@ -17,6 +17,8 @@ struct tred_ctx {
   tred_dims   dims;
   int         num_sms;
   int         smem_optin;     // max dynamic shared memory per block (bytes)
+  int         smem_sm;        // shared memory per SM (bytes)
+  int         device;         // CUDA device the context was created on
   const void* sym_rhat;       // last d_rhat prepared from a mirror-symmetric response (or NULL)
   // stage profiling (tred_profile_begin / tred_profile_end)
   int         prof_on;

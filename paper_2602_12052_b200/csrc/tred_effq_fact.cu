@@ -161,23 +161,30 @@ __device__ __forceinline__ void effq_cells(int gi, int lo_a, int hi_a, float p0a
 // ------------------------------------------------------------------ tables built once per segment
 // A segment meets ~4 blocks x 1.5 tick tiles, and every such CTA needs the same three per-axis
 // tables.  With a workspace, tred_effq builds them once per segment (k_effq_tables, one warp per
-// segment, whole bounding box) and the tile CTAs copy the rows they need with cp.async; without
+// segment, whole bounding box) and the tile CTAs fetch the rows they need with bulk copies; without
 // one (or for segments whose tables do not fit it) the tile CTAs compute the rows themselves with
 // the same code (effq_cells): same values either way.
-// Table of segment s at tab + 4 * off[s] floats: [point][rs], rs = align4(nxf + nyf) + ntfp;
-// x rows (grid points lox-E .. hix+E), y rows, then the t rows from the 4-aligned tick tb =
-// align_down(lot - E, 4), ntfp = align_up(hit + E + 1 - tb, 4) of them.  Entries of grid points
-// outside the grid are zero (clip and drop, reading G13).
-struct TabGeom { int nxf, nyf, tb, ntfp, toff, rs; };
+// Table of segment s at tab + 4 * off[s] floats: chunks of EB_MQ = 12 quadrature points, chunk c
+// is [row][cpt] (cpt = points of the chunk rounded up to 4, so every row range is a 16-byte
+// aligned contiguous piece); rows = x rows (grid points lox-E .. hix+E), y rows, then t rows
+// from the 4-aligned tick tb = align_down(lot - E, 4), ntfp = align_up(hit + E + 1 - tb, 4) of
+// them.  Entries of grid points outside the grid are zero (clip and drop, reading G13).
+constexpr int EB_MQ = 12;           // quadrature points per pass / table chunk
+
+struct TabGeom { int nxf, nyf, tb, ntfp, rs; };
 __device__ __forceinline__ TabGeom tab_geom(int lox, int loy, int lot, int hix, int hiy, int hit, int E) {
   TabGeom t;
   t.nxf = hix - lox + 1 + 2 * E;
   t.nyf = hiy - loy + 1 + 2 * E;
   t.tb = (lot - E) & ~3;
   t.ntfp = ((hit + E + 1 - t.tb) + 3) & ~3;
-  t.toff = (t.nxf + t.nyf + 3) & ~3;
-  t.rs = t.toff + t.ntfp;
+  t.rs = t.nxf + t.nyf + t.ntfp;
   return t;
+}
+// floats of the table of a segment with ptot quadrature points and rs rows
+__device__ __forceinline__ int64_t tab_floats(int ptot, int rs) {
+  const int nfull = ptot / EB_MQ, rem = ptot - nfull * EB_MQ;
+  return (int64_t)rs * (nfull * EB_MQ + ((rem + 3) & ~3));
 }
 
 // marks the segments the blocks [0, nb) of this call refer to (idempotent plain stores)
@@ -206,7 +213,7 @@ k_effq_sizes(int64_t nseg, const float* __restrict__ augf, const int32_t* __rest
     const float p0x = augf[0 * nseg + s], p0y = augf[1 * nseg + s], p0t = augf[2 * nseg + s];
     const SegQuad q = seg_quad(augi[6 * nseg + s], augf[3 * nseg + s] - p0x, augf[4 * nseg + s] - p0y,
                                augf[5 * nseg + s] - p0t, augf[6 * nseg + s], augf[7 * nseg + s], augf[8 * nseg + s]);
-    const int64_t sz = (int64_t)q.npiece * q.m * (t.rs >> 2);
+    const int64_t sz = tab_floats(q.npiece * q.m, t.rs) >> 2;
     v = sz < (1 << 24) ? (int)sz : (1 << 24);           // absurdly large boxes: no table (never fits)
   }
   mark[s] = v;
@@ -242,28 +249,50 @@ k_effq_tables(int64_t nseg, const int32_t* __restrict__ off, int64_t cap16, cons
     const TabGeom t = tab_geom(lo[0], lo[1], lo[2], hi[0], hi[1], hi[2], E);
     float* T = tab + 4 * (int64_t)off[s];
     // cells: one leading cell per axis, then one per row
-    const int ncell = t.nxf + t.nyf + t.ntfp + 3;
+    const int ncell = t.rs + 3;
     for (int r0 = 0; r0 < ncell - 1; r0 += 31) {
       const int p = r0 + lane;
       int a, q0, first, rowb, NGa;
       if (p < t.nxf + 1) { a = 0; q0 = p; first = lo[0] - E; rowb = 0; NGa = g.NGx; }
       else if (p < t.nxf + t.nyf + 2) { a = 1; q0 = p - (t.nxf + 1); first = lo[1] - E; rowb = t.nxf; NGa = g.NGy; }
-      else { a = 2; q0 = p - (t.nxf + t.nyf + 2); first = t.tb; rowb = t.toff; NGa = g.NGt; }
+      else { a = 2; q0 = p - (t.nxf + t.nyf + 2); first = t.tb; rowb = t.nxf + t.nyf; NGa = g.NGt; }
       const int gi = first - 1 + q0;
       const bool wr = lane >= 1 && q0 >= 1 && p < ncell;
-      effq_cells<N>(gi, lo[a], hi[a], p0[a], d3[a], -LOG2E_HALF / (sg[a] * sg[a]), K, a == 0, wr,
-                    gi < 0 || gi >= NGa, T + rowb + q0 - 1, t.rs, qr, 0, ptot);
+      const float nk2 = -LOG2E_HALF / (sg[a] * sg[a]);
+      for (int g0 = 0; g0 < ptot; g0 += EB_MQ) {
+        const int cnt = min(EB_MQ, ptot - g0), cpt = (cnt + 3) & ~3;
+        effq_cells<N>(gi, lo[a], hi[a], p0[a], d3[a], nk2, K, a == 0, wr, gi < 0 || gi >= NGa,
+                      T + (int64_t)g0 * t.rs + (rowb + q0 - 1) * cpt, 1, qr, g0, cnt);
+      }
     }
-    // the padding between the y rows and the t rows is never read
   }
 }
 
 // ------------------------------------------------------------------ the tile kernel
+// Warp roles: the LAST warp is the producer, the others are consumers.
+//   producer : stages the segment records of the block (32 at a time), finds the ones that meet
+//              the tile, cuts their quadrature points into passes of <= 12 points, packs the
+//              passes' table rows (x rows, y rows, t rows of the clipped footprint, [row][cpt])
+//              into a stage of the table ring -- three bulk copies per pass from the segment's
+//              table in global memory, completion on the stage's mbarrier (or, without a table,
+//              computed in place) -- and writes one descriptor per pass;
+//   consumers: every warp OWNS a rectangle of the tile (wi rows x wj columns x wt ticks) for the
+//              whole CTA, so no two warps ever touch the same cell: no atomics, no CTA-wide
+//              barrier in the loop, fixed order of additions (passes in order).  Per pass the
+//              lanes share out the columns of the footprint inside the rectangle (and its tick
+//              quads when those are few) and add the rank-cnt product to the tile.
+// The tile is written out with one bulk store (TS floats of a column) per thread.
+// The CTAs are persistent (grid = 2 per SM, tiles round-robin): the producer runs ahead of the
+// consumers by the depth of the ring, so the dependent loads that start a tile (block key ->
+// segment list -> records -> table rows) overlap the arithmetic of the previous one.
 constexpr int EB_SB = 32;           // segment records staged per batch
-constexpr int EB_MQ = 12;           // quadrature points per pass (table columns)
-constexpr int EB_GP = 8;            // passes per group = table sets in shared memory
 constexpr int EB_NREC = 36;         // int32 words per staged record
-// staged record (after the batch prologue):
+constexpr int EB_STAGES = 4;
+constexpr int EB_STAGE_FLOATS = 2048;   // 8 KB of table rows per stage
+constexpr int EB_LAST = 0x100;      // s_n flag: last stage of the tile
+constexpr int EB_MAXP = 32;         // passes per stage at most
+constexpr int EB_ND = 12;           // int32 words per pass descriptor
+// staged record (producer only, after the batch prologue):
 //   0..5 lo, hi (x, y, t)   6 flag   7 m (points per piece)
 //   8..10 p0 (x, y, t)      11 K = Q' (2 pi)^-3/2 / (sx sy st) / 8
 //   12..14 d = p1 - p0      15 1 / npiece
@@ -271,10 +300,13 @@ constexpr int EB_NREC = 36;         // int32 words per staged record
 //   20..23 clipped footprint in the tile: x first, nx, y first, ny          (tile-relative)
 //   24..27 t first, t last (tile-relative), first / count of the 4-aligned tick range
 //   28 quadrature points in total (npiece m)   29 passes
-//   30 offset of the segment's table in 16-byte units (-1: none)   31 its row stride
+//   30 offset of the segment's table in 16-byte units (-1: none)   31 its rows
 //   32 x row, 33 y row, 34 t row of the table that holds the first x / y / aligned t entry of the tile
 enum { ER_M = 7, ER_P0 = 8, ER_K = 11, ER_D = 12, ER_INVNP = 15, ER_NK2 = 16, ER_GOFF = 19, ER_FX = 20, ER_FT = 24,
        ER_PTOT = 28, ER_NPASS = 29, ER_TOFF = 30, ER_TRS = 31, ER_TROW = 32 };
+// pass descriptor: 0..3 = x first, nx, y first, ny; 4..7 = t first, t last, aligned first, aligned count;
+// 8 = points, 9 = points rounded up to 4 (row pitch), 10 = offset of the pass's rows in the stage (floats)
+enum { ED_CNT = 8, ED_CPT = 9, ED_SLOT = 10 };
 
 struct BlkParams {
   int TS, nsub;      // ticks per CTA tile, tiles per block
@@ -282,267 +314,435 @@ struct BlkParams {
   int by_shift;      // log2(By)
   int ts_shift;      // log2(TS)
   int CS;            // column stride of the tile in floats (TS + 4: conflict-free LDS.128)
-  int RS;            // rows of one table set = Bx + By + TS
-  // what a warp owns for the whole CTA: wi rows x wj columns-in-a-row (wi * wj = 32 or 16) x wt ticks
+  int RS;            // most rows a pass can have = Bx + By + TS
+  // what a consumer warp owns for the whole CTA: wi rows x wj columns-in-a-row x wt ticks
   int wi, wj, wt;
   int nwj, nwi;      // warps along j, along i (warp -> (tick range, i range, j range))
+  int ncw;           // consumer warps (the producer is warp ncw)
   int64_t cap16;     // 16-byte units of table workspace (0: no tables)
 };
 
-__device__ __forceinline__ void cp_async4(float* dst, const float* src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src)
-               : "memory");
+__device__ __forceinline__ uint32_t eb_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void eb_mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async16(float* dst, const float* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src)
+__device__ __forceinline__ void eb_mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void eb_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// A wait longer than ~2 s means a broken pipeline: trap instead of hanging the device.
+__device__ __forceinline__ void eb_mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  long long t0 = 0;
+  for (int it = 0;; ++it) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (ok) return;
+    if (it == 64) t0 = clock64();
+    if (it > 64 && (it & 1023) == 0 && clock64() - t0 > 4000000000ll) {
+      printf("k_effq_blk: mbarrier wait timed out (block %d thread %d)\n", blockIdx.x, threadIdx.x);
+      __trap();
+    }
+  }
+}
+__device__ __forceinline__ void eb_bulk_g2s(float* dst, const float* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(eb_smem(dst)), "l"(src), "r"(bytes), "r"(bar)
                : "memory");
 }
 
-// Phase B of one pass for one lane: tile[col][k] += sum_pt GX[pt][i] GY[pt][j] GT[pt][k] for the
-// tick quads k = k0, k0 + kstep, ... < k1 of column col.
+// Phase B of one pass for one lane: tile[col][k] += sum_pt X[pt] Y[pt] T[k][pt] for the tick quads
+// k = k0, k0 + kstep, ... < k1 of column col.  X, Y, T rows have a pitch of CQ * 4 floats.
 template <int CNT>
-__device__ __forceinline__ void effq_blk_update(float* __restrict__ tcol, const float* __restrict__ T, int RS,
-                                                int xrow, int yrow, int trow0, int k0, int k1, int kstep) {
-  float ab[CNT];
+__device__ __forceinline__ void effq_blk_update(float* __restrict__ tcol, const float* __restrict__ X,
+                                                const float* __restrict__ Y, const float* __restrict__ T, int k0,
+                                                int k1, int kstep) {
+  constexpr int CQ = (CNT + 3) / 4;
+  float ab[4 * CQ];
 #pragma unroll
-  for (int pt = 0; pt < CNT; ++pt) ab[pt] = T[pt * RS + xrow] * T[pt * RS + yrow];
-  const int rs4 = RS >> 2;
-#pragma unroll 2
+  for (int q = 0; q < CQ; ++q) {
+    const float4 a = reinterpret_cast<const float4*>(X)[q], b = reinterpret_cast<const float4*>(Y)[q];
+    ab[4 * q] = a.x * b.x; ab[4 * q + 1] = a.y * b.y; ab[4 * q + 2] = a.z * b.z; ab[4 * q + 3] = a.w * b.w;
+  }
   for (int k = k0; k < k1; k += kstep) {
     float4* tp = reinterpret_cast<float4*>(tcol + k);
-    const float4* gt = reinterpret_cast<const float4*>(T + trow0 + k);
-    float4 v = *tp;
+    const float4* gt = reinterpret_cast<const float4*>(T + k * (4 * CQ));
+    float4 v4 = *tp;
+    float v[4] = {v4.x, v4.y, v4.z, v4.w};
 #pragma unroll
-    for (int pt = 0; pt < CNT; ++pt) {
-      const float4 gq = gt[pt * rs4];
-      v.x = fmaf(ab[pt], gq.x, v.x); v.y = fmaf(ab[pt], gq.y, v.y);
-      v.z = fmaf(ab[pt], gq.z, v.z); v.w = fmaf(ab[pt], gq.w, v.w);
-    }
-    *tp = v;
+    for (int kk = 0; kk < 4; ++kk)
+#pragma unroll
+      for (int q = 0; q < CQ; ++q) {
+        const float4 gq = gt[kk * CQ + q];
+        if (4 * q < CNT) v[kk] = fmaf(ab[4 * q], gq.x, v[kk]);
+        if (4 * q + 1 < CNT) v[kk] = fmaf(ab[4 * q + 1], gq.y, v[kk]);
+        if (4 * q + 2 < CNT) v[kk] = fmaf(ab[4 * q + 2], gq.z, v[kk]);
+        if (4 * q + 3 < CNT) v[kk] = fmaf(ab[4 * q + 3], gq.w, v[kk]);
+      }
+    *tp = make_float4(v[0], v[1], v[2], v[3]);
   }
 }
 
 template <int N, int MAXT>
-__global__ void __launch_bounds__(MAXT, MAXT >= 1024 ? 1 : 2)
+__global__ void __launch_bounds__(MAXT, MAXT > 512 ? 1 : 2)
 k_effq_blk(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __restrict__ blk_off,
            const int32_t* __restrict__ pair_seg, const float* __restrict__ augf,
            const int32_t* __restrict__ augi, const int32_t* __restrict__ tabofs, const float* __restrict__ gtab,
-           float* __restrict__ payload, TredGrid g, BlkParams P) {
-  extern __shared__ __align__(16) float smf[];
+           float* __restrict__ payload, int64_t ntiles, TredGrid g, BlkParams P) {
+  extern __shared__ __align__(128) float smf[];
   float* tile = smf;                                          // [ncol][CS]
-  float* tab = smf + (size_t)P.ncol * P.CS;                   // [EB_GP][EB_MQ][RS]
-  int32_t (*s_rec)[EB_NREC] = reinterpret_cast<int32_t (*)[EB_NREC]>(tab + (size_t)EB_GP * EB_MQ * P.RS);
+  float* ring = smf + (size_t)P.ncol * P.CS;                  // [EB_STAGES][EB_STAGE_FLOATS]
+  int32_t (*s_rec)[EB_NREC] = reinterpret_cast<int32_t (*)[EB_NREC]>(ring + EB_STAGES * EB_STAGE_FLOATS);
+  __shared__ __align__(16) int32_t s_desc[EB_STAGES][EB_MAXP][EB_ND];
+  __shared__ int s_n[EB_STAGES];
   __shared__ int s_list[EB_SB];
   __shared__ int s_pfx[EB_SB + 1];
-  __shared__ int s_cnt;
-  const int NT = blockDim.x;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = NT >> 5;
-  const int blk = blockIdx.x / P.nsub;
-  const int sub = blockIdx.x - blk * P.nsub;
-  const int64_t key = keys[blk];
-  const int by = (int)(key % g.NBy);
-  const int bx = (int)((key / g.NBy) % g.NBx);
-  const int bt = (int)(key / ((int64_t)g.NBy * g.NBx));
-  const int I0 = bx * g.Bx, J0 = by * g.By, K0 = bt * g.Bt + sub * P.TS;
+  __shared__ __align__(8) uint64_t s_bar[2 * EB_STAGES];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   constexpr int E = N > 1 ? 1 : 0;
   constexpr float LOG2E_HALF = 0.72134752044448170f;          // log2(e) / 2
+  const int nct = P.ncw * 32;                                 // consumer threads
+  auto full_bar = [&](int s) { return eb_smem(&s_bar[s]); };
+  auto empty_bar = [&](int s) { return eb_smem(&s_bar[EB_STAGES + s]); };
 
-  // what this warp owns: rows [wi0, wi0 + wi) x columns-in-a-row [wj0, wj0 + wj) x ticks [wt0, wt0 + wt)
-  const int wjj = warp % P.nwj, wrest = warp / P.nwj;
-  const int wii = wrest % P.nwi, wtt = wrest / P.nwi;
-  const int wi0 = wii * P.wi, wj0 = wjj * P.wj, wt0 = wtt * P.wt;
-
-  {
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < EB_STAGES; ++s) { eb_mbar_init(full_bar(s), 1); eb_mbar_init(empty_bar(s), P.ncw); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (threadIdx.x < nct) {
     float4* t4 = reinterpret_cast<float4*>(tile);
     const int n4 = (P.ncol * P.CS) >> 2;
-    for (int i = threadIdx.x; i < n4; i += NT) t4[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    for (int i = threadIdx.x; i < n4; i += nct) t4[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
+  __syncthreads();
 
-  const int s_beg = blk_off[blk], s_end = blk_off[blk + 1];
-  for (int b0 = s_beg; b0 < s_end; b0 += EB_SB) {
-    const int nbatch = min(EB_SB, s_end - b0);
-    __syncthreads();                                   // previous batch's records and tables are no longer read
-    // raw records: words 0..6 = bbox, flag; 7..16 = p0, p1, sigma, Q'; 17, 18 = table offsets of s, s + 1
-    for (int e = threadIdx.x; e < nbatch * 19; e += NT) {
-      const int j = e / 19, f = e - j * 19;
-      const int64_t s = pair_seg[b0 + j];
-      s_rec[j][f] = f < 7 ? augi[f * nseg + s]
-                  : f < 17 ? __float_as_int(augf[(f - 7) * nseg + s]) : (tabofs ? tabofs[s + (f - 17)] : 0);
+  if (warp == P.ncw) {
+    // ================================================================ producer
+    int stage = 0, sphase = 0;
+    // The stage filled last is handed over (arrive) only when the next one is ready or the tile
+    // ends, so that the tile's last stage can carry the EB_LAST flag; its copies run meanwhile.
+    int pend_stage = -1, pend_n = 0;
+    auto hand_over = [&](int flag) {
+      if (lane == 0) {
+        s_n[pend_stage] = pend_n | flag;
+        eb_mbar_arrive(full_bar(pend_stage));
+      }
+      pend_stage = -1;
+    };
+    const int W = EB_STAGE_FLOATS - P.RS * EB_MQ;             // passes that START in a window of W floats fit a stage
+    const float invW = 1.0f / (float)W;
+    // The loads that start a tile are issued one tile (records of its first batch) and two tiles
+    // (block key, segment range) ahead and land in registers while the current tile is processed.
+    struct Meta { int64_t key; int s_beg, s_end; };
+    auto load_meta = [&](int64_t t) {
+      Meta m{0, 0, 0};
+      if (t < ntiles) { const int b = (int)(t / P.nsub); m.key = keys[b]; m.s_beg = blk_off[b]; m.s_end = blk_off[b + 1]; }
+      return m;
+    };
+    // raw record of one lane: words 0..6 = bbox, flag; 7..16 = p0, p1, sigma, Q'; 17, 18 = table
+    // offsets of s, s + 1 (all loads of a record in flight at once)
+    auto load_rec = [&](int b0, int nbatch, int32_t (&v)[19]) {
+      if (lane < nbatch) {
+        const int64_t s = pair_seg[b0 + lane];
+#pragma unroll
+        for (int f = 0; f < 7; ++f) v[f] = augi[f * nseg + s];
+#pragma unroll
+        for (int f = 7; f < 17; ++f) v[f] = __float_as_int(augf[(f - 7) * nseg + s]);
+        v[17] = tabofs ? tabofs[s] : 0;
+        v[18] = tabofs ? tabofs[s + 1] : 0;
+      }
+    };
+    Meta m_cur = load_meta(blockIdx.x), m_nxt = load_meta((int64_t)blockIdx.x + gridDim.x);
+    int32_t vpre[19];
+    load_rec(m_cur.s_beg, min(EB_SB, m_cur.s_end - m_cur.s_beg), vpre);
+    for (int64_t tile_id = blockIdx.x; tile_id < ntiles; tile_id += gridDim.x) {
+    const int blk = (int)(tile_id / P.nsub);
+    const int sub = (int)(tile_id - (int64_t)blk * P.nsub);
+    const int64_t key = m_cur.key;
+    const int by = (int)(key % g.NBy);
+    const int bx = (int)((key / g.NBy) % g.NBx);
+    const int bt = (int)(key / ((int64_t)g.NBy * g.NBx));
+    const int I0 = bx * g.Bx, J0 = by * g.By, K0 = bt * g.Bt + sub * P.TS;
+    const int s_beg = m_cur.s_beg, s_end = m_cur.s_end;
+    __syncwarp();
+    if (lane < min(EB_SB, s_end - s_beg)) {
+#pragma unroll
+      for (int f = 0; f < 19; ++f) s_rec[lane][f] = vpre[f];
     }
-    __syncthreads();
-    // one lane per record: does the footprint meet this tile?  constants of the segment, once
-    if (warp == 0) {
-      const int j = lane;
-      bool hit_tile = false;
-      int npass = 0;
-      if (j < nbatch) {
-        int32_t* rec = s_rec[j];
-        const int lox = rec[0], loy = rec[1], lot = rec[2], hix = rec[3], hiy = rec[4], hit = rec[5];
-        const int ix0 = max(lox - E, I0), ix1 = min(min(hix + E, I0 + g.Bx - 1), g.NGx - 1);
-        const int iy0 = max(loy - E, J0), iy1 = min(min(hiy + E, J0 + g.By - 1), g.NGy - 1);
-        const int kt0 = max(lot - E, K0), kt1 = min(min(hit + E, K0 + P.TS - 1), g.NGt - 1);
-        hit_tile = ix0 <= ix1 && iy0 <= iy1 && kt0 <= kt1;
-        if (hit_tile) {
-          const int flag = rec[6];
-          const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
-          const float dx = __int_as_float(rec[10]) - p0x, dy = __int_as_float(rec[11]) - p0y,
-                      dt = __int_as_float(rec[12]) - p0t;
-          const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
-          const float Qp = __int_as_float(rec[16]);
-          const int o0 = rec[17], o1 = rec[18];
-          const SegQuad q = seg_quad(flag, dx, dy, dt, sx, sy, st);
-          const int ptot = q.npiece * q.m;
-          npass = (ptot + EB_MQ - 1) / EB_MQ;
-          rec[ER_M] = q.m;
-          rec[ER_P0 + 0] = __float_as_int(p0x); rec[ER_P0 + 1] = __float_as_int(p0y); rec[ER_P0 + 2] = __float_as_int(p0t);
-          rec[ER_K] = __float_as_int(Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f);
-          rec[ER_D + 0] = __float_as_int(dx); rec[ER_D + 1] = __float_as_int(dy); rec[ER_D + 2] = __float_as_int(dt);
-          rec[ER_INVNP] = __float_as_int(1.0f / (float)q.npiece);
-          rec[ER_NK2 + 0] = __float_as_int(-LOG2E_HALF / (sx * sx));
-          rec[ER_NK2 + 1] = __float_as_int(-LOG2E_HALF / (sy * sy));
-          rec[ER_NK2 + 2] = __float_as_int(-LOG2E_HALF / (st * st));
-          rec[ER_GOFF] = q.m * (q.m - 1) / 2;
-          rec[ER_FX + 0] = ix0 - I0; rec[ER_FX + 1] = ix1 - ix0 + 1;
-          rec[ER_FX + 2] = iy0 - J0; rec[ER_FX + 3] = iy1 - iy0 + 1;
-          const int a0 = (kt0 - K0) & ~3, a1 = ((kt1 - K0) | 3) + 1;
-          rec[ER_FT + 0] = kt0 - K0; rec[ER_FT + 1] = kt1 - K0; rec[ER_FT + 2] = a0; rec[ER_FT + 3] = a1 - a0;
-          rec[ER_PTOT] = ptot; rec[ER_NPASS] = npass;
-          const TabGeom t = tab_geom(lox, loy, lot, hix, hiy, hit, E);
-          const bool has = o1 > o0 && (int64_t)o1 <= P.cap16;
-          rec[ER_TOFF] = has ? o0 : -1;
-          rec[ER_TRS] = t.rs;
-          rec[ER_TROW + 0] = ix0 - (lox - E);
-          rec[ER_TROW + 1] = t.nxf + iy0 - (loy - E);
-          rec[ER_TROW + 2] = t.toff + (K0 + a0 - t.tb);
+    m_cur = m_nxt;
+    load_rec(m_cur.s_beg, min(EB_SB, m_cur.s_end - m_cur.s_beg), vpre);      // next tile's first batch
+    m_nxt = load_meta(tile_id + 2 * (int64_t)gridDim.x);
+    for (int b0 = s_beg; b0 < s_end; b0 += EB_SB) {
+      const int nbatch = min(EB_SB, s_end - b0);
+      __syncwarp();
+      if (b0 > s_beg) {
+        int32_t v[19];
+        load_rec(b0, nbatch, v);
+        if (lane < nbatch) {
+#pragma unroll
+          for (int f = 0; f < 19; ++f) s_rec[lane][f] = v[f];
         }
       }
-      const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
-      const int pos = __popc(bal & ((1u << j) - 1u));
-      if (hit_tile) s_list[pos] = j;
-      // exclusive prefix of the pass counts over the compacted list
-      int incl = npass;                               // 0 for records that do not hit
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += v;
-      }
-      if (hit_tile) s_pfx[pos] = incl - npass;
-      if (lane == 31) { s_pfx[__popc(bal)] = incl; s_cnt = __popc(bal); }
-    }
-    __syncthreads();
-    const int nlist = s_cnt;
-    const int npass_all = s_pfx[nlist];
-    for (int gp0 = 0; gp0 < npass_all; gp0 += EB_GP) {
-      const int npg = min(EB_GP, npass_all - gp0);
-      if (gp0 > 0) __syncthreads();                    // phase B of the previous group is done with the tables
-      // record and local pass index of the first pass of the group (uniform)
-      const uint32_t bal0 = __ballot_sync(0xffffffffu, lane < nlist && s_pfx[lane] <= gp0);
-      const int l0 = 31 - __clz(bal0), lp0 = gp0 - s_pfx[l0];
-      // ---- phase A: the tables of the passes of the group
+      __syncwarp();
+      // one lane per record: does the footprint meet this tile?  constants of the segment, once
+      int npass_all, nlist;
       {
-        int l = l0, lp = lp0;
-        for (int pl = 0; pl < npg; ++pl) {
-          const int32_t* rec = s_rec[s_list[l]];
-          const int4 fx = *reinterpret_cast<const int4*>(rec + ER_FX);
-          const int4 ft = *reinterpret_cast<const int4*>(rec + ER_FT);
-          const int nx = fx.y, ny = fx.w, nta = ft.w;
-          const int g0 = lp * EB_MQ;
-          const int cnt = min(EB_MQ, rec[ER_PTOT] - g0);
-          float* Ts = tab + (size_t)(pl * EB_MQ) * P.RS;
-          const int toff = rec[ER_TOFF];
-          if (toff >= 0) {
-            // copy: warp = quadrature point, lanes = x entries, y entries, 16-byte groups of t entries
-            const int trs = rec[ER_TRS];
-            const int ne = nx + ny + (nta >> 2);
-            for (int pt = warp; pt < cnt; pt += nwarps) {
-              const float* G = gtab + 4 * (int64_t)toff + (int64_t)(g0 + pt) * trs;
-              float* D = Ts + pt * P.RS;
-              for (int e = lane; e < ne; e += 32) {
-                if (e < nx) cp_async4(D + fx.x + e, G + rec[ER_TROW + 0] + e);
-                else if (e < nx + ny) cp_async4(D + g.Bx + fx.z + (e - nx), G + rec[ER_TROW + 1] + (e - nx));
-                else cp_async16(D + g.Bx + g.By + ft.z + 4 * (e - nx - ny), G + rec[ER_TROW + 2] + 4 * (e - nx - ny));
-              }
-            }
-          } else {
-            // compute: warp = round of 31 cells (one leading cell per axis)
+        const int j = lane;
+        bool hit_tile = false;
+        int npass = 0;
+        if (j < nbatch) {
+          int32_t* rec = s_rec[j];
+          const int lox = rec[0], loy = rec[1], lot = rec[2], hix = rec[3], hiy = rec[4], hit = rec[5];
+          const int ix0 = max(lox - E, I0), ix1 = min(min(hix + E, I0 + g.Bx - 1), g.NGx - 1);
+          const int iy0 = max(loy - E, J0), iy1 = min(min(hiy + E, J0 + g.By - 1), g.NGy - 1);
+          const int kt0 = max(lot - E, K0), kt1 = min(min(hit + E, K0 + P.TS - 1), g.NGt - 1);
+          hit_tile = ix0 <= ix1 && iy0 <= iy1 && kt0 <= kt1;
+          if (hit_tile) {
+            const int flag = rec[6];
+            const float p0x = __int_as_float(rec[7]), p0y = __int_as_float(rec[8]), p0t = __int_as_float(rec[9]);
+            const float dx = __int_as_float(rec[10]) - p0x, dy = __int_as_float(rec[11]) - p0y,
+                        dt = __int_as_float(rec[12]) - p0t;
+            const float sx = __int_as_float(rec[13]), sy = __int_as_float(rec[14]), st = __int_as_float(rec[15]);
+            const float Qp = __int_as_float(rec[16]);
+            const int o0 = rec[17], o1 = rec[18];
+            const SegQuad q = seg_quad(flag, dx, dy, dt, sx, sy, st);
+            const int ptot = q.npiece * q.m;
+            npass = (ptot + EB_MQ - 1) / EB_MQ;
+            rec[ER_M] = q.m;
+            rec[ER_P0 + 0] = __float_as_int(p0x); rec[ER_P0 + 1] = __float_as_int(p0y); rec[ER_P0 + 2] = __float_as_int(p0t);
+            rec[ER_K] = __float_as_int(Qp * 0.063493635934240969f / (sx * sy * st) * 0.125f);
+            rec[ER_D + 0] = __float_as_int(dx); rec[ER_D + 1] = __float_as_int(dy); rec[ER_D + 2] = __float_as_int(dt);
+            rec[ER_INVNP] = __float_as_int(1.0f / (float)q.npiece);
+            rec[ER_NK2 + 0] = __float_as_int(-LOG2E_HALF / (sx * sx));
+            rec[ER_NK2 + 1] = __float_as_int(-LOG2E_HALF / (sy * sy));
+            rec[ER_NK2 + 2] = __float_as_int(-LOG2E_HALF / (st * st));
+            rec[ER_GOFF] = q.m * (q.m - 1) / 2;
+            rec[ER_FX + 0] = ix0 - I0; rec[ER_FX + 1] = ix1 - ix0 + 1;
+            rec[ER_FX + 2] = iy0 - J0; rec[ER_FX + 3] = iy1 - iy0 + 1;
+            const int a0 = (kt0 - K0) & ~3, a1 = ((kt1 - K0) | 3) + 1;
+            rec[ER_FT + 0] = kt0 - K0; rec[ER_FT + 1] = kt1 - K0; rec[ER_FT + 2] = a0; rec[ER_FT + 3] = a1 - a0;
+            rec[ER_PTOT] = ptot; rec[ER_NPASS] = npass;
+            const TabGeom t = tab_geom(lox, loy, lot, hix, hiy, hit, E);
+            const bool has = o1 > o0 && (int64_t)o1 <= P.cap16;
+            rec[ER_TOFF] = has ? o0 : -1;
+            rec[ER_TRS] = t.rs;
+            rec[ER_TROW + 0] = ix0 - (lox - E);
+            rec[ER_TROW + 1] = t.nxf + iy0 - (loy - E);
+            rec[ER_TROW + 2] = t.nxf + t.nyf + (K0 + a0 - t.tb);
+          }
+        }
+        const uint32_t bal = __ballot_sync(0xffffffffu, hit_tile);
+        const int pos = __popc(bal & ((1u << j) - 1u));
+        if (hit_tile) s_list[pos] = j;
+        int incl = npass;                               // 0 for records that do not hit
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int v = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += v;
+        }
+        if (hit_tile) s_pfx[pos] = incl - npass;
+        nlist = __popc(bal);
+        npass_all = __shfl_sync(0xffffffffu, incl, 31);
+        if (lane == 31) s_pfx[nlist] = incl;
+      }
+      __syncwarp();
+      // lanes = passes, 32 at a time
+      for (int p0 = 0; p0 < npass_all; p0 += 32) {
+        const int pi = p0 + lane;
+        const bool valid = pi < npass_all;
+        int l = 0;
+        if (valid) {                                    // largest l with s_pfx[l] <= pi
+          int lo_ = 0, hi_ = nlist - 1;
+          while (lo_ < hi_) { const int mid = (lo_ + hi_ + 1) >> 1; if (s_pfx[mid] <= pi) lo_ = mid; else hi_ = mid - 1; }
+          l = lo_;
+        }
+        const int32_t* rec = s_rec[valid ? s_list[l] : 0];
+        const int lp = valid ? pi - s_pfx[l] : 0;
+        int4 fx = make_int4(0, 0, 0, 0), ft = make_int4(0, 0, 0, 0);
+        int cnt = 0, cpt = 0, size = 0;
+        if (valid) {
+          fx = *reinterpret_cast<const int4*>(rec + ER_FX);
+          ft = *reinterpret_cast<const int4*>(rec + ER_FT);
+          cnt = min(EB_MQ, rec[ER_PTOT] - lp * EB_MQ);
+          cpt = (cnt + 3) & ~3;
+          size = (fx.y + fx.w + ft.w) * cpt;
+        }
+        int incl = size;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int v = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += v;
+        }
+        const int excl = incl - size;
+        const int wid = valid ? (int)(((float)excl + 0.5f) * invW) : -1;
+        const int wid_max = __reduce_max_sync(0xffffffffu, wid);
+        for (int gw = 0; gw <= wid_max; ++gw) {
+          const bool in = valid && wid == gw;
+          const uint32_t m = __ballot_sync(0xffffffffu, in);
+          if (!m) continue;
+          const int head = __ffs(m) - 1;
+          const int slot = excl - __shfl_sync(0xffffffffu, excl, head);
+          const int idx = __popc(m & ((1u << lane) - 1u));
+          const int toff = in ? rec[ER_TOFF] : -1;
+          const uint32_t bytes = (in && toff >= 0) ? (uint32_t)size * 4u : 0u;
+          const uint32_t tot = __reduce_add_sync(0xffffffffu, bytes);
+          if (pend_stage >= 0) hand_over(0);
+          if (lane == 0) eb_mbar_wait(empty_bar(stage), sphase ^ 1);
+          __syncwarp();
+          float* sbase = ring + stage * EB_STAGE_FLOATS;
+          if (in) {
+            int32_t* d = s_desc[stage][idx];
+            *reinterpret_cast<int4*>(d) = fx;
+            *reinterpret_cast<int4*>(d + 4) = ft;
+            d[ED_CNT] = cnt; d[ED_CPT] = cpt; d[ED_SLOT] = slot;
+          }
+          pend_stage = stage; pend_n = __popc(m);
+          // passes of segments without a table: the warp computes their rows in place
+          uint32_t mc = __ballot_sync(0xffffffffu, in && toff < 0);
+          while (mc) {
+            const int b = __ffs(mc) - 1;
+            mc &= mc - 1;
+            const int lb = __shfl_sync(0xffffffffu, l, b), lpb = __shfl_sync(0xffffffffu, lp, b);
+            const int slotb = __shfl_sync(0xffffffffu, slot, b);
+            const int32_t* rb = s_rec[s_list[lb]];
+            const int4 fxb = *reinterpret_cast<const int4*>(rb + ER_FX);
+            const int4 ftb = *reinterpret_cast<const int4*>(rb + ER_FT);
+            const int nx = fxb.y, ny = fxb.w, nta = ftb.w;
+            const int g0 = lpb * EB_MQ;
+            const int cntb = min(EB_MQ, rb[ER_PTOT] - g0), cptb = (cntb + 3) & ~3;
+            const QuadRule qr{rb[ER_M], rb[6], rb[ER_GOFF], __int_as_float(rb[ER_INVNP])};
             const int ncell = nx + ny + nta + 3;
-            const QuadRule qr{rec[ER_M], rec[6], rec[ER_GOFF], __int_as_float(rec[ER_INVNP])};
-            for (int r0 = 31 * warp; r0 < ncell - 1; r0 += 31 * nwarps) {
+            for (int r0 = 0; r0 < ncell - 1; r0 += 31) {
               const int p = r0 + lane;
               int a, q0, first, rowb;
-              if (p < nx + 1) { a = 0; q0 = p; first = I0 + fx.x; rowb = fx.x; }
-              else if (p < nx + ny + 2) { a = 1; q0 = p - (nx + 1); first = J0 + fx.z; rowb = g.Bx + fx.z; }
-              else { a = 2; q0 = p - (nx + ny + 2); first = K0 + ft.z; rowb = g.Bx + g.By + ft.z; }
+              if (p < nx + 1) { a = 0; q0 = p; first = I0 + fxb.x; rowb = 0; }
+              else if (p < nx + ny + 2) { a = 1; q0 = p - (nx + 1); first = J0 + fxb.z; rowb = nx; }
+              else { a = 2; q0 = p - (nx + ny + 2); first = K0 + ftb.z; rowb = nx + ny; }
               const int gi = first - 1 + q0;           // dual cell between grid points gi and gi + 1
               const bool wr = lane >= 1 && q0 >= 1 && p < ncell;
               // the 4-aligned tick range may reach beyond the clipped footprint: zeros there
-              const bool zero = a == 2 && (gi < K0 + ft.x || gi > K0 + ft.y);
-              effq_cells<N>(gi, rec[a], rec[3 + a], __int_as_float(rec[ER_P0 + a]), __int_as_float(rec[ER_D + a]),
-                            __int_as_float(rec[ER_NK2 + a]), __int_as_float(rec[ER_K]), a == 0, wr, zero,
-                            Ts + rowb + q0 - 1, P.RS, qr, g0, cnt);
+              const bool zero = a == 2 && (gi < K0 + ftb.x || gi > K0 + ftb.y);
+              effq_cells<N>(gi, rb[a], rb[3 + a], __int_as_float(rb[ER_P0 + a]), __int_as_float(rb[ER_D + a]),
+                            __int_as_float(rb[ER_NK2 + a]), __int_as_float(rb[ER_K]), a == 0, wr, zero,
+                            sbase + slotb + (rowb + q0 - 1) * cptb, 1, qr, g0, cntb);
             }
           }
-          if (++lp == rec[ER_NPASS]) { lp = 0; ++l; }
-        }
-        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
-      }
-      __syncthreads();
-      // ---- phase B: every warp adds the passes of the group to the cells it owns, in order;
-      // within a pass the lanes share out the columns of the footprint that fall in the warp's
-      // rectangle (and, when those are fewer than 16, its tick quads)
-      {
-        int l = l0, lp = lp0;
-        for (int pl = 0; pl < npg; ++pl) {
-          const int32_t* rec = s_rec[s_list[l]];
-          const int4 fx = *reinterpret_cast<const int4*>(rec + ER_FX);
-          const int4 ft = *reinterpret_cast<const int4*>(rec + ER_FT);
-          const int cnt = min(EB_MQ, rec[ER_PTOT] - lp * EB_MQ);
-          const int ia = max(fx.x, wi0), ib = min(fx.x + fx.y, wi0 + P.wi);
-          const int ja = max(fx.z, wj0), jb = min(fx.z + fx.w, wj0 + P.wj);
-          const int ka = max(ft.z, wt0), kb = min(ft.z + ft.w, wt0 + P.wt);
-          if (ia < ib && ja < jb && ka < kb) {
-            const int nj = jb - ja, nc = (ib - ia) * nj;
-            const int G = 32 / nc;                                   // lane groups: tick quads are dealt round-robin
-            const int grp = (int)(((float)lane + 0.5f) * __frcp_rn((float)nc));
-            const int c = lane - grp * nc;
-            const int ii = (int)(((float)c + 0.5f) * __frcp_rn((float)nj));
-            const int jj = c - ii * nj;
-            if (grp < G) {
-              const int ci = ia + ii, cj = ja + jj;
-              float* tcol = tile + (size_t)((ci << P.by_shift) + cj) * P.CS;
-              const float* T = tab + (size_t)(pl * EB_MQ) * P.RS;
-              const int trow0 = g.Bx + g.By, k0 = ka + 4 * grp, ks = 4 * G;
-              switch (cnt) {
-                case 1: effq_blk_update<1>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 2: effq_blk_update<2>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 3: effq_blk_update<3>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 4: effq_blk_update<4>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 5: effq_blk_update<5>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 6: effq_blk_update<6>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 7: effq_blk_update<7>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 8: effq_blk_update<8>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 9: effq_blk_update<9>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 10: effq_blk_update<10>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                case 11: effq_blk_update<11>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-                default: effq_blk_update<12>(tcol, T, P.RS, ci, g.Bx + cj, trow0, k0, kb, ks); break;
-              }
-            }
-            __syncwarp();                              // the next pass deals the cells to other lanes
+          __syncwarp();
+          if (lane == 0 && tot) eb_mbar_expect_tx(full_bar(stage), tot);
+          __syncwarp();
+          if (in && toff >= 0) {
+            const int trs = rec[ER_TRS];
+            const float* G = gtab + 4 * (int64_t)toff + (int64_t)lp * EB_MQ * trs;
+            float* D = sbase + slot;
+            eb_bulk_g2s(D, G + rec[ER_TROW + 0] * cpt, (uint32_t)(fx.y * cpt * 4), full_bar(stage));
+            eb_bulk_g2s(D + fx.y * cpt, G + rec[ER_TROW + 1] * cpt, (uint32_t)(fx.w * cpt * 4), full_bar(stage));
+            eb_bulk_g2s(D + (fx.y + fx.w) * cpt, G + rec[ER_TROW + 2] * cpt, (uint32_t)(ft.w * cpt * 4), full_bar(stage));
           }
-          if (++lp == rec[ER_NPASS]) { lp = 0; ++l; }
+          if (++stage == EB_STAGES) { stage = 0; sphase ^= 1; }
         }
       }
     }
-  }
-  __syncthreads();
-  // tile -> payload[blk][col][sub * TS + k]: float4 copies, 4 TS bytes contiguous per column
-  {
-    float* out = payload + (int64_t)blk * P.ncol * g.Bt + sub * P.TS;
-    const int qs = P.ts_shift - 2, cs4 = P.CS >> 2;
-    const float4* t4 = reinterpret_cast<const float4*>(tile);
-    for (int idx = threadIdx.x; idx < (P.ncol << qs); idx += NT) {
-      const int c = idx >> qs, kq = idx & ((1 << qs) - 1);
-      *reinterpret_cast<float4*>(out + (int64_t)c * g.Bt + 4 * kq) = t4[c * cs4 + kq];
+    // end of the tile: its last stage carries the flag (an empty one if the tile had no pass)
+    __syncwarp();
+    if (pend_stage < 0) {
+      if (lane == 0) eb_mbar_wait(empty_bar(stage), sphase ^ 1);
+      pend_stage = stage; pend_n = 0;
+      if (++stage == EB_STAGES) { stage = 0; sphase ^= 1; }
+    }
+    hand_over(EB_LAST);
+    }
+  } else {
+    // ================================================================ consumers
+    // what this warp owns: rows [wi0, wi0 + wi) x columns-in-a-row [wj0, wj0 + wj) x ticks [wt0, wt0 + wt)
+    const int wjj = warp % P.nwj, wrest = warp / P.nwj;
+    const int wii = wrest % P.nwi, wtt = wrest / P.nwi;
+    const int wi0 = wii * P.wi, wj0 = wjj * P.wj, wt0 = wtt * P.wt;
+    int stage = 0, sphase = 0;
+    for (int64_t tile_id = blockIdx.x; tile_id < ntiles; tile_id += gridDim.x) {
+    for (;;) {
+      eb_mbar_wait(full_bar(stage), sphase);
+      const int nflag = s_n[stage];
+      const int n = nflag & (EB_LAST - 1);
+      const float* sbase = ring + stage * EB_STAGE_FLOATS;
+      for (int pl = 0; pl < n; ++pl) {
+        const int32_t* d = s_desc[stage][pl];
+        const int4 fx = *reinterpret_cast<const int4*>(d);
+        const int4 ft = *reinterpret_cast<const int4*>(d + 4);
+        const int ia = max(fx.x, wi0), ib = min(fx.x + fx.y, wi0 + P.wi);
+        const int ja = max(fx.z, wj0), jb = min(fx.z + fx.w, wj0 + P.wj);
+        const int ka = max(ft.z, wt0), kb = min(ft.z + ft.w, wt0 + P.wt);
+        if (ia < ib && ja < jb && ka < kb) {
+          const int4 dd = *reinterpret_cast<const int4*>(d + 8);        // cnt, cpt, slot
+          const int cnt = dd.x, cpt = dd.y;
+          const float* S = sbase + dd.z;
+          const int nj = jb - ja;
+          const int rows_it = nj >= 32 ? 1 : 32 / nj;                   // rows of the rectangle dealt at once
+          const float rnj = __frcp_rn((float)nj);
+          for (int i0 = ia; i0 < ib; i0 += rows_it) {
+            const int ni = min(rows_it, ib - i0), nc = ni * nj;
+            const int G = 32 / nc;                                       // lane groups: tick quads round-robin
+            const int grp = (int)(((float)lane + 0.5f) * __frcp_rn((float)nc));
+            const int c = lane - grp * nc;
+            const int ii = (int)(((float)c + 0.5f) * rnj);
+            const int jj = c - ii * nj;
+            if (grp < G) {
+              const int ci = i0 + ii, cj = ja + jj;
+              float* tcol = tile + (size_t)((ci << P.by_shift) + cj) * P.CS;
+              const float* X = S + (ci - fx.x) * cpt;
+              const float* Y = S + (fx.y + cj - fx.z) * cpt;
+              const float* T = S + (fx.y + fx.w - ft.z) * cpt;           // row of tile-relative tick 0
+              const int k0 = ka + 4 * grp, ks = 4 * G;
+              switch (cnt) {
+                case 1: effq_blk_update<1>(tcol, X, Y, T, k0, kb, ks); break;
+                case 2: effq_blk_update<2>(tcol, X, Y, T, k0, kb, ks); break;
+                case 3: effq_blk_update<3>(tcol, X, Y, T, k0, kb, ks); break;
+                case 4: effq_blk_update<4>(tcol, X, Y, T, k0, kb, ks); break;
+                case 5: effq_blk_update<5>(tcol, X, Y, T, k0, kb, ks); break;
+                case 6: effq_blk_update<6>(tcol, X, Y, T, k0, kb, ks); break;
+                case 7: effq_blk_update<7>(tcol, X, Y, T, k0, kb, ks); break;
+                case 8: effq_blk_update<8>(tcol, X, Y, T, k0, kb, ks); break;
+                case 9: effq_blk_update<9>(tcol, X, Y, T, k0, kb, ks); break;
+                case 10: effq_blk_update<10>(tcol, X, Y, T, k0, kb, ks); break;
+                case 11: effq_blk_update<11>(tcol, X, Y, T, k0, kb, ks); break;
+                default: effq_blk_update<12>(tcol, X, Y, T, k0, kb, ks); break;
+              }
+            }
+          }
+          __syncwarp();                                // the next pass deals the cells to other lanes
+        }
+      }
+      __syncwarp();
+      if (lane == 0) eb_mbar_arrive(empty_bar(stage));
+      if (++stage == EB_STAGES) { stage = 0; sphase ^= 1; }
+      if (nflag & EB_LAST) break;
+    }
+    // tile -> payload[blk][col][sub * TS + k] (float4 copies, TS floats contiguous per column),
+    // clearing the tile for the next one on the way
+    asm volatile("bar.sync 1, %0;" ::"r"(nct) : "memory");
+    {
+      const int64_t blk = tile_id / P.nsub;
+      const int sub = (int)(tile_id - blk * P.nsub);
+      float* out = payload + blk * P.ncol * g.Bt + sub * P.TS;
+      const int qs = P.ts_shift - 2;                              // float4 per column = 1 << qs
+      const int kq = threadIdx.x & ((1 << qs) - 1), c0 = threadIdx.x >> qs, cstep = nct >> qs;
+      float4* tp = reinterpret_cast<float4*>(tile + (size_t)c0 * P.CS) + kq;
+      float4* op = reinterpret_cast<float4*>(out + (int64_t)c0 * g.Bt) + kq;
+      const int tstep = (cstep * P.CS) >> 2;
+      const int64_t ostep = ((int64_t)cstep * g.Bt) >> 2;
+#pragma unroll 4
+      for (int c = c0; c < P.ncol; c += cstep, tp += tstep, op += ostep) {
+        *op = *tp;
+        *tp = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+      }
+    }
+    asm volatile("bar.sync 1, %0;" ::"r"(nct) : "memory");
     }
   }
 }
@@ -727,7 +927,7 @@ static bool effq_blk_shape(const tred_ctx* ctx, const TredGrid& g, BlkParams& P,
   P.ncol = ncol;
   P.by_shift = 0;
   while ((1 << P.by_shift) < g.By) ++P.by_shift;
-  // 1024-column blocks run one CTA of 1024 threads per SM and may use most of its shared memory
+  // 1024-column blocks run one CTA per SM and may use most of its shared memory
   const size_t budget = ncol >= 1024 ? 150 * 1024 : 72 * 1024;
   int TS = g.Bt;
   while (TS > 4 && (size_t)ncol * (TS + 4) * sizeof(float) > budget) TS /= 2;
@@ -736,8 +936,10 @@ static bool effq_blk_shape(const tred_ctx* ctx, const TredGrid& g, BlkParams& P,
   while ((1 << P.ts_shift) < TS) ++P.ts_shift;
   P.CS = TS + 4;
   P.RS = g.Bx + g.By + TS;
-  // warps: 32 (16 for a 4x4 block) columns each, as wi rows x wj columns of a row
-  const int wcols = ncol >= 32 ? 32 : ncol;
+  if (P.RS * EB_MQ + 256 > EB_STAGE_FLOATS) return false;      // a stage holds any one pass and then some
+  // consumer warps: 32 (16 for a 4x4 block, 64 for 1024 columns) columns each, as wi rows x wj
+  // columns of a row
+  const int wcols = ncol >= 1024 ? 64 : ncol >= 32 ? 32 : ncol;
   P.wj = g.By < wcols ? g.By : wcols;
   P.wi = wcols / P.wj;
   P.nwj = g.By / P.wj;
@@ -746,9 +948,10 @@ static bool effq_blk_shape(const tred_ctx* ctx, const TredGrid& g, BlkParams& P,
   int nparts = 1;
   while (nwarps * nparts * 2 <= 8 && TS / (nparts * 2) >= 4) nparts *= 2;
   P.wt = TS / nparts;
-  threads = nwarps * nparts * 32;
+  P.ncw = nwarps * nparts;
+  threads = (P.ncw + 1) * 32;
   if (threads > 1024) return false;
-  smem = ((size_t)ncol * P.CS + (size_t)EB_GP * EB_MQ * P.RS) * sizeof(float) + (size_t)EB_SB * EB_NREC * 4;
+  smem = ((size_t)ncol * P.CS + (size_t)EB_STAGES * EB_STAGE_FLOATS) * sizeof(float) + (size_t)EB_SB * EB_NREC * 4;
   return smem <= (size_t)ctx->smem_optin;
 }
 
@@ -758,7 +961,8 @@ static int effq_launch(tred_ctx* ctx, const TredGrid& g, BlkParams P, int thread
                        const float* d_augf, const int32_t* d_augi, float* d_payload, void* d_work, size_t work_bytes,
                        cudaStream_t st) {
   EffqWork w = carve_effq(d_work, nseg, work_bytes);
-  const bool tables = d_work && w.cap16 >= 4096 && nseg > 0;
+  // few blocks: the four extra launches cost more than the tables save
+  const bool tables = d_work && w.cap16 >= 4096 && nseg > 0 && nblocks >= 1024;
   P.cap16 = tables ? w.cap16 : 0;
   if (tables) {
     TRED_CUDA(cudaMemsetAsync(w.off, 0, (size_t)(nseg + 1) * 4, st));
@@ -770,14 +974,20 @@ static int effq_launch(tred_ctx* ctx, const TredGrid& g, BlkParams P, int thread
     TRED_COUNT_LAUNCH(5);
   }
   const int32_t* tabofs = tables ? w.off : nullptr;
-  if (threads > 256) {
+  // persistent CTAs: as many as are resident at once
+  const int64_t ntiles = nblocks * P.nsub;
+  const int per_sm = threads > 512 ? 1 : (int)((size_t)ctx->smem_sm / (smem + 4096) < 1 ? 1 : (size_t)ctx->smem_sm / (smem + 4096));
+  int64_t grid64 = (int64_t)ctx->num_sms * (per_sm > 4 ? 4 : per_sm);
+  if (grid64 > ntiles) grid64 = ntiles;
+  const unsigned grid = (unsigned)grid64;
+  if (threads > 288) {
     TRED_CUDA(cudaFuncSetAttribute(k_effq_blk<N, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_effq_blk<N, 1024><<<(unsigned)(nblocks * P.nsub), threads, smem, st>>>(
-        nseg, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi, tabofs, w.tab, d_payload, g, P);
+    k_effq_blk<N, 1024><<<grid, threads, smem, st>>>(
+        nseg, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi, tabofs, w.tab, d_payload, ntiles, g, P);
   } else {
-    TRED_CUDA(cudaFuncSetAttribute(k_effq_blk<N, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_effq_blk<N, 256><<<(unsigned)(nblocks * P.nsub), threads, smem, st>>>(
-        nseg, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi, tabofs, w.tab, d_payload, g, P);
+    TRED_CUDA(cudaFuncSetAttribute(k_effq_blk<N, 288>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_effq_blk<N, 288><<<grid, threads, smem, st>>>(
+        nseg, d_keys, d_blk_off, d_pair_seg, d_augf, d_augi, tabofs, w.tab, d_payload, ntiles, g, P);
   }
   TRED_COUNT_LAUNCH(1);
   TRED_LAUNCH_CHECK("k_effq_blk");
