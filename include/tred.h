@@ -69,14 +69,20 @@ typedef struct tred_config {
                                     0 = factored line integral (default, see tred_effq),
                                     1 = closed form with erf per Gauss-Legendre node          */
   int32_t mac_mode;              /* spectrum multiply-accumulate of tred_convolve:
-                                    0 = default: tensor cores over row tiles with the sum over
-                                        the offsets fused into the epilogue, on CTA pairs
-                                        (tcgen05 cta_group::2); operands split x = hi + lo, the
-                                        main product hi*hi in tf32, the two corrections lo*hi,
-                                        hi*lo (2^-11 of it) in bf16; if unsupported as 3, 2, 1,
-                                    5 = as 0 with all three products in tf32 (3xTF32),
-                                    3 = as 0 on single CTAs,
-                                    4 = as 0 with the mirror symmetry of the response
+                                    0 = default: the best of the modes below this configuration
+                                        supports, tried in the order 7, 6, 3, 2, 1
+                                        (tred_last_mac_mode reports the one that ran),
+                                    7 = tensor cores over row tiles with the sum over the offsets
+                                        fused into the epilogue, on CTA pairs (tcgen05
+                                        cta_group::2); operands split x = s (hi + lo), hi and lo
+                                        fp16, s a power of two per row / per frequency; the three
+                                        products hi*hi, lo*hi, hi*lo in fp16 with fp32
+                                        accumulation; the forward FFT writes the split operands,
+                                    6 = as 7 with fp32 spectra split in the kernel: hi*hi in tf32,
+                                        the two corrections in bf16,
+                                    5 = as 6 with all three products in tf32 (3xTF32),
+                                    3 = as 5 on single CTAs,
+                                    4 = as 5 with the mirror symmetry of the response
                                         (MPCP) spent on the product: sums and
                                         differences of mirror phase pairs, two products of half
                                         the size; falls back to 0 if the response prepared last
@@ -112,6 +118,10 @@ void tred_destroy(tred_ctx* ctx);
 const char* tred_strerror(int status);
 const char* tred_last_cuda_error(void);
 int  tred_abi_version(void);
+/* The spectrum-product kernel (a tred_config.mac_mode value 1..7) the last tred_convolve on
+ * this context launched; 0 before the first call.  A mode the configuration cannot run is
+ * replaced as tred_config.mac_mode describes, never silently: this is where it shows. */
+int  tred_last_mac_mode(const tred_ctx* ctx);
 
 /* Number of floats / int32 per segment in the augmented SoA record (see tred_drift). */
 #define TRED_AUG_NF 10

@@ -67,6 +67,7 @@ EXPORTS = {
     "tred_strerror": (C.c_char_p, [C.c_int]),
     "tred_last_cuda_error": (C.c_char_p, []),
     "tred_abi_version": (C.c_int, []),
+    "tred_last_mac_mode": (C.c_int, [_c_p]),
     "tred_drift": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p]),
     "tred_blockbin_work_bytes": (C.c_size_t, [_c_p, _c_i64, _c_i64]),
     "tred_blockbin": (C.c_int, [_c_p, _c_i64, _c_p, _c_i64, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p,
@@ -272,6 +273,10 @@ class Tred:
         ln = (C.c_int64 * n)()
         _check(self.L.tred_profile_end(self.h, n, C.cast(ms, _c_p), C.cast(ln, _c_p)), "tred_profile_end")
         return {self.L.tred_stage_name(i).decode(): (float(ms[i]), int(ln[i])) for i in range(n)}
+
+    def last_mac_mode(self) -> int:
+        """The spectrum-product kernel (tred_config.mac_mode value 1..7) the last convolve launched."""
+        return int(self.L.tred_last_mac_mode(self.h))
 
     # -- the calls ----------------------------------------------------------------
     def prepare_response(self, resp):

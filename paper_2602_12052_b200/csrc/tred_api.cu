@@ -76,7 +76,8 @@ extern "C" const char* tred_stage_name(int s) {
                                         "fft_fwd", "conv_misc", "mac", "accum", "ifft", "gather"};
   return (s >= 0 && s < ST_COUNT) ? names[s] : "?";
 }
-extern "C" int tred_abi_version(void) { return 1; }
+extern "C" int tred_abi_version(void) { return 2; }
+extern "C" int tred_last_mac_mode(const tred_ctx* c) { return c ? c->last_mac_mode : TRED_EINVAL; }
 
 extern "C" const char* tred_strerror(int s) {
   switch (s) {
@@ -97,7 +98,7 @@ extern "C" int tred_get_dims(const tred_config* c, tred_dims* d) {
   if (c->npix_x <= 0 || c->npix_y <= 0 || c->sub <= 0 || c->nticks <= 0) return TRED_EINVAL;
   if (c->gl_n < 1 || c->gl_n > 4) return TRED_EINVAL;
   if (c->resp_half < 0 || c->resp_nticks <= 0) return TRED_EINVAL;
-  if (c->effq_mode < 0 || c->effq_mode > 1 || c->mac_mode < 0 || c->mac_mode > 5) return TRED_EINVAL;
+  if (c->effq_mode < 0 || c->effq_mode > 1 || c->mac_mode < 0 || c->mac_mode > 7) return TRED_EINVAL;
   if (!(c->pitch_mm > 0) || !(c->tick_us > 0) || !(c->v_mm_us > 0) || !(c->lifetime_us > 0))
     return TRED_EINVAL;
   if (!(c->nsigma > 0) || !(c->sigma_min_xy_mm > 0) || !(c->sigma_min_t_us > 0)) return TRED_EINVAL;

@@ -20,6 +20,7 @@ struct tred_ctx {
   int         smem_sm;        // shared memory per SM (bytes)
   int         device;         // CUDA device the context was created on
   const void* sym_rhat;       // last d_rhat prepared from a mirror-symmetric response (or NULL)
+  int         last_mac_mode;  // spectrum-product kernel the last tred_convolve launched (tred_last_mac_mode)
   // stage profiling (tred_profile_begin / tred_profile_end)
   int         prof_on;
   int64_t     launches[ST_COUNT];
@@ -88,8 +89,12 @@ static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 // [W: fp32 complex [f][phase][kp]] [B_hi][B_lo: [f][2 kp][2 nph] tf32 parts]
 // [Bs_hi][Bs_lo][Bd_hi][Bd_lo: [f][SYM_N][nph] mirror-symmetric halves, see tred_conv.cu] [flag]
 // [B_hi, B_lo rounded to bf16, same shape as B_hi: operands of the bf16 correction products]
+// [B16: [f][2 kp][h16_kp] fp16, hi / lo parts of B / bscale[f] in blocks of 16 reals (tred_mac_h3.cu)]
+// [bscale: [f] float, power of two]
 constexpr int SYM_N = 128;           // rows of the symmetric matrices: 2 x (noff + 1) / 2 padded
-struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, bhb, blb, total; };
+// halves per operand row in the fp16 hi / lo block layout: ceil(2 nph / 16) blocks of (16 hi | 16 lo)
+static inline int h16_kp(const tred_dims& d) { return (2 * d.n_phase + 15) / 16 * 32; }
+struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, bhb, blb, b16, bsc, total; };
 static inline RhatLayout rhat_layout(const tred_dims& d) {
   RhatLayout L;
   const int64_t rb = (int64_t)d.n_freq * d.n_phase * d.n_off_pad;
@@ -99,7 +104,9 @@ static inline RhatLayout rhat_layout(const tred_dims& d) {
   L.flag = L.bd_lo + sb;
   L.bhb = L.flag + 8;                 // bf16 copies of B_hi and B_lo, [f][2 kp][2 nph] bf16 = 2 rb floats each
   L.blb = L.bhb + 2 * rb;
-  L.total = L.blb + 2 * rb;
+  L.b16 = L.blb + 2 * rb;              // 16-byte aligned: every term above is a multiple of 8 floats
+  L.bsc = L.b16 + (int64_t)d.n_freq * 2 * d.n_off_pad * (h16_kp(d) / 2);
+  L.total = L.bsc + (d.n_freq + 7) / 8 * 8;
   return L;
 }
 

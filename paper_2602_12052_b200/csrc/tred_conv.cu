@@ -16,6 +16,7 @@
 //   (e) overlap-add of the slab outputs into tiles (pixel, Bt ticks)      (k_gather_*)
 // Spectra hold L/2 complex numbers: slot 0 packs (DC, Nyquist), both real.
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include "tred_common.cuh"
 #include "tred_fft.cuh"
 
@@ -86,6 +87,67 @@ k_resp_dft64(const float* __restrict__ resp, float2* __restrict__ W, float* __re
       put(2 * off, 2 * phase + 1, -fim);
       put(2 * off + 1, 2 * phase + 1, fre);
     }
+  }
+}
+
+// fp16 hi / lo operands of the three-product tensor-core path (tred_mac_h3.cu): per frequency
+// slot a power-of-two scale s_f with max |W[f]| / s_f in [2^14, 2^15), then
+// B16[f][n][block(kk)] = fp16 parts of B[n][kk] / s_f, B as above, kk in blocks of (16 hi | 16 lo).
+__device__ __forceinline__ float h16_scale(float m) {       // power of two s, m / s in [2^14, 2^15); 1 for m = 0
+  const int ex = (int)((__float_as_uint(m) >> 23) & 0xffu);
+  if (ex == 0 || ex == 255) return 1.0f;
+  const int se = max(1, ex - 14);
+  return __uint_as_float((uint32_t)se << 23);
+}
+__device__ __forceinline__ float pow2_inverse(float s) {    // 1 / s for s = 2^k, exponent field in [1, 253]
+  return __uint_as_float((254u - (__float_as_uint(s) >> 23)) << 23);
+}
+
+__global__ void __launch_bounds__(256)
+k_resp_h16_scale(const float2* __restrict__ W, float* __restrict__ bscale, int nph, int kp, int noff) {
+  __shared__ float red[8];
+  const int f = blockIdx.x;
+  float m = 0.0f;
+  for (int i = threadIdx.x; i < nph * kp; i += 256)
+    if (i % kp < noff) {
+      const float2 w = W[(int64_t)f * nph * kp + i];
+      m = fmaxf(m, fmaxf(fabsf(w.x), fabsf(w.y)));
+    }
+  for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, red[w]);
+    bscale[f] = h16_scale(m);
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_resp_h16(const float2* __restrict__ W, const float* __restrict__ bscale, __half* __restrict__ B16,
+           int nf, int nph, int noff, int kp, int kp16) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (int64_t)nf * nph * noff) return;
+  const int off = (int)(i % noff);
+  const int ph = (int)((i / noff) % nph);
+  const int f = (int)(i / ((int64_t)noff * nph));
+  const float2 w = W[((int64_t)f * nph + ph) * kp + off];
+  const float inv = pow2_inverse(bscale[f]);
+  __half* plane = B16 + (int64_t)f * (2 * kp) * kp16;
+  auto put = [&](int n, int kk, float v) {
+    v *= inv;
+    const __half h = __float2half_rn(v);
+    __half* e = plane + (int64_t)n * kp16 + (kk >> 4) * 32 + (kk & 15);
+    e[0] = h;
+    e[16] = __float2half_rn(v - __half2float(h));
+  };
+  if (f == 0) {                         // slot 0: DC in the real lane, Nyquist in the imaginary lane
+    put(2 * off, 2 * ph, w.x);
+    put(2 * off + 1, 2 * ph + 1, w.y);
+  } else {
+    put(2 * off, 2 * ph, w.x);
+    put(2 * off + 1, 2 * ph, w.y);
+    put(2 * off, 2 * ph + 1, -w.y);
+    put(2 * off + 1, 2 * ph + 1, w.x);
   }
 }
 
@@ -430,11 +492,17 @@ k_fft_fwd_ct(const float* __restrict__ payload, const int32_t* __restrict__ bloc
 // SYM: the 20 columns of the CTA are the sums (first 10) and differences (last 10) of the
 // mirror phase pairs p = 10 grp + pl and nph-1-p (the FFT is linear, so they are formed
 // on the samples), written to qhat[f][row][s: 50 | d: 50] for the mirror-symmetric product.
-template <int M, int B, int NZA, bool SYM>
-__global__ void __launch_bounds__((20 * (M / B) + 31) / 32 * 32)
+// MODE 2 (H16): the spectra leave as fp16 hi / lo parts in the block layout of tred_mac_h3.cu,
+// qhat = [f][row][KP16] halves, scaled per row by the power of two rscale[row] chosen from
+// sum |q| over the row's columns (no spectrum value can exceed it, so nothing overflows).
+template <int M, int B, int NZA, int MODE>
+__global__ void __launch_bounds__((20 * (M / B) + 31) / 32 * 32, MODE == 2 ? 65536 / 80 / ((20 * (M / B) + 31) / 32 * 32) : 1)
 k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ blockmap,
-             RowSrc rs, int rp, float2* __restrict__ qhat, const float2* __restrict__ gtw, TredGrid g) {
+             RowSrc rs, int rp, float2* __restrict__ qhat, float* __restrict__ rscale,
+             const float2* __restrict__ gtw, TredGrid g) {
+  constexpr bool SYM = MODE == 1, H16 = MODE == 2;
   constexpr int A = M / B, CG = 20, S = 10, JG = 2, NGRP = 5, NPH = 100;
+  constexpr int KP16 = (2 * NPH + 15) / 16 * 32;
   constexpr int NT = (CG * A + 31) / 32 * 32;
   constexpr int BP = B + 1, ZP = M + 1;
   constexpr int LOGB = tred_log2(B);
@@ -466,6 +534,29 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   __syncthreads();
   const int hb = g.Bt >> 1;
   const int64_t fstride = (int64_t)rp * NPH;
+  float sdown = 1.0f;                                        // H16: 1 / rscale[row]
+  if constexpr (H16) {
+    __shared__ float red[NT / 32];
+    float sum = 0.0f;
+    const int nq = g.Bt >> 2;
+    for (int i = threadIdx.x; i < NGRP * CG * nq; i += NT) {
+      const int c = i / nq, q4 = i - c * nq;
+      const long long base = colbase_all[c];
+      if (base >= 0) {
+        const float4 v = __ldg(reinterpret_cast<const float4*>(payload + base) + q4);
+        sum += (fabsf(v.x) + fabsf(v.y)) + (fabsf(v.z) + fabsf(v.w));
+      }
+    }
+    for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    float tot = red[0];
+#pragma unroll
+    for (int w = 1; w < NT / 32; ++w) tot += red[w];
+    const float sc = h16_scale(tot);
+    sdown = pow2_inverse(sc);
+    if (threadIdx.x == 0) rscale[row] = sc;
+  }
 #pragma unroll 1
   for (int grp = 0; grp < NGRP; ++grp) {
   const long long* colbase = colbase_all + grp * CG;
@@ -549,7 +640,64 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
   // ---- real-FFT post-processing on pairs (k, M - k); slot 0 packs (DC, Nyquist).
   // Thread (kr, c): column c, pairs k = 1 + kr, 1 + kr + KR, ...; the two output pointers
   // advance by a constant, no index arithmetic in the loop.
-  {
+  if constexpr (H16) {
+    // thread (kr, cp): the two adjacent columns 2 cp, 2 cp + 1 (phases p0, p0 + 1 share a block
+    // of 8 phases, so their hi parts are 8 contiguous bytes and their lo parts the 8 bytes 32
+    // bytes further on)
+    constexpr int CP = CG / 2, KR = NT / CP;
+    const int cp = threadIdx.x % CP, kr = threadIdx.x / CP;
+    const int p0 = grp * CG + 2 * cp;
+    __half* out = reinterpret_cast<__half*>(qhat) + (int64_t)row * KP16 + (p0 >> 3) * 32 + (p0 & 7) * 2;
+    const int64_t fstride_h = (int64_t)rp * KP16;
+    const float2* Z0 = buf + (2 * cp) * ZP;
+    const float2* Z1 = Z0 + ZP;
+    auto h2u = [](__half2 h) { return *reinterpret_cast<uint32_t*>(&h); };
+    // (the operands arrive already scaled by sdown.)  Phases 98, 99 end the last block of 16 reals:
+    // that thread also zeroes the block's 8 padding reals (hi and lo), which the tensor core reads
+    const bool pad = (2 * NPH) % 16 != 0 && p0 == NPH - 2;
+    auto put = [&](__half* o, float2 a, float2 b) {
+      const __half2 ha = __floats2half2_rn(a.x, a.y), hb2 = __floats2half2_rn(b.x, b.y);
+      const float2 fa = __half22float2(ha), fb = __half22float2(hb2);
+      const __half2 la = __floats2half2_rn(a.x - fa.x, a.y - fa.y), lb = __floats2half2_rn(b.x - fb.x, b.y - fb.y);
+      *reinterpret_cast<uint2*>(o) = make_uint2(h2u(ha), h2u(hb2));
+      *reinterpret_cast<uint2*>(o + 16) = make_uint2(h2u(la), h2u(lb));
+      if (pad) {
+        *reinterpret_cast<uint4*>(o + 4) = make_uint4(0u, 0u, 0u, 0u);
+        *reinterpret_cast<uint4*>(o + 20) = make_uint4(0u, 0u, 0u, 0u);
+      }
+    };
+    const float hs = 0.5f * sdown;
+    if (kr < KR) {
+      if (kr == 0) {
+        const float2 a = Z0[0], b = Z1[0];
+        put(out, make_float2(sdown * (a.x + a.y), sdown * (a.x - a.y)),
+            make_float2(sdown * (b.x + b.y), sdown * (b.x - b.y)));
+      } else if (kr == 1) {
+        const float2 a = Z0[M / 2], b = Z1[M / 2];                  // X[M/2] = conj(Z[M/2])
+        put(out + (M / 2) * fstride_h, make_float2(sdown * a.x, -sdown * a.y), make_float2(sdown * b.x, -sdown * b.y));
+      }
+      __half* o1 = out + (int64_t)(1 + kr) * fstride_h;
+      __half* o2 = out + (int64_t)(M - 1 - kr) * fstride_h;
+      const int64_t step = (int64_t)KR * fstride_h;
+#pragma unroll 2
+      for (int k = 1 + kr; k < M / 2; k += KR, o1 += step, o2 -= step) {
+        const float2 w = __ldg(gtw + k);
+        float2 x1[2], x2[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const float2* Z = j ? Z1 : Z0;
+          const float2 pz = Z[k], qz = Z[M - k];
+          const float2 e = make_float2(hs * (pz.x + qz.x), hs * (pz.y - qz.y));
+          const float2 o = make_float2(hs * (pz.x - qz.x), hs * (pz.y + qz.y));
+          const float2 wo = cmulf(w, o);
+          x1[j] = make_float2(e.x + wo.y, e.y - wo.x);              // X[k]
+          x2[j] = make_float2(e.x - wo.y, -e.y - wo.x);             // X[M-k]
+        }
+        put(o1, x1[0], x1[1]);
+        put(o2, x2[0], x2[1]);
+      }
+    }
+  } else {
     constexpr int KR = NT / CG;                                    // pair rows per sweep
     const int c = threadIdx.x % CG, kr = threadIdx.x / CG;
     const int cm = SYM ? (c < S ? c : c - S + NPH / 2) : c;
@@ -952,9 +1100,10 @@ static int launch_fft_fwd_ct(const tred_ctx* ctx, const TredGrid& g, const float
 
 #define TRED_FFT_2S_SHAPES(X) X(128, 32) X(144, 16) X(256, 32) X(288, 32) X(384, 32) X(512, 32)
 
-template <int MM, int BB, int NZA, bool SYM>
+template <int MM, int BB, int NZA, int MODE>
 static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
-                               const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
+                               const RowSrc& rs, int nr, int rp, float2* qhat, float* rscale, const float2* tw,
+                               cudaStream_t st) {
   constexpr int A = MM / BB;
   constexpr int NT = (20 * A + 31) / 32 * 32;
   constexpr size_t smem =
@@ -962,25 +1111,28 @@ static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const flo
   if (smem > (size_t)ctx->smem_optin) return 0;
   static bool set = false;
   if (!set) {
-    TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA, SYM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     set = true;
   }
-  k_fft_fwd_2s<MM, BB, NZA, SYM><<<(unsigned)nr, NT, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);
+  k_fft_fwd_2s<MM, BB, NZA, MODE><<<(unsigned)nr, NT, smem, st>>>(payload, blockmap, rs, rp, qhat, rscale, tw, g);
   return 1;
 }
 
-template <bool SYM>
+// MODE 0: fp32 spectra, 1: mirror-pair sums / differences (fp32), 2: fp16 hi / lo parts + row scales
+template <int MODE>
 static int launch_fft_fwd_2s(const tred_ctx* ctx, const TredGrid& g, const float* payload, const int32_t* blockmap,
-                             const RowSrc& rs, int nr, int rp, float2* qhat, const float2* tw, cudaStream_t st) {
+                             const RowSrc& rs, int nr, int rp, float2* qhat, float* rscale, const float2* tw,
+                             cudaStream_t st) {
   if (g.S != 10 || nr < 1) return 0;
+  if (MODE == 2 && (g.Bt & 3)) return 0;
   const int M = g.L / 2, hb = g.Bt / 2;
   switch (M) {
 #define X(MM, BB)                                                                                          \
   case MM: {                                                                                               \
     const int nza = (hb + BB - 1) / BB;                                                                    \
-    if (nza <= 1) return launch_fft_fwd_2s_t<MM, BB, 1, SYM>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
-    if (nza == 2) return launch_fft_fwd_2s_t<MM, BB, 2, SYM>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
-    if (nza <= 4) return launch_fft_fwd_2s_t<MM, BB, 4, SYM>(ctx, g, payload, blockmap, rs, nr, rp, qhat, tw, st); \
+    if (nza <= 1) return launch_fft_fwd_2s_t<MM, BB, 1, MODE>(ctx, g, payload, blockmap, rs, nr, rp, qhat, rscale, tw, st); \
+    if (nza == 2) return launch_fft_fwd_2s_t<MM, BB, 2, MODE>(ctx, g, payload, blockmap, rs, nr, rp, qhat, rscale, tw, st); \
+    if (nza <= 4) return launch_fft_fwd_2s_t<MM, BB, 4, MODE>(ctx, g, payload, blockmap, rs, nr, rp, qhat, rscale, tw, st); \
     return 0;                                                                                              \
   }
     TRED_FFT_2S_SHAPES(X)
@@ -1074,7 +1226,7 @@ static ConvWork carve_conv(const tred_ctx* c, void* base, int64_t rows, int64_t 
 }
 
 struct TiledWork {
-  int32_t* blockmap; float2* tw; float2* ohat; float2* qhat; float2* opart;
+  int32_t* blockmap; float2* tw; float2* ohat; float2* qhat; float2* opart; float* rscale;
   size_t total, per_tile;
 };
 
@@ -1089,9 +1241,12 @@ static TiledWork carve_tiled(const tred_ctx* c, void* base, int64_t ntile, int64
   w.blockmap = (int32_t*)take((size_t)(d.NB[0] * d.NB[1] * d.NB[2]) * 4);
   w.tw = (float2*)take((size_t)d.fft_len * 8);
   w.ohat = (float2*)take((size_t)nsp * d.n_freq * 8);
-  w.qhat = (float2*)take((size_t)d.n_freq * ntile * RT_ROWS * d.n_phase * 8);
+  // a row of spectra: fp32 complex [phase], or fp16 hi / lo blocks (h16_kp halves)
+  const size_t row_bytes = (size_t)d.n_phase * 8 > (size_t)h16_kp(d) * 2 ? (size_t)d.n_phase * 8 : (size_t)h16_kp(d) * 2;
+  w.qhat = (float2*)take((size_t)d.n_freq * ntile * RT_ROWS * row_bytes);
   w.opart = (float2*)take((size_t)ntile * d.n_freq * npos * 8);
-  w.per_tile = (size_t)d.n_freq * (RT_ROWS * d.n_phase + npos) * 8;
+  w.rscale = (float*)take((size_t)ntile * RT_ROWS * 4);
+  w.per_tile = (size_t)d.n_freq * (RT_ROWS * row_bytes + npos * 8) + RT_ROWS * 4;
   w.total = o;
   return w;
 }
@@ -1112,6 +1267,11 @@ bool tred_mac_tc2_supported(const tred_ctx* ctx);
 int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float* Blo, const void* Bhb,
                  const void* Blb, float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2,
                  cudaStream_t st);
+
+// three fp16 products on CTA pairs, operands pre-split by the forward FFT (tred_mac_h3.cu)
+bool tred_mac_h3_supported(const tred_ctx* ctx);
+int tred_mac_h3(tred_ctx* ctx, const void* qh, const float* rscale, const void* Bh16, const float* bscale,
+                float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
 
 // mirror-symmetric response (tred_mac_tc2s.cu)
 bool tred_mac_tc2s_supported(const tred_ctx* ctx);
@@ -1163,6 +1323,11 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
   // (mac_mode 4 only: measured slower than the general product at config 3)
   const bool sym = ctx->cfg.mac_mode == 4 && ctx->sym_rhat == (const void*)d_rhat && g.nph == 100 &&
                    tred_mac_tc2s_supported(ctx) && fft_fwd_2s_available(g);
+  // default: three fp16 products, the forward FFT writes the operands already split
+  const bool h16 = (ctx->cfg.mac_mode == 0 || ctx->cfg.mac_mode == 7) && g.nph == 100 && (g.Bt & 3) == 0 &&
+                   tred_mac_h3_supported(ctx) && fft_fwd_2s_available(g);
+  if (ctx->cfg.mac_mode == 7 && !h16) return TRED_EUNSUPPORTED;
+  ctx->last_mac_mode = 0;
   int b0 = 0;
   while (b0 < g.NBt) {
     if (h_rt_off[b0 + 1] == h_rt_off[b0]) { ++b0; continue; }
@@ -1188,9 +1353,10 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{nullptr, 0, pw.rt_desc, pw.row_m2, t0, rg.nstrip, 1};
-        int ct = sym ? launch_fft_fwd_2s<true>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st)
-                     : launch_fft_fwd_2s<false>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
-        if (sym && ct == 0) return TRED_EUNSUPPORTED;
+        int ct = sym ? launch_fft_fwd_2s<1>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, nullptr, w.tw, st)
+               : h16 ? launch_fft_fwd_2s<2>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.rscale, w.tw, st)
+                     : launch_fft_fwd_2s<0>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, nullptr, w.tw, st);
+        if ((sym || h16) && ct == 0) return TRED_EUNSUPPORTED;
         if (ct == 0) ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.tw, st);
         if (ct < 0) return ct;
         if (ct == 0)
@@ -1205,14 +1371,24 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
           rc = tred_mac_tc2s(ctx, (const float*)w.qhat, d_rhat + rl.bs_hi, d_rhat + rl.bs_lo, d_rhat + rl.bd_hi,
                              d_rhat + rl.bd_lo, (float*)w.opart, nt, t0, pw.rt_desc, pw.row_m2, st);
           if (rc != TRED_OK) return rc;
-        } else if (ctx->cfg.mac_mode != 3 && tred_mac_tc2_supported(ctx))
+          ctx->last_mac_mode = 4;
+        } else if (h16) {
+          rc = tred_mac_h3(ctx, w.qhat, w.rscale, d_rhat + rl.b16, d_rhat + rl.bsc, (float*)w.opart, nt, t0,
+                           pw.rt_desc, pw.row_m2, st);
+          if (rc != TRED_OK) return rc;
+          ctx->last_mac_mode = 7;
+        } else if (ctx->cfg.mac_mode != 3 && tred_mac_tc2_supported(ctx)) {
+          ctx->last_mac_mode = ctx->cfg.mac_mode == 5 ? 5 : 6;
           rc = tred_mac_tc2(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl,
                             ctx->cfg.mac_mode != 5 ? (const void*)(d_rhat + rl.bhb) : nullptr,
                             ctx->cfg.mac_mode != 5 ? (const void*)(d_rhat + rl.blb) : nullptr, (float*)w.opart, nt,
                             t0, pw.rt_desc, pw.row_m2, st);
-        if (rc == TRED_EUNSUPPORTED)
+        }
+        if (rc == TRED_EUNSUPPORTED) {
+          ctx->last_mac_mode = 3;
           rc = tred_mac_tc_fused(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.opart, nt,
                                  t0, pw.rt_desc, pw.row_m2, st);
+        }
         if (rc != TRED_OK) return rc;
         TRED_COUNT_LAUNCH(1);
       }
@@ -1264,6 +1440,15 @@ extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* 
                                            reinterpret_cast<__nv_bfloat16*>(d_rhat + rl.blb),
                                            g.Tr, g.L, g.noff, g.kp, g.nph);
     TRED_COUNT_LAUNCH(1);
+  }
+  {
+    TredProfScope ps(ctx, ST_RESP, st);
+    float* bsc = d_rhat + rl.bsc;
+    k_resp_h16_scale<<<g.nf, 256, 0, st>>>((const float2*)d_rhat, bsc, g.nph, g.kp, g.noff);
+    const int64_t n = (int64_t)g.nf * g.nph * g.noff;
+    k_resp_h16<<<cdiv(n, 256), 256, 0, st>>>((const float2*)d_rhat, bsc, reinterpret_cast<__half*>(d_rhat + rl.b16),
+                                            g.nf, g.nph, g.noff, g.kp, h16_kp(ctx->dims));
+    TRED_COUNT_LAUNCH(2);
   }
   TRED_LAUNCH_CHECK("k_resp_dft64");
   // mirror-symmetric responses get the half-size matrices as well.  This
@@ -1440,7 +1625,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{d_cp_keys, r0, nullptr, nullptr, 0, 0, 0};
-        int ct = launch_fft_fwd_2s<false>(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
+        int ct = launch_fft_fwd_2s<0>(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, nullptr, w.tw, st);
         if (ct == 0) ct = launch_fft_fwd_ct(ctx, g, d_payload, w.blockmap, rs, nr, rp, w.qhat, w.tw, st);
         if (ct < 0) return ct;
         if (ct == 0)
@@ -1451,6 +1636,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
       {
         TredProfScope ps(ctx, ST_MAC, st);
         int rc = TRED_EUNSUPPORTED;
+        ctx->last_mac_mode = 2;
         if (ctx->cfg.mac_mode != 1)
           rc = tred_mac_tc(ctx, (const float*)w.qhat, d_rhat + wfl, d_rhat + wfl + bfl, (float*)w.T, nr, rp, st);
         if (rc == TRED_EUNSUPPORTED && ctx->cfg.mac_mode != 2) {
@@ -1459,6 +1645,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
           if (gy < 1) gy = 1;
           if (gy > ntile) gy = ntile;
           k_mac_fma<<<dim3(g.nf, gy), 256, mac_smem, st>>>(w.qhat, (const float2*)Wf, w.T, nr, rp, g);
+          ctx->last_mac_mode = 1;
           rc = TRED_OK;
         }
         if (rc != TRED_OK) return rc;

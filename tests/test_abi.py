@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(L, n), f"libtred.so does not export {n}"
     assert set(names) == set(pkg.EXPORTS), set(names) ^ set(pkg.EXPORTS)
-    assert L.tred_abi_version() == 1
+    assert L.tred_abi_version() == 2
     assert L.tred_strerror(-2).decode().startswith("capacity")
 
 

@@ -5,10 +5,14 @@ Tolerances (DESIGN.md "Tolerances"):
   integers (bbox, flags, block keys, CSR lists, slab/tile keys): bit-exact;
   effective charge (fp32 vs fp64): max|d| <= 2e-5 max|Qeff|, total within 1e-5;
   waveforms: max|d| <= 1e-4 max|signal| (north_star);
-  per-pixel integrated charge: |dQ_p| <= 1e-5 |Q_p| + 1e-6 * sum_t |I_p(t)|
-      (north_star's relative 1e-5 on the collected charge; induction-only pixels integrate
-       to ~0 by cancellation, where a relative bound is undefined, so the floor is 1e-6 of
-       the L1 norm of the pixel's own waveform -- DESIGN.md "Tolerances", reading G17).
+  per-pixel integrated charge (north_star: relative 1e-5):
+      collecting pixels (|Q_p| >= L1_p / 2, L1_p = sum_t |I_p(t)|: a mostly unipolar pulse, and
+      |Q_p| >= 1e-3 max|Q|):  |dQ_p| <= 1e-5 |Q_p|, nothing added;
+      every other pixel integrates a bipolar induction pulse to ~0 by cancellation, where a
+      relative bound is undefined (reading G17): |dQ_p| <= c 2^-24 L1_p with c from the error
+      model of DESIGN.md "Tolerances": c = 4 (fp32 rounding of samples, FFT passes, gather) for
+      the fp32 FMA product, plus 3/16 per truncating tensor-core accumulation of the product
+      that ran (75 for the tf32 products, 52 for tf32 + 2 x bf16, 39 for the three fp16 products).
 """
 import numpy as np
 import pytest
@@ -21,7 +25,13 @@ pytestmark = pytest.mark.gpu
 TOL_QEFF = 2e-5
 TOL_WAVE = 1e-4
 TOL_QPIX = 1e-5
-TOL_QPIX_L1 = 1e-6
+# tensor-core accumulations per output value by spectrum-product kernel (tred_last_mac_mode);
+# K2 = 200 reals per row: 25 K-steps of 8 (tf32) or 13 of 16 (bf16 / fp16), three products
+N_ACC = {1: 0, 2: 75, 3: 75, 4: 75, 5: 75, 6: 52, 7: 39}
+
+
+def tol_qpix_l1(mode):
+    return (4.0 + 0.1875 * N_ACC[mode]) * 2.0 ** -24
 
 
 def _torch():
@@ -214,13 +224,17 @@ def test_effq_point_like_and_clipped_segments(effq_mode):
 
 
 # ------------------------------------------------------------------ S4 + S5
-def _wave_checks(got, ref):
+def _wave_checks(got, ref, mode):
+    """`mode`: the spectrum-product kernel that ran (Tred.last_mac_mode())."""
     scale = np.abs(ref).max()
     assert scale > 0
     assert np.abs(got - ref).max() <= TOL_WAVE * scale
     qg, qr = got.sum(1), ref.sum(1)
     l1 = np.abs(ref).sum(1)
-    assert (np.abs(qg - qr) <= TOL_QPIX * np.abs(qr) + TOL_QPIX_L1 * l1).all()
+    dq = np.abs(qg - qr)
+    coll = (np.abs(qr) >= 0.5 * l1) & (np.abs(qr) >= 1e-3 * np.abs(qr).max())
+    assert (dq[coll] <= TOL_QPIX * np.abs(qr)[coll]).all(), (dq[coll] / np.abs(qr)[coll]).max()
+    assert (dq[~coll] <= tol_qpix_l1(mode) * l1[~coll]).all(), (dq[~coll] / l1[~coll]).max() * 2.0 ** 24
     # pixels the oracle leaves exactly empty stay exactly empty
     assert (got[l1 == 0] == 0).all()
 
@@ -280,11 +294,12 @@ def _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix, work_bytes=Non
     return dense.cpu().numpy()
 
 
-@pytest.mark.parametrize("mac_mode", [1, 0, 2, 3, 4, 5])
+@pytest.mark.parametrize("mac_mode", [1, 0, 2, 3, 4, 5, 6, 7])
 @pytest.mark.parametrize("cfg_id", [1, 2, 3])
 def test_convolve_parity_from_oracle_charge(cfg_id, mac_mode):
     """S4+S5 alone: the GPU convolves the ORACLE's effective charge (cast to fp32).
-    mac_mode 1: fp32 FMA spectrum product; 0: library default (tensor cores if available)."""
+    mac_mode 1: fp32 FMA spectrum product; 0: library default (7 on a B200: three fp16 products);
+    the others: include/tred.h.  The kernel that ran is the one asked for (no silent fallback)."""
     torch = _torch()
     cfg, segs = _small(cfg_id)
     cfg = cfg.with_(mac_mode=mac_mode)
@@ -300,7 +315,9 @@ def test_convolve_parity_from_oracle_charge(cfg_id, mac_mode):
     sim = _sim(cfg)
     rhat = sim.prepare_response(torch.from_numpy(R).cuda())
     got = _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix)
-    _wave_checks(got.astype(np.float64), ref)
+    # mode 4 needs a mirror-symmetric response (this one is) and 100 phases
+    assert sim.last_mac_mode() == (7 if mac_mode == 0 else mac_mode)
+    _wave_checks(got.astype(np.float64), ref, sim.last_mac_mode())
 
 
 @pytest.mark.parametrize("block,tr", [((4, 4, 32), 200), ((8, 8, 64), 137), ((16, 16, 128), 400),
@@ -347,7 +364,7 @@ def test_end_to_end_parity(cfg_id):
     assert out["nblocks"] == len(keys) and out["ntiles"] == len(tiles)
     np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
     got = out["dense"].cpu().numpy().astype(np.float64)
-    _wave_checks(got, ref)
+    _wave_checks(got, ref, sim.last_mac_mode())
     # the sparse tiles hold the same numbers as the dense rows
     tk = out["tile_keys"].cpu().numpy()
     td = out["tile_data"].cpu().numpy()
@@ -428,7 +445,7 @@ def test_chunked_equals_single_pass(cfg_id):
     ref = o.conv_fft(cfg, keys, payload, R, pix)
     c = sim.simulate_chunked(seg, rhat, pix_ids=torch.from_numpy(pix.astype(np.int32)).cuda(),
                              payload_budget_bytes=max(a["nblocks"] // 5, 1) * blk)
-    _wave_checks(c["dense"].cpu().numpy().astype(np.float64), ref)
+    _wave_checks(c["dense"].cpu().numpy().astype(np.float64), ref, sim.last_mac_mode())
 
 
 # ------------------------------------------------------------------ N2: G4Step preprocessing
@@ -531,7 +548,7 @@ def test_full_size_config3_sampled_pixels():
         sel = o.segments_touching(cfg, aug, kk)
         payload = o.effq(cfg, aug, kk, sel)
         ref = o.conv_fft(cfg, kk, payload, R, grp)
-        _wave_checks(dense[3 * gi: 3 * gi + 3], ref)
+        _wave_checks(dense[3 * gi: 3 * gi + 3], ref, sim.last_mac_mode())
         # effective charge of the same blocks
         got_q = out["payload"][torch.from_numpy(np.flatnonzero(m)).cuda()].cpu().numpy().astype(np.float64)
         assert np.abs(got_q - payload).max() <= TOL_QEFF * np.abs(payload).max()
