@@ -359,6 +359,12 @@ int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, const int32_t* 
  * s < tred_stage_count().  h_ms / h_launches: HOST arrays of nstage entries.
  */
 int tred_profile_begin(tred_ctx* ctx, int record_events);
+/* Measurement aid, not part of the path: enqueues one kernel of nothing but independent fp32
+ * FMA chains (8 per thread, 64 x iters FMAs each, 8 CTAs of 256 threads per SM) and writes the
+ * floating-point operations it executes to *h_flops (host).  Timed by the caller (CUDA events
+ * on `stream`) it gives the fp32 FMA rate this device sustains, the peak of the "alu"
+ * rooflines.  d_out: at least one float of device memory. */
+int tred_bench_fma(tred_ctx* ctx, int32_t iters, float* d_out, double* h_flops, void* stream);
 int tred_profile_end(tred_ctx* ctx, int nstage, float* h_ms, int64_t* h_launches);
 int tred_stage_count(void);
 const char* tred_stage_name(int stage);

@@ -98,6 +98,7 @@ EXPORTS = {
     "tred_truth": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_profile_begin": (C.c_int, [_c_p, C.c_int]),
     "tred_profile_end": (C.c_int, [_c_p, C.c_int, _c_p, _c_p]),
+    "tred_bench_fma": (C.c_int, [_c_p, C.c_int32, _c_p, C.POINTER(C.c_double), _c_p]),
     "tred_stage_count": (C.c_int, []),
     "tred_stage_name": (C.c_char_p, [C.c_int]),
 }
@@ -273,6 +274,21 @@ class Tred:
         ln = (C.c_int64 * n)()
         _check(self.L.tred_profile_end(self.h, n, C.cast(ms, _c_p), C.cast(ln, _c_p)), "tred_profile_end")
         return {self.L.tred_stage_name(i).decode(): (float(ms[i]), int(ln[i])) for i in range(n)}
+
+    def bench_fma(self, iters: int = 4096, reps: int = 5) -> float:
+        """Measured fp32 FMA rate of this device in TFLOP/s (best of `reps`, CUDA events)."""
+        t = self.torch
+        out = self._empty((1,), t.float32)
+        fl = C.c_double(0.0)
+        best = 0.0
+        for _ in range(reps + 1):
+            a, b = t.cuda.Event(enable_timing=True), t.cuda.Event(enable_timing=True)
+            a.record()
+            _check(self.L.tred_bench_fma(self.h, iters, _ptr(out), C.byref(fl), self._stream()), "tred_bench_fma")
+            b.record()
+            b.synchronize()
+            best = max(best, fl.value / (a.elapsed_time(b) * 1e-3) / 1e12)
+        return best
 
     def last_mac_mode(self) -> int:
         """The spectrum-product kernel (tred_config.mac_mode value 1..7) the last convolve launched."""

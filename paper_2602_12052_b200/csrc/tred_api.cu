@@ -69,6 +69,36 @@ extern "C" int tred_profile_end(tred_ctx* c, int nstage, float* h_ms, int64_t* h
   return TRED_OK;
 }
 
+// ------------------------------------------------------------------ fp32 FMA peak (measurement aid)
+// 8 independent FMA chains per thread, nothing else in the loop: what the fp32 pipes of
+// this device sustain, the denominator bench.py uses for the "alu" rooflines.
+__global__ void __launch_bounds__(256) k_bench_fma(int iters, float seed, float* __restrict__ out) {
+  float a[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) a[j] = seed + (float)(threadIdx.x + j);
+  const float m = 1.0f - 1e-7f * seed, c = 1e-3f;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = fmaf(a[j], m, c);
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) s += a[j];
+  if (s == 12345.678f) out[0] = s;                   // keeps the chains alive
+}
+
+extern "C" int tred_bench_fma(tred_ctx* ctx, int32_t iters, float* d_out, double* h_flops, void* stream) {
+  if (!ctx || iters < 1 || !d_out) return TRED_EINVAL;
+  const int blocks = ctx->num_sms * 8;
+  k_bench_fma<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, 1.0f, d_out);
+  TRED_COUNT_LAUNCH(1);
+  TRED_LAUNCH_CHECK("k_bench_fma");
+  if (h_flops) *h_flops = 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
+  return TRED_OK;
+}
+
 extern "C" int tred_stage_count(void) { return ST_COUNT; }
 
 extern "C" const char* tred_stage_name(int s) {

@@ -19,7 +19,10 @@
 // the stage goes from TMA straight to the tensor core.
 //
 // Per CTA: warp 0 TMA producer (own A tile, own half of B), warp 1 MMA issuer (leader CTA
-// only), warps 2-5 epilogue.  Barriers: `full` lives in the leader: both CTAs' producers
+// only), warps 2-5 and 6-9 two epilogue sets: set s owns TMEM accumulator s (the items of
+// the cluster alternate between the two) and its own four patch copies, so the epilogue of
+// an item has two MMA periods to finish (its chain of shared-memory read-modify-writes takes
+// longer than one).  Barriers: `full` lives in the leader: both CTAs' producers
 // arrive on it with their byte counts and both CTAs' TMA loads (cta_group::2) complete on it,
 // so the MMA issuer waits on one barrier per stage; empty / tfull are local to each CTA and
 // arrive through tcgen05.commit multicast; tempty lives in the leader, one arrival per CTA.
@@ -28,12 +31,12 @@
 
 namespace {
 
-constexpr int H3_STAGES = 5;
+constexpr int H3_STAGES = 4;
 constexpr int H3_A_BYTES = T2_M * 128;                   // 128 rows x 128 bytes
 constexpr int H3_B_BYTES = (T2_NMAX / 2) * 128;          // this CTA's half of B
 constexpr int H3_STAGE_BYTES = H3_A_BYTES + H3_B_BYTES;  // 32 KB
-constexpr int H3_THREADS = 192;
-constexpr size_t H3_SMEM = (size_t)H3_STAGES * H3_STAGE_BYTES + 1024 + 256 + 4 * T2_PATCH_FLOAT2 * 8;
+constexpr int H3_THREADS = 320;
+constexpr size_t H3_SMEM = (size_t)H3_STAGES * H3_STAGE_BYTES + 1024 + 256 + 8 * T2_PATCH_FLOAT2 * 8;
 
 struct H3Maps { CUtensorMap a, b; };
 
@@ -182,13 +185,17 @@ k_mac_h3(const __grid_constant__ H3Maps tm, H3Params p) {
   } else {
     // ------------------------------------------------------------ epilogue: sum over offsets
     const int q = warp & 3;
-    const int et = threadIdx.x - 64;
-    float2* patch = reinterpret_cast<float2*>(base_ptr + H3_STAGES * H3_STAGE_BYTES + 256);
+    const int es = (warp - 2) >> 2;                               // epilogue set = accumulator
+    const int et = (threadIdx.x - 64) & 127;
+    const uint32_t ebar = 1 + es;                                  // named barrier of the set
+    float2* patch = reinterpret_cast<float2*>(base_ptr + H3_STAGES * H3_STAGE_BYTES + 256) + es * 4 * T2_PATCH_FLOAT2;
     float2* P = patch + q * T2_PATCH_FLOAT2;
     for (int i = et; i < 4 * T2_PATCH_FLOAT2; i += 128) patch[i] = make_float2(0.0f, 0.0f);
-    asm volatile("bar.sync 1, 128;" ::: "memory");
+    asm volatile("bar.sync %0, 128;" ::"r"(ebar) : "memory");
     const int PX = RT_SW + 2 * p.H;
-    int as = 0, aphase = 0;
+    const int as = es;
+    int aphase = 0;
+    const int first = cid + es * ncl, stride = 2 * ncl;            // this set's items
     // Row tile descriptor and this thread's row record are fetched one / two items ahead
     // (two dependent global loads otherwise sit on the epilogue's critical path).
     auto item_tile = [&](int it) { return it < nitems ? 2 * (it % p.npair) + (int)rank : p.ntile; };
@@ -197,10 +204,10 @@ k_mac_h3(const __grid_constant__ H3Maps tm, H3Params p) {
       return t < p.ntile ? p.rt_desc[p.t0 + t] : make_int4(0, 0, 0, 0);
     };
     const int r = q * 32 + lane;
-    int4 d_cur = load_desc(cid), d_nxt = load_desc(cid + ncl);
+    int4 d_cur = load_desc(first), d_nxt = load_desc(first + stride);
     int m2_cur = r < d_cur.y ? p.row_m2[d_cur.x + r] : 0;
-    float rs_cur = r < d_cur.y ? p.rscale[item_tile(cid) * T2_M + r] : 0.0f;
-    for (int item = cid; item < nitems; item += ncl) {
+    float rs_cur = r < d_cur.y ? p.rscale[item_tile(first) * T2_M + r] : 0.0f;
+    for (int item = first; item < nitems; item += stride) {
       const int f = item / p.npair, pr = item - f * p.npair;
       const int mt = 2 * pr + (int)rank;
       const bool has_tile = mt < p.ntile;
@@ -209,8 +216,8 @@ k_mac_h3(const __grid_constant__ H3Maps tm, H3Params p) {
       const float sc = rs_cur * __ldg(p.bscale + f);
       // prefetch: record of the next item (its descriptor arrived an iteration ago), descriptor of the one after
       const int m2_nxt = r < d_nxt.y ? p.row_m2[d_nxt.x + r] : 0;
-      const float rs_nxt = r < d_nxt.y ? p.rscale[item_tile(item + ncl) * T2_M + r] : 0.0f;
-      const int4 d_nn = load_desc(item + 2 * ncl);
+      const float rs_nxt = r < d_nxt.y ? p.rscale[item_tile(item + stride) * T2_M + r] : 0.0f;
+      const int4 d_nn = load_desc(item + 2 * stride);
       const bool valid = r < d.y;
       const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
       const int yl = (m2 >> 3) % p.npy - d.z;
@@ -294,9 +301,9 @@ k_mac_h3(const __grid_constant__ H3Maps tm, H3Params p) {
       }
       d_cur = d_nxt; d_nxt = d_nn; m2_cur = m2_nxt; rs_cur = rs_nxt;
       tc_fence_before();
-      asm volatile("bar.sync 1, 128;" ::: "memory");
+      asm volatile("bar.sync %0, 128;" ::"r"(ebar) : "memory");
       if (et == 0) mbar_arrive_cluster(mapa(tempty_bar(as), 0));   // this CTA's accumulator is free
-      if (++as == 2) { as = 0; aphase ^= 1; }
+      aphase ^= 1;
       if (has_tile) {
         const int nyp = d.w + 2 * p.H, ncell = PX * nyp;
         float2* dst = p.opart + ((int64_t)mt * p.nf + f) * (PX * RT_PY);
@@ -314,7 +321,7 @@ k_mac_h3(const __grid_constant__ H3Maps tm, H3Params p) {
           dst[X * RT_PY + Y] = a;
         }
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");
+      asm volatile("bar.sync %0, 128;" ::"r"(ebar) : "memory");
     }
   }
   tc_fence_before();

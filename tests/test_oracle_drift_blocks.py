@@ -4,6 +4,7 @@ import math
 import os
 
 import numpy as np
+import pytest
 
 import gen
 import oracle as o
@@ -142,3 +143,38 @@ def test_paper_padding_example():
             while n < exact:
                 n *= 2
             assert n == pow2
+
+
+@pytest.mark.parametrize("tr", [65, 66])
+def test_out_tiles_exact_by_brute_force(tr):
+    """O6 pinned to equality: blocks filled with ones, a response of ones on every offset, phase
+    and tick, direct sum of Eq. (12).  Everything is positive, so the support of
+    the current IS the output footprint of the blocks, and its tiles must EQUAL the list -- no
+    tile too few and none too many.  Bt = 64: with Tr = 65 a block's last output tick
+    Bt bt + Bt + Tr - 2 is the last tick of tile bt + 1, with Tr = 66 the first tick of tile
+    bt + 2; a footprint one tick too long or too short fails one of the two.  The blocks include
+    ones that straddle two pixels (8 fine points per block, 10 per pixel), ones at the plane's
+    rim and one whose output runs past the readout window."""
+    cfg = gen.make_config(1).with_(npix_x=12, npix_y=10, nticks=400, resp_nticks=tr, resp_half=1)
+    g = o.grid_of(cfg)
+    assert g.B == (8, 8, 64) and cfg.sub == 10
+    blocks = [(0, 0, 0), (1, 5, 0), (6, 3, 1), (14, 12, 2), (7, 7, 3), (3, 9, 5), (9, 2, 6)]
+    keys = np.array(sorted((bt * g.NB[0] + bx) * g.NB[1] + by for bx, by, bt in blocks), dtype=np.int64)
+    payload = np.ones((len(keys),) + tuple(g.B))
+    K = 2 * cfg.resp_half + 1
+    R = np.ones((cfg.sub, cfg.sub, K, K, tr), dtype=np.float32)
+    pix = np.arange(cfg.npix_x * cfg.npix_y, dtype=np.int64)
+    wave = o.conv_direct(cfg, keys, payload, R, pix)
+    nz = np.argwhere(wave > 0)
+    brute = np.unique((nz[:, 1] // g.B[2]) * (cfg.npix_x * cfg.npix_y) + nz[:, 0])
+    np.testing.assert_array_equal(o.out_tiles(cfg, keys), brute)
+    # the support itself, per block, is the stated box (pixels and ticks), not just its tiles
+    bx, by, bt = o.key_to_bxyz(g, keys[:1])
+    on = np.zeros_like(wave, dtype=bool)
+    for x, y, t in blocks:
+        px0, px1 = max(8 * x // 10 - 1, 0), min((8 * x + 7) // 10 + 1, cfg.npix_x - 1)
+        py0, py1 = max(8 * y // 10 - 1, 0), min((8 * y + 7) // 10 + 1, cfg.npix_y - 1)
+        t1 = min(64 * t + 64 + tr - 2, cfg.nticks - 1)
+        for px in range(px0, px1 + 1):
+            on[px * cfg.npix_y + py0: px * cfg.npix_y + py1 + 1, 64 * t: t1 + 1] = True
+    np.testing.assert_array_equal(wave > 0, on)

@@ -59,3 +59,50 @@ def test_records_add_up_to_the_collected_charge():
     last = rk // npix
     assert (last.max() + 1) * cfg.block[2] + cfg.resp_nticks <= cfg.nticks      # nothing truncated in time
     assert np.allclose(sim["wave"].sum(1), per_pixel[pix], rtol=1e-6)
+
+
+def test_record_keys_by_dense_box_sums_and_arrival_tick():
+    """The (pixel, time tile) index of every entry, pinned twice without truth_record's own
+    per-block bookkeeping: (1) the segment's effective charge scattered onto the dense fine
+    grid and summed over S x S x Bt boxes by a reshape gives the same keys and the same charges;
+    (2) the tile that books most of a segment's charge is the one holding its arrival tick
+    (z / v - t_origin) / tick (reading G11) whenever the charge cloud lies well
+    inside that tile."""
+    cfg, segs = gen.make_segments(1)
+    cfg = cfg.with_(npix_x=16, npix_y=16, nticks=512)
+    segs = {k: v[40:64].copy() for k, v in segs.items()}
+    for a in ("x", "y"):                               # move the piece of track into the small plane
+        sh = 35.0 - segs[a + "0"][0]
+        segs[a + "0"] = (segs[a + "0"] + sh).astype(np.float32)
+        segs[a + "1"] = (segs[a + "1"] + sh).astype(np.float32)
+    zs = 120.0 - segs["z0"][0]
+    segs["z0"] = (segs["z0"] + zs).astype(np.float32)
+    segs["z1"] = (segs["z1"] + zs).astype(np.float32)
+    cfg = cfg.with_(t_origin_us=float(segs["z0"].min() / cfg.v_mm_us - 8.0))
+    aug = o.drift(cfg, segs)
+    rs, rk, rq = o.truth_record(cfg, aug)
+    g = o.grid_of(cfg)
+    S, Bt = cfg.sub, cfg.block[2]
+    npix = cfg.npix_x * cfg.npix_y
+    ntb = g.NG[2] // Bt
+    keys = o.blocks(cfg, aug)
+    checked = dominant = 0
+    for s in range(len(aug["Qp"])):
+        dense = o.payload_to_dense(cfg, keys, o.effq(cfg, aug, keys, [s]))
+        box = dense.reshape(cfg.npix_x, S, cfg.npix_y, S, ntb, Bt).sum((1, 3, 5))      # [px][py][tb]
+        ref = {(tb * cfg.npix_x + px) * cfg.npix_y + py: box[px, py, tb] for px, py, tb in np.argwhere(box != 0)}
+        got = dict(zip(rk[rs == s].tolist(), rq[rs == s].tolist()))
+        # an entry may be an exact zero (a footprint cell the 4-sigma box reaches with underflow); not vice versa
+        assert set(ref) <= set(got)
+        for k, v in got.items():
+            assert abs(v - ref.get(k, 0.0)) <= 1e-12 * max(abs(v), 1e-300) + 1e-300
+        checked += len(ref)
+        # (2) arrival tick of the segment's midpoint, cloud (4 sigma + half length) inside one tile
+        tick_mid = (0.5 * (aug["p0"][s, 2] + aug["p1"][s, 2]) - cfg.t_origin_us) / cfg.tick_us
+        half = 0.5 * abs(aug["p1"][s, 2] - aug["p0"][s, 2]) / cfg.tick_us + cfg.nsigma * aug["sig"][s, 2] / cfg.tick_us
+        tb = int(tick_mid // Bt)
+        if tick_mid - half > tb * Bt + 1 and tick_mid + half < (tb + 1) * Bt - 1:
+            per_tb = np.bincount(rk[rs == s] // npix, weights=rq[rs == s], minlength=ntb)
+            assert per_tb.argmax() == tb and per_tb[tb] >= (1 - 1e-3) * per_tb.sum()
+            dominant += 1
+    assert checked > 50 and dominant >= 5
