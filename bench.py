@@ -103,19 +103,39 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def _load_traffic(workload_name: str) -> dict:
+def csrc_sha() -> str:
+    """sha1 over the CUDA sources and the header: the code state a profile belongs to."""
+    import hashlib
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2602_12052_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+    h.update(open(os.path.join(ROOT, "include", "tred.h"), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def _load_traffic(workload_name: str):
     """DRAM bytes per step and stage from the committed ncu --set full capture
-    (profiles/traffic.csv: workload,stage,dram_bytes_per_step); {} if there is none."""
-    out = {}
+    (profiles/traffic.csv: a `# csrc_sha=<hash>` line, then workload,stage,dram_bytes_per_step).
+    The capture belongs to one state of the kernels: if csrc/ has changed since, the numbers
+    are refused ({} and the reason)."""
+    out, sha = {}, None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for line in f:
+                if line.startswith("#"):
+                    if "csrc_sha=" in line:
+                        sha = line.split("csrc_sha=")[1].split()[0]
+                    continue
                 p = [x.strip() for x in line.split(",")]
                 if len(p) >= 3 and p[0] == workload_name:
                     out[p[1]] = float(p[2])
     except (OSError, ValueError):
-        pass
-    return out
+        return {}, "no profiles/traffic.csv"
+    if sha != csrc_sha():
+        return {}, f"profiles/traffic.csv was captured at csrc_sha {sha}, the sources are now {csrc_sha()}: refused"
+    return out, f"ncu --set full capture at csrc_sha {sha} (profiles/traffic.csv)"
 
 
 # --------------------------------------------------------------------------- oracle legs
@@ -169,24 +189,37 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- CUDA arm
-def run_cuda(args):
+MAC_KERNELS = {   # tred_last_mac_mode -> (arithmetic of the spectrum product, tensor-core products per fp32 product,
+                  #                        rate of those products relative to the bf16 / fp16 dense peak)
+    1: ("fp32 FMA", 0, 0.0),
+    2: ("3xTF32 split (tf32 tensor cores, fp32 accumulate), products in memory", 3.0, 0.5),
+    3: ("3xTF32 split (tf32 tensor cores, fp32 accumulate)", 3.0, 0.5),
+    4: ("3xTF32 split on mirror-pair sums / differences", 1.5, 0.5),
+    5: ("3xTF32 split (tf32 tensor cores, fp32 accumulate)", 3.0, 0.5),
+    6: ("tf32 + 2 x bf16 split (fp32 accumulate)", 2.0, 0.5),
+    7: ("3 x fp16 split, x = s (hi + lo) with power-of-two scales (fp32 accumulate)", 3.0, 1.0),
+}
+
+
+def measure(args, cfg_id, rank, world, dev, steps, stages: bool):
+    """Times one workload: device-resident inputs (CUDA events), per-stage events, and end to
+    end through tred_simulate with pinned HOST buffers on both sides."""
     import torch
     import torch.distributed as dist
     from paper_2602_12052_b200 import Tred
 
-    world = _env_int("WORLD_SIZE", 1)
-    rank = _env_int("RANK", 0)
-    local = _env_int("LOCAL_RANK", 0)
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    cfg, segs, seg_h, R = workload(args.config, rank)
+    cfg, segs, seg_h, R = workload(cfg_id, rank)
     if args.mac_mode:
         cfg = cfg.with_(mac_mode=args.mac_mode)
     nseg = seg_h.shape[1]
-    sim = Tred(cfg, device=dev, conv_work_bytes=args.work_gb << 30 if args.work_gb else None)
+    conv_cap = None
+    budget = 0
+    if cfg_id == 4:                         # device-memory-bounded chunks of occupied blocks (peak <= 40 GB)
+        conv_cap = (args.work_gb or 5) << 30
+        budget = args.budget_gb << 30
+    elif args.work_gb:
+        conv_cap = args.work_gb << 30
+    sim = Tred(cfg, device=dev, conv_work_bytes=conv_cap)
     rhat = sim.prepare_response(torch.from_numpy(R).to(dev))       # once per response (PAPER.md:L230)
     seg_d = torch.from_numpy(seg_h).to(dev)
     seg_pinned = torch.from_numpy(seg_h).pin_memory()
@@ -198,33 +231,22 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # config 4: device-memory-bounded chunks of occupied blocks (peak <= 40 GB)
-    if args.config == 4:
-        sim.conv_work_bytes = (args.work_gb or 5) << 30
+    def simulate(s, **kw):
+        return sim.simulate(s, rhat, payload_budget_bytes=budget, **kw)
 
-        def simulate(s):
-            return sim.simulate_chunked(s, rhat, payload_budget_bytes=args.budget_gb << 30)
-    else:
-        def simulate(s):
-            return sim.simulate(s, rhat)
-
-    # ---- warm-up
     out = None
     for _ in range(max(args.warmup, 3)):
         out = None                          # a step's outputs are released before the next step
         out = simulate(seg_d)
     barrier()
-    info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles", "nrt")}
-    # Gauss-Legendre node evaluations of one step = cuboids of every bounding box x n^3
-    _, augi0, _ = sim.drift(seg_d)
-    ext = (augi0[3:6] - augi0[0:3] + 1).to(torch.float64)
-    info["gl_nodes"] = float((ext[0] * ext[1] * ext[2]).sum().item()) * cfg.gl_n ** 3
+    info = {k: out[k] for k in ("npairs", "nblocks", "ncp", "nsp", "ntiles", "nrt", "nchunks", "host_reads")}
+    mac_mode = out["mac_mode"]
 
     # ---- timed region 1: inputs resident in HBM, device time by CUDA events
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(dev.index or 0)
     sampler.start()
     sim.profile_begin(events=False)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     barrier()
     t_wall0 = time.perf_counter()
     torch.cuda.reset_peak_memory_stats(dev)
@@ -238,59 +260,102 @@ def run_cuda(args):
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
     peak_mem = torch.cuda.max_memory_allocated(dev)
-    nchunks = len(out.get("chunks", [])) or 1
     out = None
     launches = sum(v[1] for v in sim.profile_end().values())
-    ms_steps = [a.elapsed_time(b) for a, b in ev]
-    ms = float(np.mean(ms_steps))
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
 
-    # ---- timed region 2: per-stage events (roofline of the dominant kernel)
-    stage_ms = {}
-    stage_prof_last = {}
-    for _ in range(args.steps):
-        flush.zero_()
-        sim.profile_begin(events=True)
-        simulate(seg_d)
-        torch.cuda.synchronize()
-        stage_prof_last = sim.profile_end()
-        for k, (m, n) in stage_prof_last.items():
-            stage_ms[k] = stage_ms.get(k, 0.0) + m / args.steps
-    barrier()
+    # ---- timed region 2: per-stage events
+    stage_ms, stage_n = {}, {}
+    if stages:
+        for _ in range(steps):
+            flush.zero_()
+            sim.profile_begin(events=True)
+            simulate(seg_d)
+            torch.cuda.synchronize()
+            for k, (m, n) in sim.profile_end().items():
+                stage_ms[k] = stage_ms.get(k, 0.0) + m / steps
+                stage_n[k] = n
+        barrier()
 
-    # ---- timed region 3: end to end through the public API with HOST buffers: segments from
-    # pinned host memory in, tile keys and waveform tiles back to pinned host memory
-    e2e_ms = []
-    h2d = seg_pinned.numel() * 4
-    d2h = 0
-    o2 = None
+    # ---- timed region 3: end to end through the C-ABI call with HOST buffers: segments from
+    # pinned host memory in, tile keys and waveform tiles written to pinned host memory
     nt_cap = int(info["ntiles"] * 1.05) + 1024
     keys_h = torch.empty((nt_cap,), dtype=torch.int64).pin_memory()
     data_h = torch.empty((nt_cap, cfg.block[2]), dtype=torch.float32).pin_memory()
-    for i in range(args.steps + 1):
-        o2 = None
+    e2e_ms = []
+    for i in range(steps + 1):
         flush.zero_()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        sd = seg_pinned.to(dev, non_blocking=True)
-        o2 = simulate(sd)
-        nt = o2["ntiles"]
-        if nt > nt_cap:                     # cannot happen for a fixed workload; keep the copy honest anyway
-            keys_h = torch.empty((nt,), dtype=torch.int64).pin_memory()
-            data_h = torch.empty((nt, cfg.block[2]), dtype=torch.float32).pin_memory()
-            nt_cap = nt
-        keys_h[:nt].copy_(o2["tile_keys"], non_blocking=True)
-        data_h[:nt].copy_(o2["tile_data"], non_blocking=True)
+        o2 = simulate(seg_pinned, host_out=(keys_h, data_h))
         torch.cuda.synchronize()
         if i > 0:
             e2e_ms.append(1e3 * (time.perf_counter() - t0))
-        d2h = nt * 8 + nt * cfg.block[2] * 4
     e2e = float(np.mean(e2e_ms))
-    o2 = None
+    h2d = seg_pinned.numel() * 4
+    d2h = o2["ntiles"] * 8 + o2["ntiles"] * cfg.block[2] * 4
     barrier()
+    return dict(cfg=cfg, segs=segs, R=R, sim=sim, nseg=nseg, info=info, mac_mode=mac_mode, ms=ms, e2e=e2e, h2d=h2d,
+                d2h=d2h, launches=int(launches) // max(steps, 1), clocks=clocks, peak_mem=peak_mem, t_wall=t_wall,
+                stage_ms=stage_ms, stage_n=stage_n, seg_d=seg_d, rhat=rhat)
+
+
+def cufft_s4_comparison(torch, m, rows_sample: int = 8192):
+    """Timed comparison only (north_star (d); PAPER.md:L230, L264 is this form): S4 with library
+    FFTs -- torch.fft.rfft (cuFFT) of the zero-padded time columns of a sample of charge pixels,
+    the per-frequency product with the precomputed response spectrum as a batched complex
+    matrix product (cuBLAS), the inverse cuFFT of the products -- extrapolated to the event by
+    the number of charge pixels.  The overlap-add over the offsets is not included (lower bound)."""
+    cfg, sim, info = m["cfg"], m["sim"], m["info"]
+    dev = m["seg_d"].device
+    d = sim.dims
+    L, nph, noff = d.fft_len, d.n_phase, d.n_off
+    n = min(rows_sample, max(info["ncp"], 1))
+    q = torch.rand((n, nph, cfg.block[2]), dtype=torch.float32, device=dev)       # same shape as the payload columns
+    W = torch.randn((L // 2 + 1, nph, noff), dtype=torch.complex64, device=dev)    # stands in for FFT(R^j), precomputed
+    ms = []
+    for i in range(4):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        qh = torch.fft.rfft(q, n=L, dim=2)                            # [n][phase][f]
+        T = torch.matmul(qh.permute(2, 0, 1), W)                      # [f][n][off]
+        o = torch.fft.irfft(T.permute(1, 2, 0), n=L, dim=2)          # [n][off][L]
+        b.record()
+        torch.cuda.synchronize()
+        if i > 0:
+            ms.append(a.elapsed_time(b))
+        del qh, T, o
+    per_row = float(np.mean(ms)) / n
+    return {"impl": "torch.fft.rfft (cuFFT) + batched complex matmul (cuBLAS) + torch.fft.irfft, comparison only",
+            "rows_sampled": n, "ms_sample": float(np.mean(ms)), "ms_per_spill_extrapolated": per_row * info["ncp"],
+            "not_included": "overlap-add over the offsets, gather of the payload columns"}
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    world = _env_int("WORLD_SIZE", 1)
+    rank = _env_int("RANK", 0)
+    local = _env_int("LOCAL_RANK", 0)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    m = measure(args, args.config, rank, world, dev, args.steps, stages=True)
+    cfg, sim, info, nseg = m["cfg"], m["sim"], m["info"], m["nseg"]
+    stage_ms, clocks = m["stage_ms"], m["clocks"]
+    fma_tflops = sim.bench_fma()                                   # measured fp32 FMA rate of this device
+    # Gauss-Legendre node evaluations of one step = cuboids of every bounding box x n^3
+    _, augi0, _ = sim.drift(m["seg_d"])
+    ext = (augi0[3:6] - augi0[0:3] + 1).to(torch.float64)
+    info["gl_nodes"] = float((ext[0] * ext[1] * ext[2]).sum().item()) * cfg.gl_n ** 3
+    del augi0, ext
 
     # ---- max over ranks of the times, sum of the units (paper_2602_12052_b200/shard.py)
     from paper_2602_12052_b200.shard import reduce_timing
-    (ms_max, e2e_max), total_seg = reduce_timing([ms, e2e], nseg, device=dev)
+    (ms_max, e2e_max), total_seg = reduce_timing([m["ms"], m["e2e"]], nseg, device=dev)
 
     if rank == 0:
         d = sim.dims
@@ -299,83 +364,124 @@ def run_cuda(args):
             peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
         except Exception:
             pass
-        # per-stage rooflines: algorithmic work of the METHOD per step
-        # / CUDA-event time of the stage, against the measured peaks
+        # per-stage rooflines: ALGORITHMIC work of the method per step
+        # / CUDA-event time of the stage, against the measured peaks; `own_*`:
+        # the bytes this design moves in the stage (its intermediates included)
         nb = info["nblocks"]
         ncols = cfg.block[0] * cfg.block[1]
         K = 2 * cfg.resp_half + 1
-        nf, L = d.n_freq, d.fft_len
-        sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        nf, L, Bt = d.n_freq, d.fft_len, cfg.block[2]
         hbm = peaks.get("hbm_gbs", 6650.0)
-        hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650"
-        alu_peak = 148 * FMA_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12          # fp32 TFLOP/s at max clock
-        tf32_peak = peaks.get("bf16_tflops", 1590.0) * 0.5                     # guide: tf32 = bf16 / 2 nominal
+        hbm_src = "measured copy bandwidth (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
+        # tensor peak of the dtype the product runs in; the kernel is timed inside a long step: sustained figure
+        bf16 = peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1590.0))
+        bf16_src = ("measured cuBLAS bf16, sustained (MEASURED_PEAKS.json bf16_tflops_sustained)"
+                    if "bf16_tflops_sustained" in peaks else "fallback")
+        mac_name, nprod, rel_rate = MAC_KERNELS.get(m["mac_mode"], ("?", 0, 0.0))
         fftf = 2.5 * L * np.log2(L)                                            # flops of one real FFT of length L
         payload_b = nb * d.block_floats * 4.0
-        spd_b = info["nsp"] * d.n_over * cfg.block[2] * 4.0
-        work = {
-            "effq": ("hbm", payload_b + nseg * 104.0),
-            "fft_fwd": ("alu", nb * ncols * fftf),
-            "mac": ("tensor" if sim.cfg.mac_mode != 1 else "alu", nb * ncols * K * K * (8.0 * (nf - 1) + 4.0)),
-            "accum": ("hbm", info["nsp"] * nf * 8.0),
-            "ifft": ("alu", info["nsp"] * fftf),
-            "gather": ("hbm", spd_b + info["ntiles"] * cfg.block[2] * 4.0),
+        rows_pad = info["nrt"] * 128
+        row_b = max(d.n_phase * 8, ((2 * d.n_phase + 15) // 16) * 32 * 2)      # a row of spectra: fp32 complex or fp16 hi/lo
+        qhat_b = rows_pad * nf * row_b * 1.0
+        opart_b = info["nrt"] * nf * (8 + 2 * cfg.resp_half) * 64 * 8.0
+        ohat_b = info["nsp"] * nf * 8.0
+        spd_b = info["nsp"] * d.n_over * Bt * 4.0
+        tiles_b = info["ntiles"] * Bt * 4.0
+        mac_flops = nb * ncols * K * K * (8.0 * (nf - 1) + 4.0)
+        work = {   # stage: (bound, algorithmic work, own bytes)
+            "effq": ("hbm", payload_b + nseg * 104.0, payload_b + nseg * 104.0),
+            "fft_fwd": ("hbm", payload_b, payload_b + qhat_b),
+            "mac": ("tensor" if nprod else "alu", mac_flops, qhat_b + opart_b),
+            "accum": ("hbm", ohat_b, opart_b + 2 * ohat_b),
+            "ifft": ("hbm", ohat_b + spd_b, ohat_b + spd_b),
+            "gather": ("hbm", spd_b + tiles_b, spd_b + tiles_b),
         }
         pk = {"hbm": (hbm, "GB/s", 1e9, hbm_src),
-              "alu": (alu_peak, "TFLOP/s", 1e12, "derived: 148 SM x 128 lanes x 2 x sm_max_mhz (DESIGN.md)"),
-              "tensor": (tf32_peak, "TFLOP/s", 1e12,
-                         "tf32 dense = measured bf16_tflops x 1/2 (nominal ratio); the kernel executes one tf32 "
-                         "and two bf16 products per algorithmic fp32 product (2 tf32-equivalents), so 1/2 "
-                         "is its ceiling")}
-        nlaunch = {k: v[1] for k, v in stage_prof_last.items()}
-        traffic = _load_traffic(cfg.name)
+              "alu": (fma_tflops, "TFLOP/s", 1e12, "measured in this run: tred_bench_fma (independent fp32 FMA chains)"),
+              "tensor": (bf16 * rel_rate, "TFLOP/s", 1e12,
+                         f"{bf16_src} x {rel_rate} (rate of the product's tensor-core dtype relative to bf16 / fp16)")}
+        traffic, traffic_src = _load_traffic(cfg.name)
         stage_roof = {}
-        for k, (bound, w) in work.items():
+        for k, (bound, w, own) in work.items():
             if stage_ms.get(k, 0.0) <= 0:
                 continue
             peak, unit, sc, src = pk[bound]
-            nl = max(nlaunch.get(k, 1), 1)
-            ach = w / (stage_ms[k] * 1e-3) / sc
+            nl = max(m["stage_n"].get(k, 1), 1)
+            sec = stage_ms[k] * 1e-3
+            ach = w / sec / sc
             tr = traffic.get(k)
             stage_roof[k] = {"kernel": k, "bound": bound, "achieved": ach, "peak": peak, "unit": unit,
-                             "frac": ach / peak, "ms_per_launch": stage_ms[k] / nl, "launches_per_step": nl,
-                             "work_per_launch": w / nl, "peak_source": src,
-                             "traffic": (tr / nl) if tr else None}
-        if "mac" in stage_roof and stage_roof["mac"]["bound"] == "tensor":
-            # what the tensor cores execute: 3 products per fp32 product (tf32-equivalent: the two
-            # bf16 correction products of the default mode run at twice the tf32 rate and count
-            # half), row tiles of 128 rows (partly filled), 2 x 128 output columns for 2 x 121 offsets
-            nprod = 3.0 if sim.cfg.mac_mode in (2, 3, 4, 5) else 2.0
-            ex = nprod * 2.0 * info["nrt"] * 128 * (2 * d.n_off_pad) * (2 * d.n_phase) * nf
-            stage_roof["mac"]["executed_tflops"] = ex / (stage_ms["mac"] * 1e-3) / 1e12
-            stage_roof["mac"]["executed_frac"] = stage_roof["mac"]["executed_tflops"] / tf32_peak
+                             "frac": ach / peak if peak else None, "ms_per_launch": stage_ms[k] / nl,
+                             "launches_per_step": nl, "work_per_launch": w / nl, "peak_source": src,
+                             "traffic": (tr / nl) if tr else None, "traffic_source": traffic_src,
+                             "own_gbs": own / sec / 1e9, "own_frac_of_hbm": own / sec / 1e9 / hbm}
+        if "mac" in stage_roof and nprod:
+            # what the tensor cores execute: `nprod` products per fp32 product, row tiles of 128 rows
+            # (partly filled), 2 x kp columns for 2 x noff offsets, K padded to the MMA step
+            kpad = ((2 * d.n_phase + 15) // 16) * 16 if m["mac_mode"] == 7 else 2 * d.n_phase
+            ex = nprod * 2.0 * rows_pad * (2 * d.n_off_pad) * kpad * nf
+            r = stage_roof["mac"]
+            r["executed_tflops"] = ex / (stage_ms["mac"] * 1e-3) / 1e12
+            r["executed_frac"] = r["executed_tflops"] / r["peak"]
+            r["ceiling"] = mac_flops / ex
+            r["arithmetic"] = mac_name
+        # SURVEY 8(d)'s own S4 floor: all of S4's flops on the fp32 FMA pipes
+        s4_ms = sum(stage_ms.get(k, 0.0) for k in ("fft_fwd", "conv_misc", "mac", "accum", "ifft"))
+        s4_flops = nb * ncols * fftf + mac_flops + info["nsp"] * fftf
+        s4 = {"ms": s4_ms, "algorithmic_tflop": s4_flops / 1e12, "fma_floor_ms": s4_flops / (fma_tflops * 1e12) * 1e3,
+              "algorithmic_bytes_gb": (payload_b + spd_b) / 1e9,
+              "hbm_floor_ms": (payload_b + spd_b) / (hbm * 1e9) * 1e3}
         dom = max(stage_roof, key=lambda k: stage_ms[k])
         roof = dict(stage_roof[dom])
-        payload_gb = nb * d.block_floats * 4 / 1e9
+        payload_gb = payload_b / 1e9
         line = {"metric": METRIC, "value": total_seg / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_max,
-                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": f"f32 (spectrum product: {mac_name}; index path f64)",
                 "data": "synthetic",
                 "config": {"workload": cfg.name, "segments_per_event": nseg, "events": world,
                            "pixels": [cfg.npix_x, cfg.npix_y], "nticks": cfg.nticks, "gl_n": cfg.gl_n,
                            "block": list(cfg.block), "resp_nticks": cfg.resp_nticks, "fft_len": d.fft_len,
                            "l2": "flushed between timed iterations (256 MiB write)",
                            "parallelism": f"events x{world}, no collective",
-                           "chunks": nchunks, **info},
+                           "mac_mode_ran": m["mac_mode"], **info},
                 "e2e": {"value": total_seg / (e2e_max * 1e-3), "unit": UNIT, "ms_per_step": e2e_max,
-                        "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-                "gpu_launches": int(launches),
+                        "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"],
+                        "through": "tred_simulate (C ABI) with pinned host buffers for segments and tiles"},
+                "gpu_launches": m["launches"] * args.steps,
+                "gpu_launches_per_step": m["launches"],
                 "clocks": clocks,
+                "fma_tflops_measured": fma_tflops,
                 "stage_ms": {k: round(v, 4) for k, v in stage_ms.items() if v > 0},
                 "roofline": roof,
                 "stage_roofline": {k: {kk: (round(vv, 6) if isinstance(vv, float) else vv)
                                        for kk, vv in v.items() if kk in ("bound", "achieved", "peak", "unit", "frac",
-                                                                          "traffic", "executed_tflops",
-                                                                          "executed_frac")}
+                                                                          "traffic", "own_gbs", "own_frac_of_hbm",
+                                                                          "executed_tflops", "executed_frac",
+                                                                          "ceiling")}
                                    for k, v in stage_roof.items()},
-                "peak_mem_gb": peak_mem / 1e9,
+                "s4": s4,
+                "peak_mem_gb": m["peak_mem"] / 1e9,
                 "payload_gb": payload_gb,
-                "wall_s_timed_region": t_wall}
+                "wall_s_timed_region": m["t_wall"]}
+        if world == 1 and not args.no_extras:
+            line["cufft_s4_comparison"] = cufft_s4_comparison(torch, m)
+        segs, R = m["segs"], m["R"]
+        # release the main workload before the other configurations are timed
+        m.clear(); sim = None
+        torch.cuda.empty_cache()
+        if world == 1 and not args.no_extras and args.config == 3:
+            extra = {}
+            for cid in (1, 2, 4):
+                x = measure(args, cid, 0, 1, dev, 10 if cid < 4 else 2, stages=False)
+                extra[x["cfg"].name] = {"segments": x["nseg"], "ms_per_step": x["ms"],
+                                        "segments_per_s": x["nseg"] / (x["ms"] * 1e-3), "e2e_ms_per_step": x["e2e"],
+                                        "gpu_launches_per_step": x["launches"], "host_reads_per_step": x["info"]["host_reads"],
+                                        "chunks": x["info"]["nchunks"], "nblocks": x["info"]["nblocks"],
+                                        "peak_mem_gb": x["peak_mem"] / 1e9, "mac_mode_ran": x["mac_mode"]}
+                x.clear()
+                torch.cuda.empty_cache()
+            line["extra"] = extra
         if not args.no_cpu_baseline and world == 1:
             n, dt, cores = oracle_sample(cfg, segs, R, _ref_segments(args))
             line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -502,6 +608,7 @@ def main():
     ap.add_argument("--budget-gb", type=int, default=7, help="config 4: block payload per chunk (GiB)")
     ap.add_argument("--mac-mode", type=int, default=0, help="tred_config.mac_mode (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip configs 1, 2, 4 and the cuFFT comparison")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

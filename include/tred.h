@@ -332,6 +332,49 @@ int tred_readout(const tred_readout_config* cfg, int64_t npix, int32_t nticks, c
                  void* stream);
 
 /*
+ * tred_simulate -- the whole path in one call: segments in, per-pixel current waveforms out
+ * (Fig. 1): tred_drift, tred_blockbin, tred_convolve_plan, tred_effq,
+ * tred_convolve, tred_gather_waveforms on buffers carved from one caller-provided workspace.
+ *   seg          [8][nseg] float32 as for tred_drift, in HOST memory if seg_on_host != 0 (copied
+ *                to the device by the call), else in device memory
+ *   d_rhat       from tred_prepare_response
+ *   payload_budget_bytes  0: the block payload of the whole event is held at once.  > 0 and smaller
+ *                than the payload: the event is processed in ranges of time slabs whose payload
+ *                fits (chunks bounded by device memory; BASELINE config 4); the
+ *                result is bit-identical to one pass (a slab's output depends on that slab's
+ *                blocks only, and the overlap-add continues the running sum in slab order)
+ *   d_work       device workspace, work_bytes long.  Too small: TRED_ECAP with
+ *                h_result->work_bytes_needed set (a size that is enough for this event)
+ *   tile_keys    [cap_tiles] int64 out, tile_data [cap_tiles][Bt] float32 out: the waveform tiles,
+ *                keys ascending, in HOST memory if out_on_host != 0, else device memory.
+ *                h_result->ntiles > cap_tiles: TRED_ECAP, nothing written
+ *   d_pix_ids, d_dense  optional dense rows as for tred_gather_waveforms (device memory)
+ *   h_result     HOST, filled by the call
+ * Host waits: the call reads the device-side counts ONCE per event (pairs, blocks, footprints
+ * and per-slab offsets in one copy, after the plan), plus once per slab range in the chunked
+ * form.  The capacities of the lists that precede that read come from the previous event on
+ * this context (first event, or an event that outgrows them: one more read).  The outputs are
+ * complete when `stream` has finished.
+ */
+typedef struct tred_sim_result {
+  int64_t nseg, npairs, nblocks, ncp, nsp, ntiles, nrt, nchunks;
+  int64_t work_bytes_needed;     /* set with TRED_ECAP when d_work is too small           */
+  int64_t conv_bytes_needed;     /* of which: what tred_convolve would like (it chunks the charge
+                                    pixels to what it gets) and the least it can work with; a
+                                    caller bounding peak memory may grant anything in between  */
+  int64_t conv_bytes_min;
+  int64_t work_bytes_used;
+  int32_t host_reads;            /* device-to-host reads of counts this call made           */
+  int32_t mac_mode;              /* tred_last_mac_mode                                      */
+} tred_sim_result;
+
+int tred_simulate(tred_ctx* ctx, int64_t nseg, const float* seg, int seg_on_host, const float* d_rhat,
+                  int64_t payload_budget_bytes, void* d_work, size_t work_bytes,
+                  int64_t cap_tiles, int64_t* tile_keys, float* tile_data, int out_on_host,
+                  int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
+                  tred_sim_result* h_result, void* stream);
+
+/*
  * tred_truth -- truth record ("segment-id -> charge per (channel, short time
  * slice)"; reading G24): the effective charge of every segment summed over the grid
  * points of each pixel and each time tile (Bt ticks) of its clipped footprint.  One entry per

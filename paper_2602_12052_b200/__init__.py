@@ -59,6 +59,14 @@ class TredReadoutConfig(C.Structure):
                 ("max_hits", C.c_int32), ("adc_lsb_e", C.c_double)]
 
 
+class TredSimResult(C.Structure):
+    """Mirror of `tred_sim_result` (include/tred.h)."""
+    _fields_ = [(k, _c_i64) for k in ("nseg", "npairs", "nblocks", "ncp", "nsp", "ntiles", "nrt", "nchunks",
+                                       "work_bytes_needed", "conv_bytes_needed", "conv_bytes_min",
+                                       "work_bytes_used")] + \
+               [("host_reads", C.c_int32), ("mac_mode", C.c_int32)]
+
+
 # name -> (restype, argtypes); every symbol include/tred.h declares
 EXPORTS = {
     "tred_get_dims": (C.c_int, [C.POINTER(TredConfig), C.POINTER(TredDims)]),
@@ -90,6 +98,8 @@ EXPORTS = {
                                 _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
     "tred_gather_waveforms": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_p, _c_i64, _c_i64, _c_p, _c_p, C.c_int,
                                         _c_i64, _c_p, _c_p, _c_p]),
+    "tred_simulate": (C.c_int, [_c_p, _c_i64, _c_p, C.c_int, _c_p, _c_i64, _c_p, C.c_size_t,
+                                _c_i64, _c_p, _c_p, C.c_int, _c_i64, _c_p, _c_p, C.POINTER(TredSimResult), _c_p]),
     "tred_steps_work_bytes": (C.c_size_t, [_c_i64]),
     "tred_steps": (C.c_int, [C.POINTER(TredStepsConfig), _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
                              C.c_size_t, _c_p]),
@@ -430,9 +440,69 @@ class Tred:
         return tile_data, dense
 
     # -- whole path -----------------------------------------------------------------
-    def simulate(self, seg, rhat, pix_ids=None, keep=False):
-        """Segments in, per-pixel current waveforms out.  Reads three
-        device-side counts back to size the buffers (the only host synchronisations)."""
+    def simulate(self, seg, rhat, pix_ids=None, keep=False, payload_budget_bytes: int = 0,
+                 host_out=None):
+        """Segments in, per-pixel current waveforms out: one call of
+        tred_simulate.  `seg` may be a CUDA tensor or a (pinned) host tensor; `host_out` =
+        (tile_keys, tile_data) host tensors to receive the tiles (default: device tensors are
+        returned).  `keep=True` runs the stepwise calls instead and returns the intermediates
+        too (tests).  The binding only owns the workspace: it grows it when the library says
+        how much this event needs and calls again."""
+        t = self.torch
+        if keep:
+            return self.simulate_steps(seg, rhat, pix_ids, keep=True)
+        assert seg.dtype == t.float32 and seg.is_contiguous() and seg.shape[0] == 8
+        nseg = seg.shape[1]
+        Bt = self.cfg.block[2]
+        res = TredSimResult()
+        npix = 0
+        dense = None
+        if pix_ids is not None and pix_ids.numel() > 0:
+            assert pix_ids.dtype == t.int32 and pix_ids.is_cuda
+            npix = pix_ids.numel()
+            dense = self._empty((npix, self.cfg.nticks), t.float32)
+        cap_tiles = getattr(self, "_cap_tiles", 0)
+        want = max(getattr(self, "_sim_bytes", 0), (2 << 30) + nseg * 4096)
+        for _ in range(8):
+            work = self._workbuf("sim", want)
+            if host_out is not None:
+                tk, td = host_out
+                cap = min(tk.numel(), td.shape[0])
+            else:
+                cap = cap_tiles
+                tk = self._empty((max(cap, 1),), t.int64)
+                td = self._empty((max(cap, 1), Bt), t.float32)
+            rc = self.L.tred_simulate(self.h, nseg, _ptr(seg), 0 if seg.is_cuda else 1, _ptr(rhat),
+                                      int(payload_budget_bytes), _ptr(work), work.numel(), cap, _ptr(tk), _ptr(td),
+                                      0 if host_out is None else 1, npix, _ptr(pix_ids), _ptr(dense), C.byref(res),
+                                      self._stream())
+            if rc == -2 and res.work_bytes_needed > work.numel():          # workspace: grow and call again
+                want = int(res.work_bytes_needed) + (64 << 20)
+                if self.conv_work_bytes is not None and res.conv_bytes_needed > 0:      # bounded peak memory
+                    grant = min(max(int(self.conv_work_bytes), int(res.conv_bytes_min)), int(res.conv_bytes_needed))
+                    want -= int(res.conv_bytes_needed) - grant
+                self._work.pop("sim", None)
+                work = None
+                continue
+            if rc == -2 and res.ntiles > cap:                               # tile capacity
+                if host_out is not None:
+                    raise TredError(f"host_out holds {cap} tiles, the event has {res.ntiles}")
+                cap_tiles = int(res.ntiles * 1.05) + 1024
+                continue
+            _check(rc, "tred_simulate")
+            break
+        else:
+            raise TredError("tred_simulate: workspace negotiation did not converge")
+        self._sim_bytes, self._cap_tiles = want, cap_tiles
+        nt = int(res.ntiles)
+        out = {k: int(getattr(res, k)) for k in ("nseg", "npairs", "nblocks", "ncp", "nsp", "ntiles", "nrt",
+                                                 "nchunks", "host_reads", "mac_mode", "work_bytes_used")}
+        out.update(tile_keys=tk[:nt], tile_data=td[:nt], dense=dense)
+        return out
+
+    def simulate_steps(self, seg, rhat, pix_ids=None, keep=False):
+        """The same path through the stepwise calls (three host reads of counts); returns the
+        intermediates as well when keep=True."""
         t = self.torch
         nseg = seg.shape[1]
         augf, augi, npairs = self.drift(seg)
@@ -497,68 +567,11 @@ class Tred:
         return out[:ngroups]
 
     # -- whole path in bounded-memory chunks of occupied blocks (BASELINE config 4) --------
-    def simulate_chunked(self, seg, rhat, pix_ids=None, payload_budget_bytes: int = 8 << 30,
-                         effq_work_bytes: int = 1 << 30):
+    def simulate_chunked(self, seg, rhat, pix_ids=None, payload_budget_bytes: int = 8 << 30):
         """Same result as `simulate`, bit for bit, with the block payload, the convolution
         workspace and the slab outputs held for one range of time slabs at a time
-        (chunks bounded by device memory).  The occupied blocks are
-        sorted slab-major, so a chunk is a contiguous range of the block list whose payload
-        fits `payload_budget_bytes`; a slab's output depends on that slab's blocks only, and
-        the overlap-add continues the running sum of the tiles (`accumulate`)."""
-        t = self.torch
-        import numpy as np
-        nseg = seg.shape[1]
-        NBt = int(self.dims.NB[2])
-        Bt = self.cfg.block[2]
-        npix = self.cfg.npix_x * self.cfg.npix_y
-        augf, augi, npairs = self.drift(seg)
-        cap_pairs = int(npairs.item())
-        keys, blk_off, pair_seg, slab_off, nblocks_d = self.blockbin(augi, cap_pairs)
-        nblocks = int(nblocks_d.item())
-        so = slab_off.cpu().numpy().astype(np.int64)
-        gplan = self.convolve_plan(nblocks, keys)                    # tile list of the whole event
-        ntiles = int(gplan["ntiles"].item())
-        tile_keys = gplan["tile_keys"]
-        tile_data = t.zeros((max(ntiles, 1), Bt), dtype=t.float32, device=self.device)
-        # first tile of every time tile index tb (tile keys are sorted, tb-major)
-        bounds = t.arange(0, NBt + self.dims.n_over + 1, device=self.device, dtype=t.int64) * npix
-        tile_lo = t.searchsorted(tile_keys[:ntiles], bounds).cpu().numpy()
-        blk_bytes = int(self.dims.block_floats) * 4
-        max_blk = max(1, int(payload_budget_bytes) // blk_bytes)
-        payload = None
-        chunks = []
-        b0 = 0
-        while b0 < NBt:
-            if so[b0 + 1] == so[b0]:
-                b0 += 1
-                continue
-            b1 = b0 + 1
-            while b1 < NBt and so[b1 + 1] - so[b0] <= max_blk:
-                b1 += 1
-            k0, k1 = int(so[b0]), int(so[b1])
-            nb = k1 - k0
-            if payload is None or payload.shape[0] < nb:
-                payload = None
-                payload = self._empty((nb, self.cfg.block[0], self.cfg.block[1], Bt), t.float32)
-            kc = keys[k0:k1]
-            self.effq(nb, kc, blk_off[k0:k1 + 1], pair_seg, augf, augi, payload=payload, work_bytes=effq_work_bytes)
-            plan = self.convolve_plan(nb, kc)
-            counts = t.cat([plan["ncp"], plan["nsp"], plan["cp_off"].to(t.int64), plan["sp_off"].to(t.int64),
-                            plan["rt_off"].to(t.int64)]).cpu().numpy()
-            ncp, nsp = int(counts[0]), int(counts[1])
-            co, po, ro = (counts[2 + i * (NBt + 1):2 + (i + 1) * (NBt + 1)] for i in range(3))
-            sp_data = self.convolve(nb, kc, payload, rhat, plan, ncp, nsp, co, po, rt_off_host=ro)
-            t_lo = int(tile_lo[b0])
-            t_hi = int(tile_lo[min(b1 - 1 + self.dims.n_over, NBt + self.dims.n_over)])
-            if t_hi > t_lo:
-                self.gather_waveforms(nsp, sp_data, plan, t_hi - t_lo, tile_plan=gplan, tile_data=tile_data,
-                                      tile_begin=t_lo, accumulate=True)
-            chunks.append((b0, b1, nb, ncp, nsp, int(ro[-1])))
-            del plan, sp_data
-            b0 = b1
-        dense = None
-        if pix_ids is not None and pix_ids.numel() > 0:
-            _, dense = self.gather_waveforms(0, None, gplan, 0, pix_ids=pix_ids, tile_data=tile_data)
-        return dict(nseg=nseg, npairs=cap_pairs, nblocks=nblocks, ntiles=ntiles, tile_keys=tile_keys[:ntiles],
-                    tile_data=tile_data[:ntiles], dense=dense, chunks=chunks,
-                    ncp=sum(c[3] for c in chunks), nsp=sum(c[4] for c in chunks), nrt=sum(c[5] for c in chunks))
+        (chunks bounded by device memory): tred_simulate with a payload
+        budget.  `chunks` in the result is the number of slab ranges."""
+        out = self.simulate(seg, rhat, pix_ids, payload_budget_bytes=payload_budget_bytes)
+        out["chunks"] = out["nchunks"]
+        return out

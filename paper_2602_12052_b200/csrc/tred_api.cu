@@ -202,6 +202,7 @@ extern "C" void tred_destroy(tred_ctx* c) {
   if (!c) return;
   prof_clear(c);
   free(c->recs);
+  if (c->h_counts) cudaFreeHost(c->h_counts);
   free(c);
 }
 
@@ -328,7 +329,7 @@ k_pair_expand(int64_t nseg, const int32_t* __restrict__ augi, const int32_t* __r
   for (int bt = blo[2]; bt <= bhi[2]; ++bt)
     for (int bx = blo[0]; bx <= bhi[0]; ++bx)
       for (int by = blo[1]; by <= bhi[1]; ++by, ++o)
-        if (o < cap_pairs) {
+        if (o >= 0 && o < cap_pairs) {
           keys[o] = (uint32_t)((bt * g.NBx + bx) * g.NBy + by);
           vals[o] = (int32_t)s;
         }

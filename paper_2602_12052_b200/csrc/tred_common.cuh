@@ -21,6 +21,8 @@ struct tred_ctx {
   int         device;         // CUDA device the context was created on
   const void* sym_rhat;       // last d_rhat prepared from a mirror-symmetric response (or NULL)
   int         last_mac_mode;  // spectrum-product kernel the last tred_convolve launched (tred_last_mac_mode)
+  int64_t     hint_pairs;     // tred_simulate: (segment, block) pairs of the previous event (0: none yet)
+  int64_t*    h_counts;       // tred_simulate: pinned host mirror of the device-side counts
   // stage profiling (tred_profile_begin / tred_profile_end)
   int         prof_on;
   int64_t     launches[ST_COUNT];
@@ -118,6 +120,15 @@ constexpr int RT_PYS = 66;       // patch row stride in shared memory (66 = 2 mo
 constexpr int RT_MAXH = 5;       // largest response half-width the patch buffers hold
 constexpr int RT_PXMAX = RT_SW + 2 * RT_MAXH;
 
+
+// ---- internal entry points of the convolution plan used by tred_simulate (tred_sim.cu) ----
+int tred_convolve_plan_dev(tred_ctx* ctx, int64_t nblocks, const int64_t* d_nblocks, const int64_t* d_keys,
+                           int64_t cap_cp, int64_t* d_cp_keys, int32_t* d_cp_off, int64_t* d_ncp,
+                           int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
+                           int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
+                           int32_t* d_rt_off,
+                           void* d_plan_work, size_t plan_work_bytes, void* stream);
+int tred_plan_tile_offsets(tred_ctx* ctx, const void* d_plan_work, int32_t* d_tile_off, cudaStream_t st);
 
 // ---- S2 variants (tred_effq.cu: closed form; tred_effq_fact.cu: factored, dispatch) ---
 int tred_effq_closed_form(tred_ctx* ctx, int64_t nseg, int64_t nblocks,

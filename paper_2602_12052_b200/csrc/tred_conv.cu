@@ -209,10 +209,12 @@ k_resp_sym(const float2* __restrict__ W, float* __restrict__ Bs_hi, float* __res
 
 // ------------------------------------------------------------------ plan (O6)
 // flags over the map m = bt * npix + px * npy + py
+// d_nb: device-side block count (NULL: nblocks is exact); nblocks is then the capacity of keys
 __global__ void __launch_bounds__(256)
-k_mark_blocks(int64_t nblocks, const int64_t* __restrict__ keys, int32_t* __restrict__ cp_flag,
-              int32_t* __restrict__ sp_flag, TredGrid g) {
+k_mark_blocks(int64_t nblocks, const int64_t* __restrict__ d_nb, const int64_t* __restrict__ keys,
+              int32_t* __restrict__ cp_flag, int32_t* __restrict__ sp_flag, TredGrid g) {
   const int warp = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+  if (d_nb && *d_nb < nblocks) nblocks = *d_nb;
   if (warp >= nblocks) return;
   const int64_t key = keys[warp];
   const int by = (int)(key % g.NBy), bx = (int)((key / g.NBy) % g.NBx);
@@ -1476,12 +1478,40 @@ extern "C" size_t tred_plan_work_bytes(const tred_ctx* ctx) {
   return ctx ? carve_plan(ctx, nullptr).total : 0;
 }
 
+// first tile of every time tile index tb (slot NBt: the number of tiles), from the plan's scan
+__global__ void k_tile_offsets(int NBt, int64_t npix, const int32_t* __restrict__ tile_idx, int32_t* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i <= NBt) out[i] = tile_idx[(int64_t)i * npix];
+}
+
+int tred_plan_tile_offsets(tred_ctx* ctx, const void* d_plan_work, int32_t* d_tile_off, cudaStream_t st) {
+  const PlanWork w = carve_plan(ctx, (void*)d_plan_work);
+  const TredGrid g = make_grid(ctx);
+  k_tile_offsets<<<cdiv(g.NBt + 1, 128), 128, 0, st>>>(g.NBt, (int64_t)g.npx * g.npy, w.tile_idx, d_tile_off);
+  TRED_COUNT_LAUNCH(1);
+  TRED_LAUNCH_CHECK("k_tile_offsets");
+  return TRED_OK;
+}
+
 extern "C" int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
                                   int64_t cap_cp, int64_t* d_cp_keys, int32_t* d_cp_off, int64_t* d_ncp,
                                   int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
                                   int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
                                   int32_t* d_rt_off,
                                   void* d_plan_work, size_t plan_work_bytes, void* stream) {
+  return tred_convolve_plan_dev(ctx, nblocks, nullptr, d_keys, cap_cp, d_cp_keys, d_cp_off, d_ncp, cap_sp, d_sp_keys,
+                                d_sp_off, d_nsp, cap_tiles, d_tile_keys, d_ntiles, d_rt_off, d_plan_work,
+                                plan_work_bytes, stream);
+}
+
+// As tred_convolve_plan with the block count read on the device: nblocks is the capacity of
+// d_keys, *d_nblocks (if not NULL) the number of valid keys.
+int tred_convolve_plan_dev(tred_ctx* ctx, int64_t nblocks, const int64_t* d_nblocks, const int64_t* d_keys,
+                           int64_t cap_cp, int64_t* d_cp_keys, int32_t* d_cp_off, int64_t* d_ncp,
+                           int64_t cap_sp, int64_t* d_sp_keys, int32_t* d_sp_off, int64_t* d_nsp,
+                           int64_t cap_tiles, int64_t* d_tile_keys, int64_t* d_ntiles,
+                           int32_t* d_rt_off,
+                           void* d_plan_work, size_t plan_work_bytes, void* stream) {
   if (!ctx || nblocks < 0 || !d_ncp || !d_cp_off || !d_nsp || !d_ntiles || !d_sp_off || !d_rt_off)
     return TRED_EINVAL;
   PlanWork w = carve_plan(ctx, d_plan_work);
@@ -1495,7 +1525,8 @@ extern "C" int tred_convolve_plan(tred_ctx* ctx, int64_t nblocks, const int64_t*
   TRED_CUDA(cudaMemsetAsync(w.sp_idx, 0, (w.nmap + 1) * 4, st));
   TRED_CUDA(cudaMemsetAsync(w.tile_idx, 0, (w.nmap + 1) * 4, st));
   TRED_COUNT_LAUNCH(4 + (nblocks > 0 ? 1 : 0));
-  if (nblocks > 0) k_mark_blocks<<<cdiv(nblocks * 32, 256), 256, 0, st>>>(nblocks, d_keys, w.cp_idx, w.sp_idx, g);
+  if (nblocks > 0)
+    k_mark_blocks<<<cdiv(nblocks * 32, 256), 256, 0, st>>>(nblocks, d_nblocks, d_keys, w.cp_idx, w.sp_idx, g);
   int rc = tred_exclusive_scan_i32(w.cp_idx, w.cp_idx, w.nmap + 1, nullptr, w.scan, st);
   if (rc != TRED_OK) return rc;
   k_compact_keys<<<cdiv(w.nmap + 1, 256), 256, 0, st>>>(w.nmap, w.cp_idx, cap_cp, d_cp_keys, d_ncp,

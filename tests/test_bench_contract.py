@@ -33,7 +33,9 @@ def test_reference_arm_line():
 def test_cuda_arm_line():
     d = _run(["--config", "1", "--steps", "3", "--warmup", "3", "--ref-segments", "12"])
     assert BASE_KEYS | {"roofline", "cpu_baseline", "clocks", "stage_ms"} <= set(d)
-    assert d["n_gpus"] == 1 and d["scaling"] == "weak" and d["dtype"] == "f32" and d["vs_baseline"] is None
+    assert d["n_gpus"] == 1 and d["scaling"] == "weak" and d["dtype"].startswith("f32") and d["vs_baseline"] is None
+    assert d["config"]["mac_mode_ran"] in (1, 2, 3, 5, 6, 7) and d["fma_tflops_measured"] > 10
+    assert "tred_simulate" in d["e2e"]["through"] and d["config"]["host_reads"] == 1
     assert d["gpu_launches"] > 0 and d["value"] > 0 and d["e2e"]["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0
     r = d["roofline"]

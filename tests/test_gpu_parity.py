@@ -431,7 +431,7 @@ def test_chunked_equals_single_pass(cfg_id):
     a = sim.simulate(seg, rhat)
     blk = int(sim.dims.block_floats) * 4
     b = sim.simulate_chunked(seg, rhat, payload_budget_bytes=max(a["nblocks"] // 5, 1) * blk)
-    assert len(b["chunks"]) >= 3
+    assert b["chunks"] >= 3
     assert b["nblocks"] == a["nblocks"] and b["ntiles"] == a["ntiles"]
     assert torch.equal(a["tile_keys"], b["tile_keys"])
     assert torch.equal(a["tile_data"], b["tile_data"])
