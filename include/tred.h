@@ -89,6 +89,12 @@ typedef struct tred_config {
                                         is not exactly mirror-symmetric,
                                     1 = fp32 FMA pipe, products written to memory,
                                     2 = tensor cores 3xTF32, products written to memory       */
+  int32_t fft_mode;              /* forward transform of tred_convolve in mac_mode 7:
+                                    0 = default: pruned DFT as a dense contraction on the tensor
+                                        cores (tred_dft_h16.cu) where the shape allows it (Bt a
+                                        multiple of 32, <= 128; L with a divisor NC <= 256, NC a
+                                        multiple of 32, L / NC >= 2), else as 1,
+                                    1 = shared-memory / register FFT kernels                     */
 } tred_config;
 
 /* Sizes derived from a configuration (host-side helper, no device work). */
@@ -108,6 +114,7 @@ typedef struct tred_dims {
   int64_t rhat_floats;    /* floats of the response spectrum buffer (all layouts)         */
   int64_t block_floats;   /* Bx*By*Bt                                                     */
   int64_t conv_row_bytes; /* tred_convolve workspace bytes per charge pixel in flight     */
+  int32_t dft_ticks;      /* Bt: rows of the DFT matrix kept with the response spectrum   */
 } tred_dims;
 
 typedef struct tred_ctx tred_ctx;   /* opaque, host memory */

@@ -33,7 +33,7 @@ class TredConfig(C.Structure):
                 ("nsigma", C.c_double), ("point_thresh", C.c_double),
                 ("gl_n", C.c_int32), ("block", C.c_int32 * 3),
                 ("resp_half", C.c_int32), ("resp_nticks", C.c_int32),
-                ("effq_mode", C.c_int32), ("mac_mode", C.c_int32)]
+                ("effq_mode", C.c_int32), ("mac_mode", C.c_int32), ("fft_mode", C.c_int32)]
 
 
 class TredDims(C.Structure):
@@ -42,7 +42,8 @@ class TredDims(C.Structure):
                 ("fft_len", C.c_int32), ("out_len", C.c_int32), ("n_over", C.c_int32),
                 ("n_freq", C.c_int32), ("n_phase", C.c_int32), ("n_off", C.c_int32),
                 ("n_off_pad", C.c_int32), ("pix_per_block", C.c_int32),
-                ("rhat_floats", _c_i64), ("block_floats", _c_i64), ("conv_row_bytes", _c_i64)]
+                ("rhat_floats", _c_i64), ("block_floats", _c_i64), ("conv_row_bytes", _c_i64),
+                ("dft_ticks", C.c_int32)]
 
 
 class TredStepsConfig(C.Structure):
@@ -135,7 +136,7 @@ def lib() -> C.CDLL:
 
 
 _CFG_FIELDS = [f[0] for f in TredConfig._fields_]
-_CFG_OPTIONAL = ("effq_mode", "mac_mode")        # 0 = library default
+_CFG_OPTIONAL = ("effq_mode", "mac_mode", "fft_mode")        # 0 = library default
 
 
 def make_config(cfg) -> TredConfig:

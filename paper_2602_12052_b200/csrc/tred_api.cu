@@ -129,6 +129,7 @@ extern "C" int tred_get_dims(const tred_config* c, tred_dims* d) {
   if (c->gl_n < 1 || c->gl_n > 4) return TRED_EINVAL;
   if (c->resp_half < 0 || c->resp_nticks <= 0) return TRED_EINVAL;
   if (c->effq_mode < 0 || c->effq_mode > 1 || c->mac_mode < 0 || c->mac_mode > 7) return TRED_EINVAL;
+  if (c->fft_mode < 0 || c->fft_mode > 1) return TRED_EINVAL;
   if (!(c->pitch_mm > 0) || !(c->tick_us > 0) || !(c->v_mm_us > 0) || !(c->lifetime_us > 0))
     return TRED_EINVAL;
   if (!(c->nsigma > 0) || !(c->sigma_min_xy_mm > 0) || !(c->sigma_min_t_us > 0)) return TRED_EINVAL;
@@ -164,6 +165,7 @@ extern "C" int tred_get_dims(const tred_config* c, tred_dims* d) {
                      ((c->sub - 1 + c->block[1] - 1) / c->sub + 1);
   // response spectrum: fp32 [f][phase][off_pad] complex (2 floats) + tf32 hi and lo
   // [f][2 off_pad][2 phase] (4 floats each)
+  d->dft_ticks = c->block[2];
   d->rhat_floats = rhat_layout(*d).total;
   d->block_floats = (int64_t)c->block[0] * c->block[1] * c->block[2];
   // per charge pixel in flight: spectra [f][phase] + products [f][off_pad], complex fp32

@@ -93,10 +93,11 @@ static inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 // [B_hi, B_lo rounded to bf16, same shape as B_hi: operands of the bf16 correction products]
 // [B16: [f][2 kp][h16_kp] fp16, hi / lo parts of B / bscale[f] in blocks of 16 reals (tred_mac_h3.cu)]
 // [bscale: [f] float, power of two]
+// [Wd: [L][2 Bt] fp16 hi / lo DFT matrix of the forward transform (tred_dft_h16.cu)]
 constexpr int SYM_N = 128;           // rows of the symmetric matrices: 2 x (noff + 1) / 2 padded
 // halves per operand row in the fp16 hi / lo block layout: ceil(2 nph / 16) blocks of (16 hi | 16 lo)
 static inline int h16_kp(const tred_dims& d) { return (2 * d.n_phase + 15) / 16 * 32; }
-struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, bhb, blb, b16, bsc, total; };
+struct RhatLayout { int64_t w, bhi, blo, bs_hi, bs_lo, bd_hi, bd_lo, flag, bhb, blb, b16, bsc, wdft, total; };
 static inline RhatLayout rhat_layout(const tred_dims& d) {
   RhatLayout L;
   const int64_t rb = (int64_t)d.n_freq * d.n_phase * d.n_off_pad;
@@ -108,7 +109,8 @@ static inline RhatLayout rhat_layout(const tred_dims& d) {
   L.blb = L.bhb + 2 * rb;
   L.b16 = L.blb + 2 * rb;              // 16-byte aligned: every term above is a multiple of 8 floats
   L.bsc = L.b16 + (int64_t)d.n_freq * 2 * d.n_off_pad * (h16_kp(d) / 2);
-  L.total = L.bsc + (d.n_freq + 7) / 8 * 8;
+  L.wdft = L.bsc + (d.n_freq + 7) / 8 * 8;     // DFT matrix [L][2 Bt] fp16 (tred_dft_h16.cu): L * Bt floats
+  L.total = L.wdft + (int64_t)d.fft_len * d.dft_ticks;
   return L;
 }
 

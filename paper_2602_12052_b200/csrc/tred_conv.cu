@@ -1275,6 +1275,13 @@ bool tred_mac_h3_supported(const tred_ctx* ctx);
 int tred_mac_h3(tred_ctx* ctx, const void* qh, const float* rscale, const void* Bh16, const float* bscale,
                 float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st);
 
+// forward transform as a DFT-matrix contraction on the tensor cores (tred_dft_h16.cu)
+bool tred_dft_h16_supported(const tred_ctx* ctx);
+int tred_dft_matrix(tred_ctx* ctx, void* d_Wd, cudaStream_t st);
+int tred_dft_h16(tred_ctx* ctx, const float* payload, const int32_t* blockmap, const void* rt_desc,
+                 const int32_t* row_m2, int t0, int ntile, int nstrip, const void* d_Wd,
+                 void* qh, float* rscale, cudaStream_t st);
+
 // mirror-symmetric response (tred_mac_tc2s.cu)
 bool tred_mac_tc2s_supported(const tred_ctx* ctx);
 int tred_mac_tc2s(tred_ctx* ctx, const float* qhat, const float* Bs_hi, const float* Bs_lo, const float* Bd_hi,
@@ -1329,6 +1336,7 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
   const bool h16 = (ctx->cfg.mac_mode == 0 || ctx->cfg.mac_mode == 7) && g.nph == 100 && (g.Bt & 3) == 0 &&
                    tred_mac_h3_supported(ctx) && fft_fwd_2s_available(g);
   if (ctx->cfg.mac_mode == 7 && !h16) return TRED_EUNSUPPORTED;
+  const bool dft = h16 && ctx->cfg.fft_mode == 0 && tred_dft_h16_supported(ctx);
   ctx->last_mac_mode = 0;
   int b0 = 0;
   while (b0 < g.NBt) {
@@ -1355,7 +1363,14 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
       {
         TredProfScope ps(ctx, ST_FFT_FWD, st);
         const RowSrc rs{nullptr, 0, pw.rt_desc, pw.row_m2, t0, rg.nstrip, 1};
-        int ct = sym ? launch_fft_fwd_2s<1>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, nullptr, w.tw, st)
+        int ct = 0;
+        if (dft) {
+          const int rc = tred_dft_h16(ctx, d_payload, w.blockmap, pw.rt_desc, pw.row_m2, t0, nt, rg.nstrip,
+                                      d_rhat + rl.wdft, w.qhat, w.rscale, st);
+          if (rc != TRED_OK) return rc;
+          ct = 1;
+        } else
+        ct = sym ? launch_fft_fwd_2s<1>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, nullptr, w.tw, st)
                : h16 ? launch_fft_fwd_2s<2>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, w.rscale, w.tw, st)
                      : launch_fft_fwd_2s<0>(ctx, g, d_payload, w.blockmap, rs, rp, rp, w.qhat, nullptr, w.tw, st);
         if ((sym || h16) && ct == 0) return TRED_EUNSUPPORTED;
@@ -1451,6 +1466,10 @@ extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* 
     k_resp_h16<<<cdiv(n, 256), 256, 0, st>>>((const float2*)d_rhat, bsc, reinterpret_cast<__half*>(d_rhat + rl.b16),
                                             g.nf, g.nph, g.noff, g.kp, h16_kp(ctx->dims));
     TRED_COUNT_LAUNCH(2);
+    if (tred_dft_h16_supported(ctx)) {
+      const int rc = tred_dft_matrix(ctx, d_rhat + rl.wdft, st);
+      if (rc != TRED_OK) return rc;
+    }
   }
   TRED_LAUNCH_CHECK("k_resp_dft64");
   // mirror-symmetric responses get the half-size matrices as well.  This
