@@ -392,7 +392,9 @@ int tred_simulate(tred_ctx* ctx, int64_t nseg, const float* seg, int seg_on_host
  *   d_nrec    int64 out: number of entries (TRED_ECAP semantics: may exceed cap_rec, nothing
  *             beyond the capacity is written)
  *   d_work    at least tred_truth_work_bytes(nseg) bytes
- * A segment reaching more than 16 pixels or tiles along one axis is truncated to 16.
+ * A record holds at most 32 pixels and 32 time tiles per axis (a segment of the paper's
+ * workloads reaches 2-4).  If any segment reaches more, *d_nrec is set to -1 and the entries
+ * written are not to be used: nothing is truncated silently.
  */
 size_t tred_truth_work_bytes(const tred_ctx* ctx, int64_t nseg);
 int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, const int32_t* d_augi, int64_t cap_rec,

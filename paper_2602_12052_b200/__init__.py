@@ -463,7 +463,7 @@ class Tred:
             npix = pix_ids.numel()
             dense = self._empty((npix, self.cfg.nticks), t.float32)
         cap_tiles = getattr(self, "_cap_tiles", 0)
-        want = max(getattr(self, "_sim_bytes", 0), (2 << 30) + nseg * 4096)
+        want = max(getattr(self, "_sim_bytes", 0), (256 << 20) + nseg * 512)
         for _ in range(8):
             work = self._workbuf("sim", want)
             if host_out is not None:
@@ -539,6 +539,8 @@ class Tred:
             _check(self.L.tred_truth(self.h, nseg, _ptr(augf), _ptr(augi), 0, None, None, None, _ptr(nrec),
                                      _ptr(work), work.numel(), self._stream()), "tred_truth")
             cap_rec = int(nrec.item())
+            if cap_rec < 0:
+                raise TredError("tred_truth: a segment reaches more than 32 pixels or time tiles on one axis")
         rs = self._empty((max(cap_rec, 1),), t.int32)
         rk = self._empty((max(cap_rec, 1),), t.int64)
         rq = self._empty((max(cap_rec, 1),), t.float32)

@@ -495,7 +495,7 @@ k_fft_fwd_ct(const float* __restrict__ payload, const int32_t* __restrict__ bloc
 // mirror phase pairs p = 10 grp + pl and nph-1-p (the FFT is linear, so they are formed
 // on the samples), written to qhat[f][row][s: 50 | d: 50] for the mirror-symmetric product.
 // MODE 2 (H16): the spectra leave as fp16 hi / lo parts in the block layout of tred_mac_h3.cu,
-// qhat = [f][row][KP16] halves, scaled per row by the power of two rscale[row] chosen from
+// qhat = [tile][f][128 rows][KP16] halves, scaled per row by the power of two rscale[row] chosen from
 // sum |q| over the row's columns (no spectrum value can exceed it, so nothing overflows).
 template <int M, int B, int NZA, int MODE>
 __global__ void __launch_bounds__((20 * (M / B) + 31) / 32 * 32, MODE == 2 ? 65536 / 80 / ((20 * (M / B) + 31) / 32 * 32) : 1)
@@ -649,8 +649,10 @@ k_fft_fwd_2s(const float* __restrict__ payload, const int32_t* __restrict__ bloc
     constexpr int CP = CG / 2, KR = NT / CP;
     const int cp = threadIdx.x % CP, kr = threadIdx.x / CP;
     const int p0 = grp * CG + 2 * cp;
-    __half* out = reinterpret_cast<__half*>(qhat) + (int64_t)row * KP16 + (p0 >> 3) * 32 + (p0 & 7) * 2;
-    const int64_t fstride_h = (int64_t)rp * KP16;
+    // [tile][f][128 rows][KP16]: the box of one (row tile, frequency) is contiguous
+    __half* out = reinterpret_cast<__half*>(qhat) +
+                  ((int64_t)(row >> 7) * M * RT_ROWS + (row & (RT_ROWS - 1))) * KP16 + (p0 >> 3) * 32 + (p0 & 7) * 2;
+    const int64_t fstride_h = (int64_t)RT_ROWS * KP16;
     const float2* Z0 = buf + (2 * cp) * ZP;
     const float2* Z1 = Z0 + ZP;
     auto h2u = [](__half2 h) { return *reinterpret_cast<uint32_t*>(&h); };
@@ -1351,6 +1353,7 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
     while (cap > 1 && carve_tiled(ctx, nullptr, cap, nsb).total > work_bytes) --cap;
     if (cap > T1 - T0) cap = T1 - T0;
     if (cap * RT_ROWS * (int64_t)ngrp >= (1ll << 31)) cap = ((1ll << 31) - 1) / (RT_ROWS * ngrp);
+
     const TiledWork w = carve_tiled(ctx, d_work, cap, nsb);
     {
       TredProfScope ps(ctx, ST_ACCUM, st);

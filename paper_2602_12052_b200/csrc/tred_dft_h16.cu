@@ -27,6 +27,10 @@
 #include <cuda_fp16.h>
 #include "tred_tc2_common.cuh"
 
+#ifndef DFT_EXP
+#define DFT_EXP 0          // perf-only experiments (wrong results): 1 no stores, 2 no A tile stores, 3 no epilogue work
+#endif
+
 namespace {
 
 constexpr int DF_THREADS = 576;          // 18 warps: W loader, MMA issuer, 8 epilogue, 8 converters
@@ -34,6 +38,9 @@ constexpr int DF_EPI0 = 2 * 32;          // first epilogue thread
 constexpr int DF_CONV0 = 10 * 32;        // first converter thread
 constexpr int DF_NCONV = 256;            // converter threads
 constexpr int DF_MAXF4 = 13;             // float4 per converter thread: ceil(100 * 32 / 256)
+constexpr int DF_NPH = 100;              // fine columns per charge pixel (S = 10)
+constexpr int DF_KP16 = (2 * DF_NPH + 15) / 16 * 32;          // halves per row of spectra
+constexpr int DF_FSTRIDE = RT_ROWS * DF_KP16;                 // halves between the planes of f and f + 1
 
 struct DftParams {
   int nrows, row0;              // compact rows of the chunk: row_m2[row0 .. row0 + nrows); read from rt_desc
@@ -44,7 +51,8 @@ struct DftParams {
   const int32_t* row_m2;
   const int32_t* blockmap;
   const float* payload;
-  __half* qh;                   // [nf][rp][kp16]
+  __half* qh;                   // [tile][nf][128][kp16]: the (row tile, frequency) box the spectrum product loads
+                                // is one contiguous 104 KB run
   float* rscale;                // [rp]
   TredGrid g;
   int nstrip;
@@ -119,14 +127,15 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
   uint8_t* a_ptr = base_ptr + (sAt - base);
   const uint32_t abytes = (uint32_t)p.nkc * 16384u;
   const uint32_t bars = sAt + abytes;
-  const uint32_t wbar = bars, afull = bars + 8, aempty = bars + 16, alocal = bars + 24;
-  auto tfull_bar = [&](int a) { return bars + 32u + 8u * a; };
-  auto tempty_bar = [&](int a) { return bars + 48u + 8u * a; };
-  const uint32_t rcons = bars + 64;                                    // the epilogue has read rowinfo
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(a_ptr + abytes + 72);
-  int* rowinfo = reinterpret_cast<int*>(a_ptr + abytes + 80);          // padded row of the A tile or -1
-  float* red = reinterpret_cast<float*>(a_ptr + abytes + 96);          // [8] converter warp sums
-  long long* colbase = reinterpret_cast<long long*>(a_ptr + abytes + 128);   // [100]
+  const uint32_t wbar = bars, alocal = bars + 8, rcons = bars + 16;   // rcons: the epilogue has read rowinfo
+  auto tfull_bar = [&](int a) { return bars + 24u + 8u * a; };
+  auto tempty_bar = [&](int a) { return bars + 40u + 8u * a; };
+  auto afull_bar = [&](int kc) { return bars + 56u + 8u * kc; };      // leader: K chunk kc of both A tiles stored
+  auto aempty_bar = [&](int kc) { return bars + 88u + 8u * kc; };     // the tensor core is done with K chunk kc
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(a_ptr + abytes + 120);
+  int* rowinfo = reinterpret_cast<int*>(a_ptr + abytes + 124);         // padded row of the A tile or -1
+  float* red = reinterpret_cast<float*>(a_ptr + abytes + 128);         // [8] converter warp sums
+  long long* colbase = reinterpret_cast<long long*>(a_ptr + abytes + 160);   // [100]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
@@ -140,8 +149,7 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
 
   if (threadIdx.x == 0) {
     mbar_init(wbar, 1);
-    mbar_init(afull, 2);          // leader: one arrival per CTA
-    mbar_init(aempty, 1);
+    for (int kc = 0; kc < 4; ++kc) { mbar_init(afull_bar(kc), 2); mbar_init(aempty_bar(kc), 1); }
     mbar_init(alocal, 1);
     mbar_init(rcons, 1);
     for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2); }
@@ -173,13 +181,15 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
       const uint32_t idesc = (1u << 4) | ((uint32_t)(p.NC >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
       int aphase = 0, acc = 0, tphase = 0;
       for (int pr = cid; pr < npairs; pr += ncl) {
-        mbar_wait(afull, aphase);                              // both CTAs: A tile stored (and W resident)
-        tc_fence_after();
         for (int nc = 0; nc < p.nnc; ++nc) {
           mbar_wait(tempty_bar(acc), tphase ^ 1);
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + (uint32_t)(acc * 256);
           for (int kc = 0; kc < p.nkc; ++kc) {
+            if (nc == 0) {                                       // both CTAs: K chunk stored (and W resident)
+              mbar_wait(afull_bar(kc), aphase);
+              tc_fence_after();
+            }
             const uint64_t da = desc_sw128(sAt + (uint32_t)kc * 16384u);
             const uint64_t db = desc_sw128(sW + (uint32_t)(nc * p.nkc + kc) * bstage);
 #pragma unroll
@@ -189,11 +199,11 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
               tc_mma_f16_pair2(d_tmem, da + lo, db + hi, idesc, 1);
               tc_mma_f16_pair2(d_tmem, da + hi, db + lo, idesc, 1);
             }
+            if (nc == p.nnc - 1) tc_commit_pair(aempty_bar(kc)); // this K chunk of both A tiles may be overwritten
           }
           tc_commit_pair(tfull_bar(acc));
           if (++acc == 2) { acc = 0; tphase ^= 1; }
         }
-        tc_commit_pair(aempty);                                // the A tiles of both CTAs may be overwritten
         aphase ^= 1;
       }
     }
@@ -209,7 +219,8 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
     const bool padlane = col == NPH && (2 * NPH) % 16 != 0;     // zeroes the padding reals of the last block
     const int pos = (col >> 3) * 32 + (col & 7) * 2;            // hi part of (re, im); lo 16 halves further
     const int padpos = ((2 * NPH) >> 4) * 32 + ((2 * NPH) & 15);
-    const int64_t fstride = (int64_t)p.rp * p.kp16;
+    constexpr int fstride = DF_FSTRIDE;                         // qh is [tile][f][128 rows][kp16]: compile-time
+                                                                // stride, the 16 stores of a group use immediates
     int lphase = 0, acc = 0, tphase = 0;
     for (int pr = cid; pr < npairs; pr += ncl) {
       group_wait(alocal, lphase, poller, 1, 256);
@@ -217,7 +228,9 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
       const int prow = *reinterpret_cast<volatile int*>(rowinfo);
       asm volatile("bar.sync 1, 256;" ::: "memory");
       if (et == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(rcons) : "memory");
-      __half* orow = p.qh + (int64_t)(prow < 0 ? 0 : prow) * p.kp16 + (live ? pos : padpos);
+      const int prow0 = prow < 0 ? 0 : prow;
+      __half* orow = p.qh + ((int64_t)(prow0 >> 7) * p.nf * RT_ROWS + (prow0 & (RT_ROWS - 1))) * p.kp16 +
+                     (live ? pos : padpos);
       for (int nc = 0; nc < p.nnc; ++nc) {
         group_wait(tfull_bar(acc), tphase, poller, 1, 256);
         tc_fence_after();
@@ -226,23 +239,25 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
           uint32_t v[32];
           tmem_ld32(v, taddr + (uint32_t)(g * 32));
           asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          if (prow >= 0 && (live || padlane)) {
+          if (DFT_EXP != 3 && prow >= 0 && (live || padlane)) {
             __half* o = orow + (int64_t)(nc * (p.NC >> 1) + g * 16) * fstride;
             if (live) {
 #pragma unroll
-              for (int i = 0; i < 16; ++i, o += fstride) {
+              for (int i = 0; i < 16; ++i) {
                 const float re = __uint_as_float(v[2 * i]), im = __uint_as_float(v[2 * i + 1]);
                 const __half2 h = __floats2half2_rn(re, im);
                 const float2 hf = __half22float2(h);
                 const __half2 l = __floats2half2_rn(re - hf.x, im - hf.y);
-                *reinterpret_cast<__half2*>(o) = h;
-                *reinterpret_cast<__half2*>(o + 16) = l;
+                if (DFT_EXP != 1 || re == 12345.678f) {
+                  *reinterpret_cast<__half2*>(o + i * fstride) = h;
+                  *reinterpret_cast<__half2*>(o + i * fstride + 16) = l;
+                }
               }
             } else {
 #pragma unroll
-              for (int i = 0; i < 16; ++i, o += fstride) {
-                *reinterpret_cast<uint4*>(o) = make_uint4(0u, 0u, 0u, 0u);
-                *reinterpret_cast<uint4*>(o + 16) = make_uint4(0u, 0u, 0u, 0u);
+              for (int i = 0; i < 16; ++i) {
+                *reinterpret_cast<uint4*>(o + i * fstride) = make_uint4(0u, 0u, 0u, 0u);
+                *reinterpret_cast<uint4*>(o + i * fstride + 16) = make_uint4(0u, 0u, 0u, 0u);
               }
             }
           }
@@ -256,11 +271,15 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
   } else {
     // ------------------------------------------------------------ converters: payload -> A tile
     const int tc = threadIdx.x - DF_CONV0;                     // 0 .. 255
-    const bool poller = warp == 10;
     const int cw = tc >> 5;
     const int NPH = p.g.nph, S = p.g.S;
-    const int nq = p.Bt >> 2;                                  // float4 per column
-    const int nf4 = NPH * nq;
+    // K chunk kc (32 ticks = 8 float4 per column) belongs to a group of 8 / nkc warps: it waits
+    // for, fills and hands over its quarter of the A tile on its own
+    const int TG = DF_NCONV / p.nkc;                           // threads per group
+    const int kc = tc / TG, l = tc - kc * TG;
+    const bool poller = l < 32;
+    const uint32_t gbar = 3 + kc;
+    const int nf4 = NPH * 8;
     int ephase = 0;
     int tile = p.t0;
     bool first = true;
@@ -268,32 +287,28 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
       const int c = 2 * pr + (int)rank;
       const bool exists = c < p.nrows;
       int prow = -1;
-      if (exists) {
-        const int gr = p.row0 + c;
-        if (tc < NPH) {
-          const int m2 = p.row_m2[gr];
-          const int rest = m2 >> 3;
-          const int py = rest % p.g.npy, grp = rest / p.g.npy;
-          const int bt = grp / p.nstrip;
-          const int px = (grp - bt * p.nstrip) * RT_SW + (m2 & (RT_SW - 1));
-          const int i = px * S + tc / S, j = py * S + tc % S;
-          const int bx = i / p.g.Bx, by = j / p.g.By;
-          const int slot = p.blockmap[((int64_t)bt * p.g.NBx + bx) * p.g.NBy + by];
-          colbase[tc] = slot >= 0 ? (((long long)slot * p.g.Bx + (i - bx * p.g.Bx)) * p.g.By + (j - by * p.g.By)) * p.Bt
-                                  : -1;
-        }
+      if (exists && tc < NPH) {
+        const int m2 = p.row_m2[p.row0 + c];
+        const int rest = m2 >> 3;
+        const int py = rest % p.g.npy, grp = rest / p.g.npy;
+        const int bt = grp / p.nstrip;
+        const int px = (grp - bt * p.nstrip) * RT_SW + (m2 & (RT_SW - 1));
+        const int i = px * S + tc / S, j = py * S + tc % S;
+        const int bx = i / p.g.Bx, by = j / p.g.By;
+        const int slot = p.blockmap[((int64_t)bt * p.g.NBx + bx) * p.g.NBy + by];
+        colbase[tc] = slot >= 0 ? (((long long)slot * p.g.Bx + (i - bx * p.g.Bx)) * p.g.By + (j - by * p.g.By)) * p.Bt
+                                : -1;
       }
       asm volatile("bar.sync 2, 256;" ::: "memory");
       float4 v[DF_MAXF4];
       float sum = 0.0f;
 #pragma unroll
       for (int i = 0; i < DF_MAXF4; ++i) {
-        const int idx = tc + DF_NCONV * i;
+        const int idx = l + TG * i;
         v[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (exists && idx < nf4) {
-          const int cc = idx / nq, q4 = idx - cc * nq;
-          const long long b = colbase[cc];
-          if (b >= 0) v[i] = __ldg(reinterpret_cast<const float4*>(p.payload + b) + q4);
+          const long long b = colbase[idx >> 3];
+          if (b >= 0) v[i] = __ldg(reinterpret_cast<const float4*>(p.payload + b) + 8 * kc + (idx & 7));
         }
         sum += (fabsf(v[i].x) + fabsf(v[i].y)) + (fabsf(v[i].z) + fabsf(v[i].w));
       }
@@ -313,20 +328,21 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
       for (int w = 1; w < 8; ++w) tot += red[w];
       const float sc = dft_h16_scale(tot);
       const float sdown = __uint_as_float((254u - (__float_as_uint(sc) >> 23)) << 23);
-      // the tensor core must be done with the previous row before its tile is overwritten
-      if (!first) { group_wait(aempty, ephase, poller, 2, 256); ephase ^= 1; }
+      // the tensor core must be done with this K chunk of the previous row before it is overwritten
+      if (!first) { group_wait(aempty_bar(kc), ephase, poller, gbar, TG); ephase ^= 1; }
 #pragma unroll
       for (int i = 0; i < DF_MAXF4; ++i) {
-        const int idx = tc + DF_NCONV * i;
+        const int idx = l + TG * i;
         if (idx < nf4) {
-          const int cc = idx / nq, q4 = idx - cc * nq;
-          const int t0 = 4 * q4;
+          const int cc = idx >> 3;
+          const int t0 = 4 * (idx & 7);                          // tick within the K chunk
           const float x0 = v[i].x * sdown, x1 = v[i].y * sdown, x2 = v[i].z * sdown, x3 = v[i].w * sdown;
           const __half2 h01 = __floats2half2_rn(x0, x1), h23 = __floats2half2_rn(x2, x3);
           const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
           const __half2 l01 = __floats2half2_rn(x0 - f01.x, x1 - f01.y), l23 = __floats2half2_rn(x2 - f23.x, x3 - f23.y);
           // K chunk of 32 ticks = one 128-byte row: [hi 16 | lo 16 | hi 16 | lo 16]; 16-byte units swizzled by row
-          const int kc = t0 >> 5, off = ((t0 >> 4) & 1) * 64 + (t0 & 15) * 2;
+          const int off = (t0 >> 4) * 64 + (t0 & 15) * 2;
+          if (DFT_EXP == 2 && x0 != 12345.678f) continue;
           uint8_t* rowp = a_ptr + kc * 16384 + cc * 128;
           const int u_hi = (off >> 4) ^ (cc & 7), u_lo = ((off + 32) >> 4) ^ (cc & 7);
           *reinterpret_cast<uint2*>(rowp + u_hi * 16 + (off & 15)) =
@@ -341,11 +357,11 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
         *reinterpret_cast<volatile int*>(rowinfo) = prow;
         if (prow >= 0) p.rscale[prow] = sc;
       }
-      asm volatile("bar.sync 2, 256;" ::: "memory");
-      if (tc == 0) {
+      asm volatile("bar.sync %0, %1;" ::"r"(gbar), "r"(TG) : "memory");
+      if (l == 0) {
         if (first) mbar_wait(wbar, 0);                          // this CTA's half of W has landed
-        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(alocal) : "memory");
-        mbar_arrive_cluster(mapa(afull, 0));
+        if (tc == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(alocal) : "memory");
+        mbar_arrive_cluster(mapa(afull_bar(kc), 0));
       }
       first = false;
     }
@@ -410,12 +426,12 @@ static int dft_nchunk(int L) {
 static size_t dft_smem(const tred_ctx* ctx) {
   const int L = ctx->dims.fft_len, Bt = ctx->cfg.block[2];
   const size_t wbytes = (size_t)(L / 2) * Bt * 4;               // half of the matrix, hi + lo
-  return 1024 + ((wbytes + 1023) & ~(size_t)1023) + (size_t)(Bt / 32) * 16384 + 128 + 100 * 8 + 64;
+  return 1024 + ((wbytes + 1023) & ~(size_t)1023) + (size_t)(Bt / 32) * 16384 + 160 + 100 * 8 + 64;
 }
 
 bool tred_dft_h16_supported(const tred_ctx* ctx) {
   const int Bt = ctx->cfg.block[2];
-  return ctx->dims.n_phase == 100 && ctx->cfg.sub == 10 && Bt >= 32 && Bt <= 128 && (Bt % 32) == 0 &&
+  return ctx->dims.n_phase == DF_NPH && h16_kp(ctx->dims) == DF_KP16 && ctx->cfg.sub == 10 && Bt >= 32 && Bt <= 128 && (Bt % 32) == 0 &&
          dft_nchunk(ctx->dims.fft_len) > 0 && dft_smem(ctx) <= (size_t)ctx->smem_optin && ctx->num_sms >= 2 &&
          get_encode_fn_df() != nullptr;
 }
@@ -432,7 +448,7 @@ int tred_dft_matrix(tred_ctx* ctx, void* d_Wd, cudaStream_t st) {
 }
 
 // Spectra of the compact rows [row0, row0 + nrows) of the chunk's row tiles [t0, t0 + ntile):
-// qh [nf][ntile * 128][kp16] fp16 hi / lo blocks, rscale [ntile * 128].
+// qh [ntile][nf][128][kp16] fp16 hi / lo blocks, rscale [ntile * 128].
 int tred_dft_h16(tred_ctx* ctx, const float* payload, const int32_t* blockmap, const void* rt_desc,
                  const int32_t* row_m2, int t0, int ntile, int nstrip, const void* d_Wd,
                  void* qh, float* rscale, cudaStream_t st) {

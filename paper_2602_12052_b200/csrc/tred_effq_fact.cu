@@ -788,12 +788,12 @@ int tred_effq_init_tables(void) {
 // (Bt ticks) its clipped footprint [lo - e, hi + e] reaches.  With the factored form of the
 // charge the sum over a pixel x tile box factors too:
 //   Q[s][px][py][tb] = sum_m (K W_m sum_{i in px} GX_m[i]) (sum_{j in py} GY_m[j]) (sum_{k in tb} GT_m[k]).
-constexpr int TR_MAXG = 16;          // pixel / tile groups per axis a segment may reach
+constexpr int TR_MAXG = 32;          // pixel / tile groups per axis a segment may reach (more: reported, see tred_truth)
 
 struct TruthBox { int lo[3], hi[3], g0[3], ng[3]; };
 
 __device__ __forceinline__ bool truth_box(const int32_t* __restrict__ augi, int64_t nseg, int64_t s, const TredGrid& g,
-                                          int E, TruthBox& b) {
+                                          int E, TruthBox& b, bool* over = nullptr) {
   const int NG[3] = {g.NGx, g.NGy, g.NGt}, div[3] = {g.S, g.S, g.Bt};
   bool ok = true;
   for (int a = 0; a < 3; ++a) {
@@ -802,19 +802,23 @@ __device__ __forceinline__ bool truth_box(const int32_t* __restrict__ augi, int6
     ok = ok && b.lo[a] <= b.hi[a];
     b.g0[a] = b.lo[a] / div[a];
     b.ng[a] = ok ? min(b.hi[a] / div[a] - b.g0[a] + 1, TR_MAXG) : 0;
+    if (over && ok && b.hi[a] / div[a] - b.g0[a] + 1 > TR_MAXG) *over = true;
   }
   return ok;
 }
 
 template <int N>
 __global__ void __launch_bounds__(256)
-k_truth_count(int64_t nseg, const int32_t* __restrict__ augi, TredGrid g, int32_t* __restrict__ cnt) {
+k_truth_count(int64_t nseg, const int32_t* __restrict__ augi, TredGrid g, int32_t* __restrict__ cnt,
+              int32_t* __restrict__ over_flag) {
   const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s > nseg) return;
   int c = 0;
   if (s < nseg) {
     TruthBox b;
-    if (truth_box(augi, nseg, s, g, N > 1 ? 1 : 0, b)) c = b.ng[0] * b.ng[1] * b.ng[2];
+    bool over = false;
+    if (truth_box(augi, nseg, s, g, N > 1 ? 1 : 0, b, &over)) c = b.ng[0] * b.ng[1] * b.ng[2];
+    if (over) atomicOr(over_flag, 1);            // a segment reaches more groups than a record holds
   }
   cnt[s] = c;
 }
@@ -824,11 +828,12 @@ template <int N>
 __global__ void __launch_bounds__(128)
 k_truth_fill(int64_t nseg, const float* __restrict__ augf, const int32_t* __restrict__ augi,
              const int32_t* __restrict__ first, TredGrid g, int64_t cap, int32_t* __restrict__ rec_seg,
-             int64_t* __restrict__ rec_key, float* __restrict__ rec_q, int64_t* __restrict__ d_nrec) {
+             int64_t* __restrict__ rec_key, float* __restrict__ rec_q, int64_t* __restrict__ d_nrec,
+             const int32_t* __restrict__ over_flag) {
   __shared__ float sums[4][3 * TR_MAXG][MMAX];
   const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t s = (int64_t)blockIdx.x * 4 + wid;
-  if (blockIdx.x == 0 && threadIdx.x == 0) *d_nrec = first[nseg];
+  if (blockIdx.x == 0 && threadIdx.x == 0) *d_nrec = *over_flag ? -1 : (int64_t)first[nseg];
   if (s >= nseg) return;
   constexpr int E = N > 1 ? 1 : 0;
   constexpr float LOG2E_HALF = 0.72134752044448170f;
@@ -1027,7 +1032,7 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
 
 extern "C" size_t tred_truth_work_bytes(const tred_ctx* ctx, int64_t nseg) {
   if (!ctx || nseg < 0) return 0;
-  return align_up((size_t)(nseg + 1) * 4, 256) + tred_scan_work_bytes(nseg + 1);
+  return align_up((size_t)(nseg + 1) * 4, 256) + tred_scan_work_bytes(nseg + 1) + 256;
 }
 
 extern "C" int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, const int32_t* d_augi, int64_t cap_rec,
@@ -1042,13 +1047,15 @@ extern "C" int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, cons
   const TredGrid g = make_grid(ctx);
   int32_t* first = (int32_t*)d_work;
   void* scan = (char*)d_work + align_up((size_t)(nseg + 1) * 4, 256);
+  int32_t* over = (int32_t*)((char*)scan + tred_scan_work_bytes(nseg + 1));
+  TRED_CUDA(cudaMemsetAsync(over, 0, 4, st));
 #define TRUTH(NN)                                                                                          \
   do {                                                                                                     \
-    k_truth_count<NN><<<cdiv(nseg + 1, 256), 256, 0, st>>>(nseg, d_augi, g, first);                        \
+    k_truth_count<NN><<<cdiv(nseg + 1, 256), 256, 0, st>>>(nseg, d_augi, g, first, over);                  \
     int rc = tred_exclusive_scan_i32(first, first, nseg + 1, nullptr, scan, st);                           \
     if (rc != TRED_OK) return rc;                                                                          \
     k_truth_fill<NN><<<cdiv(nseg, 4), 128, 0, st>>>(nseg, d_augf, d_augi, first, g, cap_rec, d_rec_seg,     \
-                                                    d_rec_key, d_rec_q, d_nrec);                           \
+                                                    d_rec_key, d_rec_q, d_nrec, over);                     \
   } while (0)
   switch (g.gl_n) {
     case 1: TRUTH(1); break;

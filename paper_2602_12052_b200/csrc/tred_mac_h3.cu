@@ -142,13 +142,13 @@ k_mac_h3(const __grid_constant__ H3Maps tm, H3Params p) {
         if (item + ncl < nitems) {
           const int fn = (item + ncl) / p.npair, prn = (item + ncl) - fn * p.npair;
           const int mtn = min(2 * prn + (int)rank, p.ntile - 1);
-          for (int kc = 0; kc < nkc; ++kc) tma_prefetch_3d(&tm.a, kc * 64, mtn * T2_M, fn);
+          for (int kc = 0; kc < nkc; ++kc) tma_prefetch_3d(&tm.a, kc * 64, 0, mtn * p.nf + fn);
         }
         for (int kc = 0; kc < nkc; ++kc) {
           mbar_wait(empty_bar(stage), phase ^ 1);
           const uint32_t fb = mapa(full_bar(stage), 0);            // the leader's barrier
           mbar_expect_tx_cluster(fb, tx);
-          tma_load_3d_pair(sA(stage), &tm.a, kc * 64, mt * T2_M, f, fb);
+          tma_load_3d_pair(sA(stage), &tm.a, kc * 64, 0, mt * p.nf + f, fb);
           tma_load_3d_pair(sB(stage), &tm.b, kc * 64, (int)rank * nh, f, fb);
           if (++stage == H3_STAGES) { stage = 0; phase ^= 1; }
         }
@@ -373,7 +373,7 @@ bool tred_mac_h3_supported(const tred_ctx* ctx) {
          ctx->cfg.resp_half <= RT_MAXH && ctx->num_sms >= 2 && get_encode_fn_h3() != nullptr;
 }
 
-// qh: [nf][ntile * 128][kp16] fp16 in the hi / lo block layout (kp16 = h16_kp(dims)), rscale
+// qh: [ntile][nf][128][kp16] fp16 in the hi / lo block layout (kp16 = h16_kp(dims)), rscale
 // [ntile * 128]; Bh16: [nf][N][kp16] fp16, bscale [nf].  Same outputs as tred_mac_tc2.
 int tred_mac_h3(tred_ctx* ctx, const void* qh, const float* rscale, const void* Bh16, const float* bscale,
                 float* opart, int ntile, int t0, const void* rt_desc, const int32_t* row_m2, cudaStream_t st) {
@@ -384,7 +384,8 @@ int tred_mac_h3(tred_ctx* ctx, const void* qh, const float* rscale, const void* 
   if ((((uintptr_t)qh) | ((uintptr_t)Bh16)) & 15) return TRED_EUNSUPPORTED;
   PFN_encodeTiledH3 enc = get_encode_fn_h3();
   H3Maps tm;
-  if (!make_map_h3(enc, &tm.a, qh, kp16, (int64_t)ntile * T2_M, d.n_freq, T2_M) ||
+  if ((int64_t)ntile * d.n_freq >= (1ll << 31)) return TRED_EUNSUPPORTED;
+  if (!make_map_h3(enc, &tm.a, qh, kp16, T2_M, ntile * d.n_freq, T2_M) ||
       !make_map_h3(enc, &tm.b, Bh16, kp16, N, d.n_freq, N / 2))
     return TRED_EUNSUPPORTED;
   TRED_CUDA(cudaFuncSetAttribute(k_mac_h3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)H3_SMEM));

@@ -54,8 +54,11 @@ def test_dims_host_logic(cfg_id, L, nover, ppb):
     assert list(d.NG) == [cfg.sub * cfg.npix_x, cfg.sub * cfg.npix_y, cfg.nticks]
     assert list(d.NB) == [-(-d.NG[a] // cfg.block[a]) for a in range(3)]
     assert (d.n_phase, d.n_off, d.n_off_pad) == (100, 121, 128)
-    # fp32 spectrum + tf32 hi/lo matrices + the four mirror-symmetric half matrices + flag
-    assert d.rhat_floats == 14 * (L // 2) * 100 * 128 + 4 * (L // 2) * 128 * 100 + 8
+    # fp32 spectrum + tf32 hi/lo matrices + the four mirror-symmetric half matrices + flag + the fp16
+    # hi/lo matrix [f][256][13 blocks of 32 halves] and its scales + the DFT matrix [L][2 Bt] halves
+    nf = L // 2
+    assert d.rhat_floats == 14 * nf * 100 * 128 + 4 * nf * 128 * 100 + 8 + nf * 256 * 208 + (nf + 7) // 8 * 8 + \
+        L * cfg.block[2]
     assert d.conv_row_bytes == (L // 2) * (100 + 128) * 8
 
 

@@ -6,7 +6,8 @@ Tolerances (DESIGN.md "Tolerances"):
   effective charge (fp32 vs fp64): max|d| <= 2e-5 max|Qeff|, total within 1e-5;
   waveforms: max|d| <= 1e-4 max|signal| (north_star);
   per-pixel integrated charge (north_star: relative 1e-5):
-      collecting pixels (|Q_p| >= L1_p / 2, L1_p = sum_t |I_p(t)|: a mostly unipolar pulse, and
+      collecting pixels (|Q_p| >= L1_p / 10, L1_p = sum_t |I_p(t)|: the collection pulse is not
+      buried under the bipolar induction of the neighbours, and
       |Q_p| >= 1e-3 max|Q|):  |dQ_p| <= 1e-5 |Q_p|, nothing added;
       every other pixel integrates a bipolar induction pulse to ~0 by cancellation, where a
       relative bound is undefined (reading G17): |dQ_p| <= c 2^-24 L1_p with c from the error
@@ -14,6 +15,8 @@ Tolerances (DESIGN.md "Tolerances"):
       the fp32 FMA product, plus 3/16 per truncating tensor-core accumulation of the product
       that ran (75 for the tf32 products, 52 for tf32 + 2 x bf16, 39 for the three fp16 products).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -232,7 +235,7 @@ def _wave_checks(got, ref, mode):
     qg, qr = got.sum(1), ref.sum(1)
     l1 = np.abs(ref).sum(1)
     dq = np.abs(qg - qr)
-    coll = (np.abs(qr) >= 0.5 * l1) & (np.abs(qr) >= 1e-3 * np.abs(qr).max())
+    coll = (np.abs(qr) >= 0.1 * l1) & (np.abs(qr) >= 1e-3 * np.abs(qr).max())
     assert (dq[coll] <= TOL_QPIX * np.abs(qr)[coll]).all(), (dq[coll] / np.abs(qr)[coll]).max()
     assert (dq[~coll] <= tol_qpix_l1(mode) * l1[~coll]).all(), (dq[~coll] / l1[~coll]).max() * 2.0 ** 24
     # pixels the oracle leaves exactly empty stay exactly empty
@@ -509,49 +512,122 @@ def test_readout_parity(with_noise):
     assert int(readout(z, par)[0].sum()) == 0
 
 
-# ------------------------------------------------------------------ full size (config 3)
-def test_full_size_config3_sampled_pixels():
-    """BASELINE config 3 at full size, in the configuration bench.py times: all integer outputs
-    (block keys, output tile keys) bit-exact in full; waveforms and effective charge on sampled
-    pixels, which the oracle can compute one neighbourhood at a time (only the blocks within
-    the response's reach of a pixel contribute to it)."""
+# ------------------------------------------------------------------ full size (configs 3 and 4)
+# Neighbourhoods checked against the oracle at full size.  The oracle needs about a minute per
+# neighbourhood (every segment within the response's reach, all time slabs), so the default keeps the
+# suite short; TRED_FULL_NEIGHBOURHOODS=16 runs the wide sample (its log is kept under profiles/).
+NFULL = int(os.environ.get("TRED_FULL_NEIGHBOURHOODS", "4"))
+
+
+def _check_neighbourhoods(cfg, aug, keys, R, groups, dense, mode, payload_rows=None):
+    """Waveforms of every pixel group against the oracle run on the blocks within the response's
+    reach of the group (only those contribute), and the effective charge of those blocks."""
     torch = _torch()
-    cfg, segs = gen.make_segments(3)
-    R = gen.make_response(cfg, 2003)
-    aug = o.drift(cfg, segs)
-    keys = o.blocks(cfg, aug)
-    tiles = o.out_tiles(cfg, keys)
     g = o.grid_of(cfg)
     npy, S, H = cfg.npix_y, cfg.sub, cfg.resp_half
-    rng = np.random.default_rng(33)
-    act = np.unique(tiles % (cfg.npix_x * cfg.npix_y))
-    centres = rng.choice(act[(act // npy > 8) & (act // npy < cfg.npix_x - 8) &
-                             (act % npy > 8) & (act % npy < npy - 8)], 2, replace=False)
-    groups = [np.array([c, c + 1, c + npy], dtype=np.int64) for c in centres]
-    pix_all = np.concatenate(groups)
-    sim = _sim(cfg)
-    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
-    out = sim.simulate(_seg_tensor(segs), rhat, torch.from_numpy(pix_all.astype(np.int32)).cuda(), keep=True)
-    assert out["nblocks"] == len(keys)
-    gk = out["keys"].cpu().numpy()
-    np.testing.assert_array_equal(gk, keys)
-    np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
-    dense = out["dense"].cpu().numpy().astype(np.float64)
     bx, by, bt = o.key_to_bxyz(g, keys)
     Bx, By = cfg.block[0], cfg.block[1]
-    for gi, grp in enumerate(groups):
+    row = 0
+    for grp in groups:
         px, py = grp // npy, grp % npy
-        # blocks whose pixel span reaches any pixel of the group through the (2H+1)^2 response
         m = ((Bx * bx + Bx - 1) // S >= px.min() - H) & ((Bx * bx) // S <= px.max() + H) & \
             ((By * by + By - 1) // S >= py.min() - H) & ((By * by) // S <= py.max() + H)
         kk = keys[m]
         sel = o.segments_touching(cfg, aug, kk)
         payload = o.effq(cfg, aug, kk, sel)
         ref = o.conv_fft(cfg, kk, payload, R, grp)
-        _wave_checks(dense[3 * gi: 3 * gi + 3], ref, sim.last_mac_mode())
-        # effective charge of the same blocks
-        got_q = out["payload"][torch.from_numpy(np.flatnonzero(m)).cuda()].cpu().numpy().astype(np.float64)
-        assert np.abs(got_q - payload).max() <= TOL_QEFF * np.abs(payload).max()
+        _wave_checks(dense[row: row + len(grp)], ref, mode)
+        row += len(grp)
+        if payload_rows is not None:
+            got_q = payload_rows[torch.from_numpy(np.flatnonzero(m)).cuda()].cpu().numpy().astype(np.float64)
+            assert np.abs(got_q - payload).max() <= TOL_QEFF * np.abs(payload).max()
+
+
+def _pick_groups(cfg, tiles, n, seed):
+    npy = cfg.npix_y
+    rng = np.random.default_rng(seed)
+    act = np.unique(tiles % (cfg.npix_x * npy))
+    inner = act[(act // npy > 8) & (act // npy < cfg.npix_x - 8) & (act % npy > 8) & (act % npy < npy - 8)]
+    centres = rng.choice(inner, n, replace=False)
+    return [np.array([c, c + npy], dtype=np.int64) for c in centres]
+
+
+def test_full_size_config3_sampled_pixels():
+    """BASELINE config 3 at full size, in the configuration bench.py times: all integer outputs
+    (block keys, output tile keys) bit-exact in full; waveforms and effective charge on sampled
+    pixel neighbourhoods, which the oracle can compute one at a time."""
+    torch = _torch()
+    cfg, segs = gen.make_segments(3)
+    R = gen.make_response(cfg, 2003)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    tiles = o.out_tiles(cfg, keys)
+    groups = _pick_groups(cfg, tiles, NFULL, 33)
+    pix_all = np.concatenate(groups)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    out = sim.simulate(_seg_tensor(segs), rhat, torch.from_numpy(pix_all.astype(np.int32)).cuda(), keep=True)
+    assert out["nblocks"] == len(keys)
+    np.testing.assert_array_equal(out["keys"].cpu().numpy(), keys)
+    np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
+    dense = out["dense"].cpu().numpy().astype(np.float64)
+    _check_neighbourhoods(cfg, aug, keys, R, groups, dense, sim.last_mac_mode(), out["payload"])
+    # the one-call path (tred_simulate) gives the same bits as the stepwise calls
+    one = sim.simulate(_seg_tensor(segs), rhat, torch.from_numpy(pix_all.astype(np.int32)).cuda())
+    assert torch.equal(one["tile_keys"], out["tile_keys"]) and torch.equal(one["dense"], out["dense"])
+
+
+def test_full_size_config4_chunked():
+    """BASELINE config 4 at full size (10 overlaid spills, ~10.5 M segments, 700 x 700 pixels), run as
+    bench.py runs it: slab-range chunks under a 7 GiB payload budget and a 5 GiB convolution
+    workspace.  The tile list is compared in full with the oracle's, the waveforms on sampled
+    neighbourhoods (chunking must not change the result)."""
+    torch = _torch()
+    cfg, segs = gen.make_segments(4)
+    R = gen.make_response(cfg, 2004)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    tiles = o.out_tiles(cfg, keys)
+    groups = _pick_groups(cfg, tiles, max(1, NFULL // 4), 44)
+    pix_all = np.concatenate(groups)
+    sim = _sim(cfg, conv_work_bytes=5 << 30)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    torch.cuda.reset_peak_memory_stats()
+    out = sim.simulate_chunked(_seg_tensor(segs), rhat, torch.from_numpy(pix_all.astype(np.int32)).cuda(),
+                               payload_budget_bytes=7 << 30)
+    torch.cuda.synchronize()
+    assert out["chunks"] >= 9 and out["nblocks"] == len(keys)
+    assert torch.cuda.max_memory_allocated() <= 40e9                     # BASELINE: peak memory <= 40 GB
+    np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
+    dense = out["dense"].cpu().numpy().astype(np.float64)
+    _check_neighbourhoods(cfg, aug, keys, R, groups, dense, sim.last_mac_mode())
+
+
+def test_dense_grid_equals_block_sparse():
+    """BASELINE config 5's comparison point as a test: the convolution of the WHOLE plane on the dense
+    grid (one 3-D FFT per sub-pixel phase, the paper's Eq. (14) as printed; torch.fft
+    on the GPU as a library step of the check) equals the block-sparse result on every pixel of a
+    reduced plane -- only blocks with activity matter."""
+    torch = _torch()
+    import bench
+    cfg, segs = gen.make_segments(2)
+    cfg = cfg.with_(npix_x=48, npix_y=40, nticks=1024)
+    segs = {k: v[:1500].copy() for k, v in segs.items()}
+    for a, n in (("x", cfg.npix_x), ("y", cfg.npix_y)):                 # fold the event into the small plane
+        for e in ("0", "1"):
+            segs[a + e] = np.mod(segs[a + e], n * cfg.pitch_mm * 0.98).astype(np.float32)
+    keep = (np.abs(segs["x1"] - segs["x0"]) < 2.0) & (np.abs(segs["y1"] - segs["y0"]) < 2.0)   # not wrapped
+    segs = {k: v[keep] for k, v in segs.items()}
+    R = gen.make_random_response(cfg, 9)
+    sim = _sim(cfg)
+    R_d = torch.from_numpy(R).cuda()
+    rhat = sim.prepare_response(R_d)
+    pix = torch.arange(cfg.npix_x * cfg.npix_y, dtype=torch.int32, device="cuda")
+    out = sim.simulate(_seg_tensor(segs), rhat, pix, keep=True)
+    assert out["nblocks"] > 50
+    rows, _, _ = bench.dense_grid_convolution(torch, cfg, out["keys"], out["payload"], R_d, pix)
+    err = float((rows - out["dense"]).abs().max() / out["dense"].abs().max())
+    assert err <= 2e-5, err
 
 
 # ------------------------------------------------------------------ N4: truth attribution
@@ -635,3 +711,30 @@ def test_truth_record_parity(cfg_id):
     gs2, gk2, gq2, nrec2 = sim.truth(augf, augi, cap_rec=7)
     assert int(nrec2.item()) == len(rs) and gs2.numel() == 7
     np.testing.assert_array_equal(gk2.cpu().numpy(), rk[:7])
+
+
+def test_truth_long_segments_and_overflow():
+    """A record holds up to 32 pixels / time tiles per axis: a 90 mm step far from the anode (about 60
+    sigma long, 22 pixels) is booked in full and matches the oracle; a 200 mm step exceeds the record
+    and is REPORTED (count -1), not truncated."""
+    import paper_2602_12052_b200 as pkg
+    cfg = gen.make_config(2)
+    rows = [(100.0, 200.0, 400.0, 190.0, 203.0, 401.0, 5.4e5, 0.0),        # 90 mm along x
+            (300.0, 100.0, 250.0, 300.5, 100.2, 290.0, 2.4e5, 0.0)]        # 40 mm along the drift: 250 ticks, 3 tiles
+    segs = {k: np.array([r[i] for r in rows], np.float32) for i, k in enumerate(gen.SEG_FIELDS)}
+    aug = o.drift(cfg, segs)
+    rs, rk, rq = o.truth_record(cfg, aug)
+    sim = _sim(cfg)
+    augf, augi, _ = sim.drift(_seg_tensor(segs))
+    gs, gk, gq, nrec = sim.truth(augf, augi)
+    assert int(nrec.item()) == len(rs) and len(rs) > 60
+    np.testing.assert_array_equal(gs.cpu().numpy(), rs)
+    np.testing.assert_array_equal(gk.cpu().numpy(), rk)
+    got = gq.cpu().numpy().astype(np.float64)
+    assert np.abs(got - rq).max() <= TOL_QEFF * np.abs(rq).max()
+    assert np.allclose(np.bincount(rs, weights=got), np.bincount(rs, weights=rq), rtol=1e-5)
+    long = {k: np.array([(100.0, 200.0, 400.0, 300.0, 203.0, 401.0, 1.2e6, 0.0)[i]], np.float32)
+            for i, k in enumerate(gen.SEG_FIELDS)}
+    augf, augi, _ = sim.drift(_seg_tensor(long))
+    with pytest.raises(pkg.TredError):
+        sim.truth(augf, augi)
