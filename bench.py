@@ -605,7 +605,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--ref-segments", type=int, default=0, help="oracle sample size (0 = per config)")
     ap.add_argument("--work-gb", type=int, default=0, help="tred_convolve workspace cap (GiB), 0 = default")
-    ap.add_argument("--budget-gb", type=int, default=7, help="config 4: block payload per chunk (GiB)")
+    ap.add_argument("--budget-gb", type=int, default=5, help="config 4: block payload per chunk (GiB)")
     ap.add_argument("--mac-mode", type=int, default=0, help="tred_config.mac_mode (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip configs 1, 2, 4 and the cuFFT comparison")

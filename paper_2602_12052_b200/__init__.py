@@ -464,6 +464,7 @@ class Tred:
             dense = self._empty((npix, self.cfg.nticks), t.float32)
         cap_tiles = getattr(self, "_cap_tiles", 0)
         want = max(getattr(self, "_sim_bytes", 0), (256 << 20) + nseg * 512)
+        tk = td = None
         for _ in range(8):
             work = self._workbuf("sim", want)
             if host_out is not None:
@@ -471,8 +472,10 @@ class Tred:
                 cap = min(tk.numel(), td.shape[0])
             else:
                 cap = cap_tiles
-                tk = self._empty((max(cap, 1),), t.int64)
-                td = self._empty((max(cap, 1), Bt), t.float32)
+                if tk is None or tk.numel() != max(cap, 1):
+                    tk = td = None                                # release before allocating the larger ones
+                    tk = self._empty((max(cap, 1),), t.int64)
+                    td = self._empty((max(cap, 1), Bt), t.float32)
             rc = self.L.tred_simulate(self.h, nseg, _ptr(seg), 0 if seg.is_cuda else 1, _ptr(rhat),
                                       int(payload_budget_bytes), _ptr(work), work.numel(), cap, _ptr(tk), _ptr(td),
                                       0 if host_out is None else 1, npix, _ptr(pix_ids), _ptr(dense), C.byref(res),
@@ -488,7 +491,7 @@ class Tred:
             if rc == -2 and res.ntiles > cap:                               # tile capacity
                 if host_out is not None:
                     raise TredError(f"host_out holds {cap} tiles, the event has {res.ntiles}")
-                cap_tiles = int(res.ntiles * 1.05) + 1024
+                cap_tiles = int(res.ntiles * 1.01) + 1024
                 continue
             _check(rc, "tred_simulate")
             break

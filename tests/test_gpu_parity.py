@@ -579,7 +579,7 @@ def test_full_size_config3_sampled_pixels():
 
 def test_full_size_config4_chunked():
     """BASELINE config 4 at full size (10 overlaid spills, ~10.5 M segments, 700 x 700 pixels), run as
-    bench.py runs it: slab-range chunks under a 7 GiB payload budget and a 5 GiB convolution
+    bench.py runs it: slab-range chunks under a 5 GiB payload budget and a 5 GiB convolution
     workspace.  The tile list is compared in full with the oracle's, the waveforms on sampled
     neighbourhoods (chunking must not change the result)."""
     torch = _torch()
@@ -594,10 +594,11 @@ def test_full_size_config4_chunked():
     rhat = sim.prepare_response(torch.from_numpy(R).cuda())
     torch.cuda.reset_peak_memory_stats()
     out = sim.simulate_chunked(_seg_tensor(segs), rhat, torch.from_numpy(pix_all.astype(np.int32)).cuda(),
-                               payload_budget_bytes=7 << 30)
+                               payload_budget_bytes=5 << 30)
     torch.cuda.synchronize()
     assert out["chunks"] >= 9 and out["nblocks"] == len(keys)
-    assert torch.cuda.max_memory_allocated() <= 40e9                     # BASELINE: peak memory <= 40 GB
+    peak = torch.cuda.max_memory_allocated()
+    assert peak <= 40e9, peak                                            # BASELINE: peak memory <= 40 GB
     np.testing.assert_array_equal(out["tile_keys"].cpu().numpy(), tiles)
     dense = out["dense"].cpu().numpy().astype(np.float64)
     _check_neighbourhoods(cfg, aug, keys, R, groups, dense, sim.last_mac_mode())
