@@ -331,6 +331,44 @@ def cufft_s4_comparison(torch, m, rows_sample: int = 8192):
             "not_included": "overlap-add over the offsets, gather of the payload columns"}
 
 
+def next_rows_overhead(torch, m, ms_step):
+    """SURVEY 8(f) rows timed on the same workload, as overhead over one step (context: the paper
+    quotes +5-10 % for truth provenance): the truth record of every segment
+    (tred_truth, counting pass + fill) and the trigger-reset readout of the whole pixel plane."""
+    from paper_2602_12052_b200 import readout
+    sim, cfg = m["sim"], m["cfg"]
+    augf, augi, _ = sim.drift(m["seg_d"])
+
+    def timed(fn, n=3):
+        fn()
+        ms = []
+        for _ in range(n):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); b.synchronize()
+            ms.append(a.elapsed_time(b))
+        return float(np.mean(ms))
+    nrec = [0]
+
+    def truth():
+        nrec[0] = int(sim.truth(augf, augi)[3].item())
+    t_truth = timed(truth)
+    out = {"truth_record_ms": t_truth, "truth_records": nrec[0], "truth_overhead": t_truth / ms_step}
+    del augf, augi
+    npix = cfg.npix_x * cfg.npix_y
+    if npix * cfg.nticks * 4 <= (8 << 30):
+        pix = torch.arange(npix, dtype=torch.int32, device=m["seg_d"].device)
+        dense = sim.simulate(m["seg_d"], m["rhat"], pix)["dense"]
+        par = dict(threshold_e=5000.0, n_integ=16, n_reset=8, max_hits=16, adc_lsb_e=0.0)
+        hits = [0]
+
+        def ro():
+            hits[0] = int(readout(dense, par)[0].sum().item())
+        t_ro = timed(ro)
+        out.update({"readout_ms": t_ro, "readout_channels": npix, "readout_hits": hits[0], "readout_overhead": t_ro / ms_step})
+        del dense
+    return out
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -466,6 +504,7 @@ def run_cuda(args):
                 "wall_s_timed_region": m["t_wall"]}
         if world == 1 and not args.no_extras:
             line["cufft_s4_comparison"] = cufft_s4_comparison(torch, m)
+            line["next_rows"] = next_rows_overhead(torch, m, ms_max)
         segs, R = m["segs"], m["R"]
         # release the main workload before the other configurations are timed
         m.clear(); sim = None

@@ -1087,11 +1087,11 @@ static int launch_fft_fwd_ct(const tred_ctx* ctx, const TredGrid& g, const float
   switch (M) {
 #define X(MM)                                                                                             \
   case MM: {                                                                                              \
-    static bool set = false;                                                                              \
-    if (!set) {                                                                                           \
+    static bool set_dev[64] = {false};                                                                              \
+    if (!set_dev[ctx->device & 63]) {                                                                                           \
       TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_ct<MM>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
                                      (int)smem));                                                         \
-      set = true;                                                                                         \
+      set_dev[ctx->device & 63] = true;                                                                                         \
     }                                                                                                     \
     k_fft_fwd_ct<MM><<<(unsigned)(nr * 5), 256, smem, st>>>(payload, blockmap, rs, rp, qhat, tw, g);      \
     return 1;                                                                                             \
@@ -1113,10 +1113,10 @@ static int launch_fft_fwd_2s_t(const tred_ctx* ctx, const TredGrid& g, const flo
   constexpr size_t smem =
       sizeof(float2) * (size_t)((20 * A * (BB + 1) > 20 * (MM + 1)) ? 20 * A * (BB + 1) : 20 * (MM + 1));
   if (smem > (size_t)ctx->smem_optin) return 0;
-  static bool set = false;
-  if (!set) {
+  static bool set_dev[64] = {false};
+  if (!set_dev[ctx->device & 63]) {
     TRED_CUDA(cudaFuncSetAttribute(k_fft_fwd_2s<MM, BB, NZA, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    set = true;
+    set_dev[ctx->device & 63] = true;
   }
   k_fft_fwd_2s<MM, BB, NZA, MODE><<<(unsigned)nr, NT, smem, st>>>(payload, blockmap, rs, rp, qhat, rscale, tw, g);
   return 1;
@@ -1166,11 +1166,11 @@ static int launch_ifft_ct(const tred_ctx* ctx, const TredGrid& g, const float2* 
   switch (M) {
 #define X(MM)                                                                                             \
   case MM: {                                                                                              \
-    static bool set = false;                                                                              \
-    if (!set) {                                                                                           \
+    static bool set_dev[64] = {false};                                                                              \
+    if (!set_dev[ctx->device & 63]) {                                                                                           \
       TRED_CUDA(cudaFuncSetAttribute(k_ifft_ct<MM, IP>, cudaFuncAttributeMaxDynamicSharedMemorySize,      \
                                      (int)smem));                                                         \
-      set = true;                                                                                         \
+      set_dev[ctx->device & 63] = true;                                                                                         \
     }                                                                                                     \
     k_ifft_ct<MM, IP><<<cdiv(ns, IP), 256, smem, st>>>(ohat, s0, ns, sbase, sp_data, tw, g, out_len);     \
     return 1;                                                                                             \

@@ -432,11 +432,11 @@ int tred_mac_tc_fused(tred_ctx* ctx, const float* qhat, const float* Bhi, const 
   if (!make_map(enc, &tmA, qhat, K2, rp, d.n_freq, TC_M) || !make_map(enc, &tmBh, Bhi, K2, N, d.n_freq, N) ||
       !make_map(enc, &tmBl, Blo, K2, N, d.n_freq, N))
     return TRED_EUNSUPPORTED;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static bool attr_set[64] = {false};
+  if (!attr_set[ctx->device & 63]) {
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_FUSED));
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<true, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_FUSED));
-    attr_set = true;
+    attr_set[ctx->device & 63] = true;
   }
   TcParams p;
   p.nf = d.n_freq; p.ntile = ntile; p.nrows = rp; p.rp = rp;
@@ -468,10 +468,10 @@ int tred_mac_tc(tred_ctx* ctx, const float* qhat, const float* Bhi, const float*
   if (!make_map(enc, &tmA, qhat, K2, rp, d.n_freq, TC_M) || !make_map(enc, &tmBh, Bhi, K2, N, d.n_freq, N) ||
       !make_map(enc, &tmBl, Blo, K2, N, d.n_freq, N))
     return TRED_EUNSUPPORTED;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static bool attr_set[64] = {false};
+  if (!attr_set[ctx->device & 63]) {
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_PLAIN));
-    attr_set = true;
+    attr_set[ctx->device & 63] = true;
   }
   TcParams p;
   p.nf = d.n_freq; p.ntile = (nrows + TC_M - 1) / TC_M; p.nrows = nrows; p.rp = rp;

@@ -425,13 +425,13 @@ int tred_mac_tc2(tred_ctx* ctx, const float* qhat, const float* Bhi, const float
     if (!make_map2(enc, &tm.bl, Blo, K2, N, d.n_freq, N / 2)) return TRED_EUNSUPPORTED;
     tm.bl2 = tm.bl;
   }
-  static bool attr_set = false;
-  if (!attr_set) {
+  static bool attr_set[64] = {false};
+  if (!attr_set[ctx->device & 63]) {
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<11, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2<11, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T2_SMEM));
-    attr_set = true;
+    attr_set[ctx->device & 63] = true;
   }
   T2Params p;
   p.nf = d.n_freq; p.ntile = ntile; p.npair = (ntile + 1) / 2;

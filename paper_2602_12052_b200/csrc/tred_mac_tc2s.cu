@@ -333,10 +333,10 @@ int tred_mac_tc2s(tred_ctx* ctx, const float* qhat, const float* Bs_hi, const fl
   };
   if (!bmap(&tm.bsh, Bs_hi) || !bmap(&tm.bsl, Bs_lo) || !bmap(&tm.bdh, Bd_hi) || !bmap(&tm.bdl, Bd_lo))
     return TRED_EUNSUPPORTED;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static bool attr_set[64] = {false};
+  if (!attr_set[ctx->device & 63]) {
     TRED_CUDA(cudaFuncSetAttribute(k_mac_tc2_sym, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S2_SMEM));
-    attr_set = true;
+    attr_set[ctx->device & 63] = true;
   }
   T2Params p;
   p.nf = d.n_freq; p.ntile = ntile; p.npair = (ntile + 1) / 2;

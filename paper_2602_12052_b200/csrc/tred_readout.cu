@@ -5,21 +5,23 @@
 //   RESET q = d_base[h], the next n_reset ticks are dead.
 // The crossing tick is an integer decided by a floating-point comparison, so the running sum
 // is a plain fp32 sum in tick order (one thread per channel; the oracle does the same).
-// One warp per 32 channels: the rows are staged chunk by chunk in shared memory with
-// coalesced loads, then every lane walks its own row.
+// One warp per 32 channels, four warps per CTA: the rows are staged chunk by chunk in shared
+// memory with coalesced loads, then every lane walks its own row.
 #include "tred_common.cuh"
 
 namespace {
 
-constexpr int RO_CH = 128;            // ticks per staged chunk
+constexpr int RO_CH = 64;             // ticks per staged chunk
+constexpr int RO_WARPS = 4;           // warps (groups of 32 channels) per CTA
 
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * RO_WARPS)
 k_readout(int64_t npix, int nticks, const float* __restrict__ wave, const float* __restrict__ noise,
           tred_readout_config c, int32_t* __restrict__ nhit, int32_t* __restrict__ hit_tick,
           float* __restrict__ hit_adc) {
-  __shared__ float tile[32][RO_CH + 1];
-  const int lane = threadIdx.x;
-  const int64_t p0 = (int64_t)blockIdx.x * 32, p = p0 + lane;
+  __shared__ float tiles[RO_WARPS][32][RO_CH + 1];
+  const int lane = threadIdx.x & 31;
+  float (*tile)[RO_CH + 1] = tiles[threadIdx.x >> 5];
+  const int64_t p0 = ((int64_t)blockIdx.x * RO_WARPS + (threadIdx.x >> 5)) * 32, p = p0 + lane;
   const bool on = p < npix;
   const int mh = c.max_hits;
   const float thr0 = (float)c.threshold_e, lsb = (float)c.adc_lsb_e;
@@ -77,9 +79,10 @@ extern "C" int tred_readout(const tred_readout_config* cfg, int64_t npix, int32_
     return TRED_EINVAL;
   if (npix == 0) return TRED_OK;
   if (!d_nhit || (nticks > 0 && !d_wave) || (cfg->max_hits > 0 && (!d_hit_tick || !d_hit_adc))) return TRED_EINVAL;
-  if ((npix + 31) / 32 >= (1ll << 31)) return TRED_EUNSUPPORTED;
+  const int64_t per_cta = 32 * RO_WARPS;
+  if ((npix + per_cta - 1) / per_cta >= (1ll << 31)) return TRED_EUNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;
-  k_readout<<<(unsigned)((npix + 31) / 32), 32, 0, st>>>(npix, nticks, d_wave, d_noise, *cfg, d_nhit, d_hit_tick,
+  k_readout<<<(unsigned)((npix + per_cta - 1) / per_cta), 32 * RO_WARPS, 0, st>>>(npix, nticks, d_wave, d_noise, *cfg, d_nhit, d_hit_tick,
                                                           d_hit_adc);
   TRED_COUNT_LAUNCH(1);
   TRED_LAUNCH_CHECK("k_readout");

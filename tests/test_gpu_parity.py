@@ -617,7 +617,10 @@ def test_dense_grid_equals_block_sparse():
     for a, n in (("x", cfg.npix_x), ("y", cfg.npix_y)):                 # fold the event into the small plane
         for e in ("0", "1"):
             segs[a + e] = np.mod(segs[a + e], n * cfg.pitch_mm * 0.98).astype(np.float32)
-    keep = (np.abs(segs["x1"] - segs["x0"]) < 2.0) & (np.abs(segs["y1"] - segs["y0"]) < 2.0)   # not wrapped
+    for e in ("0", "1"):                                                  # ... and into the short time window
+        segs["z" + e] = (10.0 + np.mod(segs["z" + e], 120.0)).astype(np.float32)
+    keep = (np.abs(segs["x1"] - segs["x0"]) < 2.0) & (np.abs(segs["y1"] - segs["y0"]) < 2.0) & \
+           (np.abs(segs["z1"] - segs["z0"]) < 2.0)                                               # not wrapped
     segs = {k: v[keep] for k, v in segs.items()}
     R = gen.make_random_response(cfg, 9)
     sim = _sim(cfg)
