@@ -1035,26 +1035,57 @@ k_ifft_ct(const float2* __restrict__ ohat, int s0, int ns, int sbase, float* __r
 #define TRED_FFT_CT_LENGTHS(X) X(128) X(144) X(216) X(256) X(288) X(384) X(512)
 
 // ------------------------------------------------------------------ (e) S5 overlap-add
+// One thread per 4 ticks of a tile (float4), Bt / 4 threads per tile, 256 / (Bt / 4) tiles per CTA.
+// VEC = false: one thread per tick (Bt not a multiple of 4, or more than 1024 ticks per tile).
+template <bool VEC>
 __global__ void __launch_bounds__(256)
-k_gather_tiles(int64_t tile_begin, const int64_t* __restrict__ tile_keys, const int32_t* __restrict__ sp_idx,
-               const float* __restrict__ sp_data, float* __restrict__ tile_data, int accumulate, TredGrid g) {
-  const int64_t tile = tile_begin + blockIdx.x;
-  const int64_t key = tile_keys[tile];
+k_gather_tiles(int64_t tile_begin, int64_t ntiles, const int64_t* __restrict__ tile_keys,
+               const int32_t* __restrict__ sp_idx, const float* __restrict__ sp_data, float* __restrict__ tile_data,
+               int accumulate, TredGrid g) {
   const int64_t npix = (int64_t)g.npx * g.npy;
-  const int tb = (int)(key / npix);
-  const int64_t p = key - tb * npix;
   const int row = g.nover * g.Bt;
-  for (int t = threadIdx.x; t < g.Bt; t += blockDim.x) {
+  if (VEC) {
+    const int q = g.Bt >> 2;                                       // float4 per tile
+    const int per = 256 / q;                                       // tiles per CTA
+    const int tl = threadIdx.x / q, k4 = threadIdx.x - tl * q;
+    const int64_t tile = tile_begin + (int64_t)blockIdx.x * per + tl;
+    if (tl >= per || tile >= tile_begin + ntiles) return;
+    const int64_t key = tile_keys[tile];
+    const int tb = (int)(key / npix);
+    const int64_t p = key - tb * npix;
+    float4* out = reinterpret_cast<float4*>(tile_data + tile * g.Bt) + k4;
     // accumulate: continue the running sum left by the earlier chunks (slab ranges in
     // ascending order), so the additions are the same sequence as in one pass
-    float acc = accumulate ? tile_data[tile * g.Bt + t] : 0.0f;
+    float4 acc = accumulate ? *out : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     for (int bt = max(tb - g.nover + 1, 0); bt <= tb; ++bt) {        // ascending slab order
       const int64_t m = bt * npix + p;
       const int i0 = sp_idx[m];
-      if (sp_idx[m + 1] != i0) acc += sp_data[(int64_t)i0 * row + (tb - bt) * g.Bt + t];
+      if (sp_idx[m + 1] != i0) {
+        const float4 v = *(reinterpret_cast<const float4*>(sp_data + (int64_t)i0 * row + (tb - bt) * g.Bt) + k4);
+        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+      }
     }
-    if (tb * g.Bt + t >= g.nticks) acc = 0.0f;
-    tile_data[tile * g.Bt + t] = acc;
+    const int t = tb * g.Bt + 4 * k4;
+    if (t >= g.nticks) acc.x = 0.0f;
+    if (t + 1 >= g.nticks) acc.y = 0.0f;
+    if (t + 2 >= g.nticks) acc.z = 0.0f;
+    if (t + 3 >= g.nticks) acc.w = 0.0f;
+    *out = acc;
+  } else {
+    const int64_t tile = tile_begin + blockIdx.x;
+    const int64_t key = tile_keys[tile];
+    const int tb = (int)(key / npix);
+    const int64_t p = key - tb * npix;
+    for (int t = threadIdx.x; t < g.Bt; t += blockDim.x) {
+      float acc = accumulate ? tile_data[tile * g.Bt + t] : 0.0f;
+      for (int bt = max(tb - g.nover + 1, 0); bt <= tb; ++bt) {
+        const int64_t m = bt * npix + p;
+        const int i0 = sp_idx[m];
+        if (sp_idx[m + 1] != i0) acc += sp_data[(int64_t)i0 * row + (tb - bt) * g.Bt + t];
+      }
+      if (tb * g.Bt + t >= g.nticks) acc = 0.0f;
+      tile_data[tile * g.Bt + t] = acc;
+    }
   }
 }
 
@@ -1750,8 +1781,16 @@ extern "C" int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_
   if (ntiles > 0) {
     if (!d_tile_keys || !d_tile_data || (nsp > 0 && !d_sp_data)) return TRED_EINVAL;
     if (ntiles >= (1ll << 31)) return TRED_EUNSUPPORTED;
-    k_gather_tiles<<<(unsigned)ntiles, g.Bt < 256 ? (g.Bt < 32 ? 32 : g.Bt) : 256, 0, st>>>(
-        tile_begin, d_tile_keys, w.sp_idx, d_sp_data, d_tile_data, accumulate, g);
+    const bool vec = (g.Bt & 3) == 0 && g.Bt <= 1024 && ((uintptr_t)d_sp_data & 15) == 0 &&
+                     ((uintptr_t)d_tile_data & 15) == 0;
+    if (vec) {
+      const int per = 256 / (g.Bt >> 2);
+      k_gather_tiles<true><<<(unsigned)((ntiles + per - 1) / per), 256, 0, st>>>(
+          tile_begin, ntiles, d_tile_keys, w.sp_idx, d_sp_data, d_tile_data, accumulate, g);
+    } else {
+      k_gather_tiles<false><<<(unsigned)ntiles, g.Bt < 256 ? (g.Bt < 32 ? 32 : g.Bt) : 256, 0, st>>>(
+          tile_begin, ntiles, d_tile_keys, w.sp_idx, d_sp_data, d_tile_data, accumulate, g);
+    }
   }
   if (npix_req > 0) {
     if (!d_pix_ids || !d_dense) return TRED_EINVAL;
