@@ -91,10 +91,10 @@ __device__ __forceinline__ void group_wait(uint32_t mbar, uint32_t parity, bool 
     for (int it = 0; !ok; ++it) {
       asm volatile(
           "{\n\t.reg .pred p;\n\t"
-          "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+          "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
           "selp.u32 %0, 1, 0, p;\n\t}"
           : "=r"(ok)
-          : "r"(mbar), "r"(parity), "r"(20000u)
+          : "r"(mbar), "r"(parity)
           : "memory");
       if (it == 64) t0 = clock64();
       if (it > 64 && (it & 255) == 0 && clock64() - t0 > 4000000000ll) {

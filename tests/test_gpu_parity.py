@@ -513,10 +513,10 @@ def test_readout_parity(with_noise):
 
 
 # ------------------------------------------------------------------ full size (configs 3 and 4)
-# Neighbourhoods checked against the oracle at full size.  The oracle needs about a minute per
-# neighbourhood (every segment within the response's reach, all time slabs), so the default keeps the
-# suite short; TRED_FULL_NEIGHBOURHOODS=16 runs the wide sample (its log is kept under profiles/).
-NFULL = int(os.environ.get("TRED_FULL_NEIGHBOURHOODS", "4"))
+# Neighbourhoods checked against the oracle at full size (config 3; a quarter as many at config 4).
+# The oracle needs about 10 s per neighbourhood on the 16+ host cores of a GPU box (every segment
+# within the response's reach, all time slabs); TRED_FULL_NEIGHBOURHOODS changes the sample size.
+NFULL = int(os.environ.get("TRED_FULL_NEIGHBOURHOODS", "16"))
 
 
 def _check_neighbourhoods(cfg, aug, keys, R, groups, dense, mode, payload_rows=None):
