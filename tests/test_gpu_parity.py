@@ -512,6 +512,37 @@ def test_readout_parity(with_noise):
     assert int(readout(z, par)[0].sum()) == 0
 
 
+def test_readout_full_plane():
+    """All 230 x 230 channels x 5000 ticks of a config-3 plane (one vertex) in one call: channels the
+    event never reaches record nothing; 150 of the busiest channels and 150 random active ones are
+    bit-exact against the oracle (which walks a channel tick by tick in Python)."""
+    torch = _torch()
+    from paper_2602_12052_b200 import readout
+    cfg, segs = gen.make_segments(3, n_vertices=1)
+    R = gen.make_response(cfg, 2003)
+    sim = _sim(cfg)
+    rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+    npix = cfg.npix_x * cfg.npix_y
+    pix = torch.arange(npix, dtype=torch.int32, device="cuda")
+    wave = sim.simulate(_seg_tensor(segs), rhat, pix_ids=pix)["dense"]
+    assert tuple(wave.shape) == (npix, cfg.nticks)
+    par = dict(threshold_e=4000.0, n_integ=16, n_reset=8, max_hits=24, adc_lsb_e=100.0)
+    rng = np.random.default_rng(7)
+    noise = (rng.standard_normal((npix, par["max_hits"], 3)) * [650.0, 500.0, 900.0]).astype(np.float32)
+    nh, tk, adc = readout(wave, par, torch.from_numpy(noise).cuda())
+    nh, tk, adc = nh.cpu().numpy(), tk.cpu().numpy(), adc.cpu().numpy()
+    l1 = wave.abs().sum(1).cpu().numpy()
+    silent = l1 == 0
+    assert silent.sum() > 1000 and (nh[silent] == 0).all() and (tk[silent] == -1).all()
+    assert nh.sum() > 5000 and nh.max() >= 4
+    active = np.flatnonzero(~silent)
+    sel = np.unique(np.concatenate([active[np.argsort(l1[active])[-150:]], rng.choice(active, 150, replace=False)]))
+    rn, rt, ra = o.readout(par, wave[torch.from_numpy(sel).cuda()].cpu().numpy(), noise[sel])
+    np.testing.assert_array_equal(nh[sel], rn)
+    np.testing.assert_array_equal(tk[sel], rt)
+    np.testing.assert_array_equal(adc[sel], ra)
+
+
 # ------------------------------------------------------------------ full size (configs 3 and 4)
 # Neighbourhoods checked against the oracle at full size (config 3; a quarter as many at config 4).
 # The oracle needs about 10 s per neighbourhood on the 16+ host cores of a GPU box (every segment
