@@ -28,6 +28,9 @@
  *     ascending.  Tile / slab-pixel key: (tb*npix_x + px)*npix_y + py.
  *   - Charge outside the grid and current outside the pixel plane / readout window are
  *     dropped (reading G13).
+ *   - A context belongs to the CUDA device that was current in tred_create; a call made while
+ *     another device is current returns TRED_EINVAL (several contexts, one per device, may live
+ *     in one process).
  *   - There is no CPU fallback: without a CUDA device every compute call fails.
  */
 #ifndef TRED_H

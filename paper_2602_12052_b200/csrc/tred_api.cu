@@ -297,6 +297,7 @@ static DriftParams make_drift_params(const tred_ctx* c) {
 extern "C" int tred_drift(tred_ctx* ctx, int64_t nseg, const float* d_seg, float* d_augf,
                           int32_t* d_augi, int64_t* d_npairs, void* stream) {
   if (!ctx || nseg < 0 || !d_npairs) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   cudaStream_t st = (cudaStream_t)stream;
   TRED_CUDA(cudaMemsetAsync(d_npairs, 0, sizeof(int64_t), st));
   if (nseg == 0) return TRED_OK;
@@ -406,6 +407,7 @@ extern "C" int tred_blockbin(tred_ctx* ctx, int64_t nseg, const int32_t* d_augi,
                              int32_t* d_slab_off, int64_t* d_nblocks,
                              void* d_work, size_t work_bytes, void* stream) {
   if (!ctx || nseg < 0 || cap_pairs < 0 || cap_blocks < 0 || !d_nblocks || !d_slab_off) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   if (cap_pairs >= (1ll << 31) || nseg >= (1ll << 31)) return TRED_EUNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);

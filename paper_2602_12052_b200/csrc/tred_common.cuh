@@ -78,6 +78,14 @@ void tred_set_cuda_error(cudaError_t e, const char* where);
     if (_e != cudaSuccess) { tred_set_cuda_error(_e, #call); return TRED_ECUDA; } \
   } while (0)
 
+// A context belongs to the device it was created on (its kernel attributes, SM count and
+// shared-memory limits are that device's): calls made with another device current are refused.
+#define TRED_CHECK_DEVICE(ctx)                                             \
+  do {                                                                     \
+    int _dev = -1;                                                         \
+    if (cudaGetDevice(&_dev) != cudaSuccess || _dev != (ctx)->device) return TRED_EINVAL; \
+  } while (0)
+
 #define TRED_LAUNCH_CHECK(name)                                            \
   do {                                                                     \
     cudaError_t _e = cudaGetLastError();                                   \

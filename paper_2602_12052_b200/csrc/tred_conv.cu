@@ -1475,6 +1475,7 @@ static int convolve_tiled(tred_ctx* ctx, int64_t nblocks, const int64_t* d_keys,
 // ==================================================================== exported calls
 extern "C" int tred_prepare_response(tred_ctx* ctx, const float* d_resp, float* d_rhat, void* stream) {
   if (!ctx || !d_resp || !d_rhat) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);
   const int nrows = g.nph * g.noff;
@@ -1567,6 +1568,7 @@ int tred_convolve_plan_dev(tred_ctx* ctx, int64_t nblocks, const int64_t* d_nblo
                            void* d_plan_work, size_t plan_work_bytes, void* stream) {
   if (!ctx || nblocks < 0 || !d_ncp || !d_cp_off || !d_nsp || !d_ntiles || !d_sp_off || !d_rt_off)
     return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   PlanWork w = carve_plan(ctx, d_plan_work);
   if (!d_plan_work || plan_work_bytes < w.total) return TRED_ECAP;
   if (nblocks > 0 && !d_keys) return TRED_EINVAL;
@@ -1629,6 +1631,7 @@ extern "C" int tred_convolve(tred_ctx* ctx, int64_t nblocks, const int64_t* d_ke
                              const void* d_plan_work, float* d_sp_data,
                              void* d_work, size_t work_bytes, void* stream) {
   if (!ctx || nblocks < 0 || nsp < 0 || ncp < 0) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   if (nblocks == 0 || nsp == 0 || ncp == 0) return TRED_OK;
   if (!d_keys || !d_payload || !d_rhat || !d_cp_keys || !h_cp_off || !d_sp_keys || !h_sp_off ||
       !d_plan_work || !d_sp_data || !d_work)
@@ -1772,6 +1775,7 @@ extern "C" int tred_gather_waveforms(tred_ctx* ctx, int64_t nsp, const float* d_
                                      int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
                                      void* stream) {
   if (!ctx || nsp < 0 || ntiles < 0 || tile_begin < 0 || npix_req < 0 || !d_plan_work) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   cudaStream_t st = (cudaStream_t)stream;
   const TredGrid g = make_grid(ctx);
   PlanWork w = carve_plan(ctx, (void*)d_plan_work);

@@ -1004,6 +1004,7 @@ extern "C" int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
                          const float* d_augf, const int32_t* d_augi,
                          float* d_payload, void* d_work, size_t work_bytes, void* stream) {
   if (!ctx || nseg < 0 || nblocks < 0) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   if (nblocks == 0) return TRED_OK;
   if (!d_keys || !d_blk_off || !d_pair_seg || !d_augf || !d_augi || !d_payload) return TRED_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;

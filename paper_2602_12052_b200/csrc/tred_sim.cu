@@ -68,6 +68,7 @@ extern "C" int tred_simulate(tred_ctx* ctx, int64_t nseg, const float* seg, int 
                              int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
                              tred_sim_result* res, void* stream) {
   if (!ctx || nseg < 0 || !res || cap_tiles < 0 || npix_req < 0) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   if (nseg > 0 && !seg) return TRED_EINVAL;
   if (nseg >= (1ll << 31)) return TRED_EUNSUPPORTED;
   memset(res, 0, sizeof(*res));
