@@ -328,6 +328,18 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
       for (int w = 1; w < 8; ++w) tot += red[w];
       const float sc = dft_h16_scale(tot);
       const float sdown = __uint_as_float((254u - (__float_as_uint(sc) >> 23)) << 23);
+      // split into fp16 hi / lo in registers NOW (the packed parts take the place of the fp32 values):
+      // only the shared-memory stores are left for after the wait, which is on the row's critical path
+      uint4 hl[DF_MAXF4];                                     // (hi01, hi23, lo01, lo23)
+#pragma unroll
+      for (int i = 0; i < DF_MAXF4; ++i) {
+        const float x0 = v[i].x * sdown, x1 = v[i].y * sdown, x2 = v[i].z * sdown, x3 = v[i].w * sdown;
+        const __half2 h01 = __floats2half2_rn(x0, x1), h23 = __floats2half2_rn(x2, x3);
+        const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
+        const __half2 l01 = __floats2half2_rn(x0 - f01.x, x1 - f01.y), l23 = __floats2half2_rn(x2 - f23.x, x3 - f23.y);
+        hl[i] = make_uint4(*reinterpret_cast<const uint32_t*>(&h01), *reinterpret_cast<const uint32_t*>(&h23),
+                           *reinterpret_cast<const uint32_t*>(&l01), *reinterpret_cast<const uint32_t*>(&l23));
+      }
       // the tensor core must be done with this K chunk of the previous row before it is overwritten
       if (!first) { group_wait(aempty_bar(kc), ephase, poller, gbar, TG); ephase ^= 1; }
 #pragma unroll
@@ -336,19 +348,13 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
         if (idx < nf4) {
           const int cc = idx >> 3;
           const int t0 = 4 * (idx & 7);                          // tick within the K chunk
-          const float x0 = v[i].x * sdown, x1 = v[i].y * sdown, x2 = v[i].z * sdown, x3 = v[i].w * sdown;
-          const __half2 h01 = __floats2half2_rn(x0, x1), h23 = __floats2half2_rn(x2, x3);
-          const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
-          const __half2 l01 = __floats2half2_rn(x0 - f01.x, x1 - f01.y), l23 = __floats2half2_rn(x2 - f23.x, x3 - f23.y);
           // K chunk of 32 ticks = one 128-byte row: [hi 16 | lo 16 | hi 16 | lo 16]; 16-byte units swizzled by row
           const int off = (t0 >> 4) * 64 + (t0 & 15) * 2;
-          if (DFT_EXP == 2 && x0 != 12345.678f) continue;
+          if (DFT_EXP == 2 && hl[i].x != 0x12345678u) continue;
           uint8_t* rowp = a_ptr + kc * 16384 + cc * 128;
           const int u_hi = (off >> 4) ^ (cc & 7), u_lo = ((off + 32) >> 4) ^ (cc & 7);
-          *reinterpret_cast<uint2*>(rowp + u_hi * 16 + (off & 15)) =
-              make_uint2(*reinterpret_cast<const uint32_t*>(&h01), *reinterpret_cast<const uint32_t*>(&h23));
-          *reinterpret_cast<uint2*>(rowp + u_lo * 16 + (off & 15)) =
-              make_uint2(*reinterpret_cast<const uint32_t*>(&l01), *reinterpret_cast<const uint32_t*>(&l23));
+          *reinterpret_cast<uint2*>(rowp + u_hi * 16 + (off & 15)) = make_uint2(hl[i].x, hl[i].y);
+          *reinterpret_cast<uint2*>(rowp + u_lo * 16 + (off & 15)) = make_uint2(hl[i].z, hl[i].w);
         }
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic writes -> tensor core reads
