@@ -12,9 +12,11 @@
  * Conventions
  *   - Every pointer named d_* is DEVICE memory, h_* is HOST memory.  All device buffers,
  *     workspaces included, are allocated by the caller and only borrowed; the library
- *     never allocates device memory and never synchronises the host inside a call
- *     (two exceptions, both outside the hot path: tred_prepare_response, once per response,
- *     and tred_profile_end).  Calls are enqueued on `stream` (a cudaStream_t passed as void*).
+ *     never allocates device memory and the stepwise calls never synchronise the host
+ *     (exceptions: tred_prepare_response, once per response; tred_profile_end; and
+ *     tred_simulate, which reads the device-side counts once per event to size what follows --
+ *     it keeps 64 KB of pinned host memory per context for that).  Calls are enqueued on
+ *     `stream` (a cudaStream_t passed as void*).
  *   - Results of data-dependent size use "capacity + device-side count": the count is
  *     written to device memory; entries beyond the capacity are not written.  The caller
  *     reads the count (its own synchronisation), re-allocates and calls again if needed.
