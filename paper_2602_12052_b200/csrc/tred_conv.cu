@@ -919,18 +919,25 @@ k_accum_tiles(const float2* __restrict__ opart, const int64_t* __restrict__ sp_k
       tile[lane][sl] = v;
     }
     __syncthreads();
+    if (my_n > 0) {
+      // this warp's four frequencies of the block together: per covering tile the four patch
+      // values are loaded before any is added (four loads in flight instead of one); for every
+      // (slab pixel, frequency) the additions are still in ascending tile order
+      float2 a[4];
+      const int fb = f0 + w * 4;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int fl = w * 4 + i, f = f0 + fl;
-      if (f < g.nf && my_n > 0) {
-        float2 a = tile[fl][lane];
-        for (int e = 0; e < my_n; ++e) {
-          const int en = ent[lane][e];
-          const float2 v = opart[((int64_t)(en >> 11) * g.nf + f) * npos + (en & 2047)];
-          a.x += v.x; a.y += v.y;
-        }
-        tile[fl][lane] = a;
+      for (int i = 0; i < 4; ++i) a[i] = tile[w * 4 + i][lane];
+      for (int e = 0; e < my_n; ++e) {
+        const int en = ent[lane][e];
+        const float2* src = opart + ((int64_t)(en >> 11) * g.nf + fb) * npos + (en & 2047);
+        float2 v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] = fb + i < g.nf ? src[(int64_t)i * npos] : make_float2(0.0f, 0.0f);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { a[i].x += v[i].x; a[i].y += v[i].y; }
       }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) if (fb + i < g.nf) tile[w * 4 + i][lane] = a[i];
     }
     __syncthreads();
 #pragma unroll
