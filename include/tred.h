@@ -317,6 +317,43 @@ int tred_steps(const tred_steps_config* cfg, int64_t nstep, const float* d_step,
                void* stream);
 
 /*
+ * tred_steps_static -- tred_steps without a workspace argument and without any allocation: the
+ * same operation (readings G21, G22), the same arithmetic in the same order,
+ * the same bits in d_seg / d_parent / d_nseg, for callers that cannot provide d_work.
+ *
+ * Who needs it.  The step splitter sits in front of the simulation, typically in an input stage
+ * that owns no device workspace and cannot get one from the CUDA runtime: all device memory of
+ * the job was given to a pool at start-up; or another thread of the process is recording a CUDA
+ * graph in the default capture mode, during which cudaMalloc / cudaFree from ANY thread are
+ * errors that also ruin that recording; or the caller is a per-event loop that cannot take the
+ * device-wide synchronisation cudaMalloc / cudaFree imply.  The call and everything under it
+ * make no cudaMalloc, cudaFree or other allocating call, on the first call or later.
+ *
+ * How.  Its scratch (first segment of every step + the block sums of the scan) is a fixed
+ * __device__ array inside libtred.so, TRED_STEPS_STATIC_BYTES long.  Consequences to know:
+ *   - limit: nstep <= TRED_STEPS_STATIC_MAX (= tred_steps_static_max()).  More returns TRED_ECAP
+ *     before anything is enqueued and leaves the outputs untouched: split the batch (segments of
+ *     different steps are independent; add the batch's first step index to d_parent), or use
+ *     tred_steps with a workspace;
+ *   - cost: every GPU on which the process has loaded libtred.so holds those ~4 MiB until the
+ *     process ends, whether or not this call is ever made;
+ *   - sharing: all calls on one device use the one array.  Calls on the same stream follow each
+ *     other and are fine (nothing needs clearing between them: a call writes every scratch entry
+ *     it later reads).  Calls that may run on the GPU at the same time -- different streams, or
+ *     several host threads with their own streams -- overwrite each other's scratch and give
+ *     wrong results: order them with events or keep one stream for this call per device;
+ *   - first call on a device: looks up the array's address on that device (cudaGetSymbolAddress,
+ *     with the device current; kept per device afterwards, under a mutex).  Make that first call
+ *     during set-up, before any stream capture is begun anywhere in the process.
+ * Arguments as for tred_steps, minus d_work / work_bytes; cap_seg = 0 is the counting pass.
+ */
+#define TRED_STEPS_STATIC_MAX   1048576      /* steps per call                                  */
+#define TRED_STEPS_STATIC_BYTES 4196608      /* (MAX + 1) int32 rounded to 256, + 2048 for the scan */
+int64_t tred_steps_static_max(void);
+int tred_steps_static(const tred_steps_config* cfg, int64_t nstep, const float* d_step, int64_t cap_seg,
+                      float* d_seg, int32_t* d_parent, int64_t* d_nseg, void* stream);
+
+/*
  * tred_readout -- trigger-reset pixel readout (Fig. 4; noise terms
  * PAPER.md:L262; reading G23).  Per channel, tick by tick: the charge on the
  * preamplifier is the running fp32 sum of the current; when it reaches threshold_e (+ the

@@ -16,7 +16,7 @@ import os
 
 from . import build as _build
 
-__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS", "split_steps", "TredStepsConfig", "readout", "TredReadoutConfig"]
+__all__ = ["Tred", "TredError", "lib", "TredConfig", "TredDims", "EXPORTS", "split_steps", "split_steps_static", "TredStepsConfig", "readout", "TredReadoutConfig"]
 
 _c_i64 = C.c_int64
 _c_p = C.c_void_p
@@ -104,6 +104,8 @@ EXPORTS = {
     "tred_steps_work_bytes": (C.c_size_t, [_c_i64]),
     "tred_steps": (C.c_int, [C.POINTER(TredStepsConfig), _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p,
                              C.c_size_t, _c_p]),
+    "tred_steps_static_max": (_c_i64, []),
+    "tred_steps_static": (C.c_int, [C.POINTER(TredStepsConfig), _c_i64, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p]),
     "tred_readout": (C.c_int, [C.POINTER(TredReadoutConfig), _c_i64, C.c_int32, _c_p, _c_p, _c_p, _c_p, _c_p, _c_p]),
     "tred_truth_work_bytes": (C.c_size_t, [_c_p, _c_i64]),
     "tred_truth": (C.c_int, [_c_p, _c_i64, _c_p, _c_p, _c_i64, _c_p, _c_p, _c_p, _c_p, _c_p, C.c_size_t, _c_p]),
@@ -227,6 +229,38 @@ def split_steps(steps, params: dict, cap_seg: int | None = None):
     _check(L.tred_steps(C.byref(c), nstep, _ptr(steps), cap_seg, _ptr(seg), _ptr(parent), _ptr(nseg), _ptr(work),
                         work.numel(), stream), "tred_steps")
     return seg[:, :cap_seg], parent[:cap_seg], nseg
+
+
+def split_steps_static(steps, params: dict, seg, parent, nseg):
+    """tred_steps_static: `split_steps` for callers that must not allocate device memory (an input
+    stage whose memory all belongs to a pool, a thread beside another thread's graph recording, a
+    per-event loop that cannot take cudaMalloc's synchronisation).  Nothing is allocated here or in
+    the library: the caller passes the outputs -- seg [8][cap_seg] float32, parent [cap_seg] int32,
+    nseg [1] int64, CUDA tensors (cap_seg = seg.shape[1]; seg and parent may be None for the
+    counting pass) -- and the scratch is a fixed array inside libtred.so.  At most
+    tred_steps_static_max() steps per call; calls that can overlap on the GPU (other streams) share
+    that array and must be ordered by the caller.  Make the first call on a device at set-up."""
+    import torch
+    if not steps.is_cuda:
+        raise TredError("tred_steps_static needs CUDA tensors: the TRED path has no CPU fallback")
+    assert steps.dtype == torch.float32 and steps.is_contiguous() and steps.shape[0] == 8
+    L = lib()
+    nstep = steps.shape[1]
+    if nstep > L.tred_steps_static_max():
+        raise TredError(f"tred_steps_static: {nstep} steps exceed the fixed scratch of "
+                        f"{L.tred_steps_static_max()} steps per call; split the batch or use split_steps")
+    c = TredStepsConfig()
+    for k, _ in TredStepsConfig._fields_:
+        setattr(c, k, params[k])
+    cap_seg = 0
+    if seg is not None:
+        assert seg.is_cuda and seg.dtype == torch.float32 and seg.is_contiguous() and seg.shape[0] == 8
+        cap_seg = seg.shape[1]
+        assert parent.is_cuda and parent.dtype == torch.int32 and parent.numel() >= cap_seg
+    assert nseg.is_cuda and nseg.dtype == torch.int64 and nseg.numel() >= 1
+    stream = C.c_void_p(torch.cuda.current_stream(steps.device).cuda_stream)
+    _check(L.tred_steps_static(C.byref(c), nstep, _ptr(steps), cap_seg, _ptr(seg) if cap_seg else None,
+                               _ptr(parent) if cap_seg else None, _ptr(nseg), stream), "tred_steps_static")
 
 
 class Tred:

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtred.so")
-SOURCES = ["tred_api.cu", "tred_scan_sort.cu", "tred_effq.cu", "tred_effq_fact.cu", "tred_conv.cu", "tred_mac_tc.cu", "tred_mac_tc2.cu", "tred_mac_tc2s.cu", "tred_mac_h3.cu", "tred_dft_h16.cu", "tred_sim.cu", "tred_steps.cu", "tred_readout.cu"]
+SOURCES = ["tred_api.cu", "tred_scan_sort.cu", "tred_effq.cu", "tred_effq_fact.cu", "tred_conv.cu", "tred_mac_tc.cu", "tred_mac_tc2.cu", "tred_mac_tc2s.cu", "tred_mac_h3.cu", "tred_dft_h16.cu", "tred_sim.cu", "tred_steps.cu", "tred_steps_static.cu", "tred_readout.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
