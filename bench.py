@@ -520,6 +520,11 @@ def run_cuda(args):
                                         "peak_mem_gb": x["peak_mem"] / 1e9, "mac_mode_ran": x["mac_mode"]}
                 x.clear()
                 torch.cuda.empty_cache()
+            # BASELINE config 5 (Fig. 11): the representation sweep, one timed
+            # spill per cell, and the dense-grid comparison
+            t_sw = time.perf_counter()
+            extra["cfg5_sweep"] = list(sweep_cells(dev, 1))
+            extra["cfg5_sweep_wall_s"] = time.perf_counter() - t_sw
             line["extra"] = extra
         if not args.no_cpu_baseline and world == 1:
             n, dt, cores = oracle_sample(cfg, segs, R, _ref_segments(args))
@@ -576,17 +581,16 @@ def dense_grid_convolution(torch, cfg, keys, payload, R_d, pix_ids):
     return rows, e0.elapsed_time(e1), torch.cuda.max_memory_allocated(dev) - base
 
 
-def run_sweep(args):
-    """BASELINE config 5: block shapes x Gauss-Legendre orders on config-3 inputs, one JSON
-    line each (ms per spill, peak GB, occupied-block fraction), then the dense-grid line."""
+def sweep_cells(dev, steps: int, with_dense: bool = True):
+    """BASELINE config 5: block shapes x Gauss-Legendre orders on config-3 inputs -- one record per
+    cell (ms per spill, peak GB, occupied-block fraction, the kernels that ran), then the
+    dense-grid comparison.  A generator: `--config 5` prints the records one per line, the
+    default run stores them under "extra"."""
     import torch
     from paper_2602_12052_b200 import Tred
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(dev)
     cfg0, segs, seg_h, R = workload(3, 0)
     seg_d = torch.from_numpy(seg_h).to(dev)
     R_d = torch.from_numpy(R).to(dev)
-    steps = max(1, min(args.steps, 3))
     for block in ((4, 4, 32), (8, 8, 64), (16, 16, 128), (32, 32, 256)):
         for n in (1, 2, 3, 4):
             cfg = cfg0.with_(block=block, gl_n=n)
@@ -605,13 +609,16 @@ def run_sweep(args):
                 ms.append(a.elapsed_time(b))
             d = sim.dims
             nb_all = int(d.NB[0] * d.NB[1] * d.NB[2])
-            print(json.dumps({"sweep": "block x gl_n", "workload": cfg0.name, "block": list(block), "gl_n": n,
-                              "fft_len": d.fft_len, "ms_per_spill": float(np.mean(ms)),
-                              "segments_per_s": seg_h.shape[1] / (float(np.mean(ms)) * 1e-3),
-                              "nblocks": out["nblocks"], "occupied_block_fraction": out["nblocks"] / nb_all,
-                              "payload_gb": out["nblocks"] * d.block_floats * 4 / 1e9,
-                              "peak_gb": torch.cuda.max_memory_allocated(dev) / 1e9}), flush=True)
+            yield {"sweep": "block x gl_n", "workload": cfg0.name, "block": list(block), "gl_n": n,
+                   "fft_len": d.fft_len, "ms_per_spill": float(np.mean(ms)), "steps": steps,
+                   "segments_per_s": seg_h.shape[1] / (float(np.mean(ms)) * 1e-3),
+                   "nblocks": out["nblocks"], "occupied_block_fraction": out["nblocks"] / nb_all,
+                   "payload_gb": out["nblocks"] * d.block_floats * 4 / 1e9,
+                   "peak_gb": torch.cuda.max_memory_allocated(dev) / 1e9,
+                   "mac_mode_ran": sim.last_mac_mode()}
             del sim, rhat, out
+    if not with_dense:
+        return
     # dense-grid comparison on the config-3 representation
     cfg = cfg0
     torch.cuda.empty_cache()
@@ -628,11 +635,33 @@ def run_sweep(args):
     rows, ms, peak = dense_grid_convolution(torch, cfg, keys, payload, R_d, pix)      # warm-up (cuFFT plans)
     rows, ms, peak = dense_grid_convolution(torch, cfg, keys, payload, R_d, pix)
     err = float((rows - sparse_rows).abs().max() / sparse_rows.abs().max())
-    print(json.dumps({"sweep": "dense grid", "workload": cfg.name, "impl": "torch.fft (cuFFT), comparison only",
-                      "ms_per_spill_convolution_only": ms, "peak_gb_convolution_only": peak / 1e9,
-                      "dense_fine_grid_gb_if_materialised": cfg.npix_x * cfg.npix_y * cfg.sub ** 2 * cfg.nticks * 4 / 1e9,
-                      "max_abs_diff_vs_block_sparse_over_max": err, "pixels_compared": int(pix.numel())}))
+    yield {"sweep": "dense grid", "workload": cfg.name, "impl": "torch.fft (cuFFT), comparison only",
+           "ms_per_spill_convolution_only": ms, "peak_gb_convolution_only": peak / 1e9,
+           "dense_fine_grid_gb_if_materialised": cfg.npix_x * cfg.npix_y * cfg.sub ** 2 * cfg.nticks * 4 / 1e9,
+           "max_abs_diff_vs_block_sparse_over_max": err, "pixels_compared": int(pix.numel())}
+
+
+def run_sweep(args):
+    import torch
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    for rec in sweep_cells(dev, max(1, min(args.steps, 3))):
+        print(json.dumps(rec), flush=True)
     return 0
+
+
+def _spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks here (one process per GPU,
+    replicas of the spill: PAPER.md:L256-260, drift volumes are independent), exactly as the
+    driver would: torch.distributed.run on this node, rendezvous on 127.0.0.1."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -649,6 +678,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip configs 1, 2, 4 and the cuFFT comparison")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return _spawn_ranks(args.gpus)
+    if args.gpus != _env_int("WORLD_SIZE", 1):
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={_env_int('WORLD_SIZE', 1)}", file=sys.stderr)
+        return 2
     if args.impl == "reference":
         return run_reference(args)
     if args.config == 5:

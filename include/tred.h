@@ -90,15 +90,20 @@ typedef struct tred_config {
                                     4 = as 5 with the mirror symmetry of the response
                                         (MPCP) spent on the product: sums and
                                         differences of mirror phase pairs, two products of half
-                                        the size; falls back to 0 if the response prepared last
-                                        is not exactly mirror-symmetric,
+                                        the size; if the response prepared last is not exactly
+                                        mirror-symmetric the general product of mode 6 runs
+                                        instead (never the fp16 path of mode 7) and
+                                        tred_last_mac_mode reports 6,
                                     1 = fp32 FMA pipe, products written to memory,
                                     2 = tensor cores 3xTF32, products written to memory       */
   int32_t fft_mode;              /* forward transform of tred_convolve in mac_mode 7:
                                     0 = default: pruned DFT as a dense contraction on the tensor
-                                        cores (tred_dft_h16.cu) where the shape allows it (Bt a
-                                        multiple of 32, <= 128; L with a divisor NC <= 256, NC a
-                                        multiple of 32, L / NC >= 2), else as 1,
+                                        cores (tred_dft_h16.cu) where the shape allows it (S = 10;
+                                        Bt a multiple of 32, <= 128; L with a divisor NC <= 256,
+                                        NC a multiple of 32, L / NC >= 2; and half of the DFT
+                                        matrix, L * Bt * 2 bytes, plus Bt * 512 bytes of operand
+                                        tile and ~2 KB fit the opt-in shared memory of one CTA:
+                                        L * Bt <= ~80 000 on B200), else as 1,
                                     1 = shared-memory / register FFT kernels                     */
 } tred_config;
 
@@ -209,6 +214,12 @@ int tred_effq(tred_ctx* ctx, int64_t nseg, int64_t nblocks,
  *          (fp32 [f][phase][offset] complex, and the real-ified matrices
  *          [f][2*offset+c][2*phase+c'] split into tf32 hi / lo parts for the tensor cores,
  *          and the half-size matrices of a mirror-symmetric response).
+ *   Dynamic range in mac_mode 7 (the default): the fp16 hi / lo parts of the spectrum share one
+ *   power-of-two scale per frequency across all phases and offsets.  An offset whose spectrum is
+ *   rho times the largest entry of that frequency keeps 22 bits while rho >= 2^-18; below that
+ *   its own contribution carries a relative error of about 2^-40 / rho (1e-6 at rho = 1e-6,
+ *   1e-5 at 1e-7; tests/test_gpu_parity.py::test_convolve_response_dynamic_range).  A response
+ *   with a wider range between its offsets than that should use mac_mode 1 (fp32).
  *   Runs once per response and, unlike every other call, waits for the stream: the context
  *   has to know whether the response has the mirror symmetry R_{-i}^{-j} = R_i^j
  *   (exact equality is tested on the device).
@@ -393,7 +404,13 @@ int tred_readout(const tred_readout_config* cfg, int64_t npix, int32_t nticks, c
  *                result is bit-identical to one pass (a slab's output depends on that slab's
  *                blocks only, and the overlap-add continues the running sum in slab order)
  *   d_work       device workspace, work_bytes long.  Too small: TRED_ECAP with
- *                h_result->work_bytes_needed set (a size that is enough for this event)
+ *                h_result->work_bytes_needed set.  Once the counts of the event have been read
+ *                (h_result->nblocks > 0) that number is enough for this event in the unchunked
+ *                form; a workspace too small even for the lists that precede the read (drift
+ *                records, pair lists, plan: h_result->nblocks == 0), and every TRED_ECAP of the
+ *                chunked form, report what is known at that point plus a margin (64 MiB / 6 GiB),
+ *                so a caller that grows the workspace by the reported size may see TRED_ECAP up
+ *                to three times for one event.  h_result is zeroed first on every return
  *   tile_keys    [cap_tiles] int64 out, tile_data [cap_tiles][Bt] float32 out: the waveform tiles,
  *                keys ascending, in HOST memory if out_on_host != 0, else device memory.
  *                h_result->ntiles > cap_tiles: TRED_ECAP, nothing written

@@ -48,6 +48,7 @@ static void prof_clear(tred_ctx* c) {
 
 extern "C" int tred_profile_begin(tred_ctx* c, int record_events) {
   if (!c) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(c);
   prof_clear(c);
   c->prof_on = record_events ? 1 : 0;
   return TRED_OK;
@@ -55,6 +56,7 @@ extern "C" int tred_profile_begin(tred_ctx* c, int record_events) {
 
 extern "C" int tred_profile_end(tred_ctx* c, int nstage, float* h_ms, int64_t* h_launches) {
   if (!c || nstage < 0) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(c);
   for (int s = 0; s < nstage; ++s) { if (h_ms) h_ms[s] = 0.0f; if (h_launches) h_launches[s] = 0; }
   for (int i = 0; i < c->nrecs; ++i) {
     TredProfRec& r = c->recs[i];
@@ -91,6 +93,7 @@ __global__ void __launch_bounds__(256) k_bench_fma(int iters, float seed, float*
 
 extern "C" int tred_bench_fma(tred_ctx* ctx, int32_t iters, float* d_out, double* h_flops, void* stream) {
   if (!ctx || iters < 1 || !d_out) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   const int blocks = ctx->num_sms * 8;
   k_bench_fma<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, 1.0f, d_out);
   TRED_COUNT_LAUNCH(1);

@@ -27,10 +27,6 @@
 #include <cuda_fp16.h>
 #include "tred_tc2_common.cuh"
 
-#ifndef DFT_EXP
-#define DFT_EXP 0          // perf-only experiments (wrong results): 1 no stores, 2 no A tile stores, 3 no epilogue work
-#endif
-
 namespace {
 
 constexpr int DF_THREADS = 576;          // 18 warps: W loader, MMA issuer, 8 epilogue, 8 converters
@@ -239,7 +235,7 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
           uint32_t v[32];
           tmem_ld32(v, taddr + (uint32_t)(g * 32));
           asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          if (DFT_EXP != 3 && prow >= 0 && (live || padlane)) {
+          if (prow >= 0 && (live || padlane)) {
             __half* o = orow + (int64_t)(nc * (p.NC >> 1) + g * 16) * fstride;
             if (live) {
 #pragma unroll
@@ -248,10 +244,8 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
                 const __half2 h = __floats2half2_rn(re, im);
                 const float2 hf = __half22float2(h);
                 const __half2 l = __floats2half2_rn(re - hf.x, im - hf.y);
-                if (DFT_EXP != 1 || re == 12345.678f) {
-                  *reinterpret_cast<__half2*>(o + i * fstride) = h;
-                  *reinterpret_cast<__half2*>(o + i * fstride + 16) = l;
-                }
+                *reinterpret_cast<__half2*>(o + i * fstride) = h;
+                *reinterpret_cast<__half2*>(o + i * fstride + 16) = l;
               }
             } else {
 #pragma unroll
@@ -350,7 +344,6 @@ k_dft_h16(const __grid_constant__ CUtensorMap tmW, DftParams p) {
           const int t0 = 4 * (idx & 7);                          // tick within the K chunk
           // K chunk of 32 ticks = one 128-byte row: [hi 16 | lo 16 | hi 16 | lo 16]; 16-byte units swizzled by row
           const int off = (t0 >> 4) * 64 + (t0 & 15) * 2;
-          if (DFT_EXP == 2 && hl[i].x != 0x12345678u) continue;
           uint8_t* rowp = a_ptr + kc * 16384 + cc * 128;
           const int u_hi = (off >> 4) ^ (cc & 7), u_lo = ((off + 32) >> 4) ^ (cc & 7);
           *reinterpret_cast<uint2*>(rowp + u_hi * 16 + (off & 15)) = make_uint2(hl[i].x, hl[i].y);

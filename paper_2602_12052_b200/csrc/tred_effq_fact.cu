@@ -170,6 +170,14 @@ __device__ __forceinline__ void effq_cells(int gi, int lo_a, int hi_a, float p0a
 // from the 4-aligned tick tb = align_down(lot - E, 4), ntfp = align_up(hit + E + 1 - tb, 4) of
 // them.  Entries of grid points outside the grid are zero (clip and drop, reading G13).
 constexpr int EB_MQ = 12;           // quadrature points per pass / table chunk
+// Table offsets are int32 prefix sums of table sizes in 16-byte units.  k_effq_sizes also adds
+// the sizes up in 64 bits, and the offsets are used only if that total is at most TAB_TOTAL_MAX,
+// i.e. if no prefix sum can have wrapped (a wrapped offset could pass every range check and put
+// a table in front of the workspace).  Beyond it (tens of millions of marked segments in one
+// call, or tens of thousands of long unsplit ones) no segment gets a table: same values,
+// computed by the tile CTAs.  One table is at most TAB_SIZE_MAX units (4 MiB).
+constexpr int64_t TAB_SIZE_MAX = 1 << 18;
+constexpr int64_t TAB_TOTAL_MAX = 0x7fffffff;
 
 struct TabGeom { int nxf, nyf, tb, ntfp, rs; };
 __device__ __forceinline__ TabGeom tab_geom(int lox, int loy, int lot, int hix, int hiy, int hit, int E) {
@@ -198,13 +206,13 @@ k_effq_mark(int64_t nb, const int32_t* __restrict__ blk_off, const int32_t* __re
   for (int p = p0 + lane; p < p1; p += 32) mark[pair_seg[p]] = 1;
 }
 
-// mark[s] = size of the table of a marked segment in 16-byte units (0 if not marked)
+// mark[s] = size of the table of a marked segment in 16-byte units (0 if not marked);
+// *total (zeroed by the caller) += all sizes, in 64 bits (integer atomics: order does not matter)
 template <int N>
 __global__ void __launch_bounds__(256)
 k_effq_sizes(int64_t nseg, const float* __restrict__ augf, const int32_t* __restrict__ augi,
-             int32_t* __restrict__ mark) {
+             int32_t* __restrict__ mark, unsigned long long* __restrict__ total) {
   const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s > nseg) return;
   int v = 0;
   if (s < nseg && mark[s]) {
     constexpr int E = N > 1 ? 1 : 0;
@@ -214,21 +222,30 @@ k_effq_sizes(int64_t nseg, const float* __restrict__ augf, const int32_t* __rest
     const SegQuad q = seg_quad(augi[6 * nseg + s], augf[3 * nseg + s] - p0x, augf[4 * nseg + s] - p0y,
                                augf[5 * nseg + s] - p0t, augf[6 * nseg + s], augf[7 * nseg + s], augf[8 * nseg + s]);
     const int64_t sz = tab_floats(q.npiece * q.m, t.rs) >> 2;
-    v = sz < (1 << 24) ? (int)sz : (1 << 24);           // absurdly large boxes: no table (never fits)
+    // tables beyond 4 MiB (absurdly large boxes): size 0 = no table, the tile CTAs evaluate the
+    // segment themselves
+    v = sz <= TAB_SIZE_MAX ? (int)sz : 0;
   }
-  mark[s] = v;
+  if (s <= nseg) mark[s] = v;
+  unsigned long long w = (unsigned long long)v;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) w += __shfl_down_sync(0xffffffffu, w, o);
+  if ((threadIdx.x & 31) == 0 && w) atomicAdd(total, w);
 }
 
 // one warp per 32 consecutive segments; the marked ones among them one after the other
 template <int N>
 __global__ void __launch_bounds__(128)
-k_effq_tables(int64_t nseg, const int32_t* __restrict__ off, int64_t cap16, const float* __restrict__ augf,
-              const int32_t* __restrict__ augi, float* __restrict__ tab, TredGrid g) {
+k_effq_tables(int64_t nseg, const int32_t* __restrict__ off, const int64_t* __restrict__ total, int64_t cap16,
+              const float* __restrict__ augf, const int32_t* __restrict__ augi, float* __restrict__ tab, TredGrid g) {
   const int64_t w = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   const int64_t s_l = w * 32 + lane;
   bool mine = false;
-  if (s_l < nseg) { const int o0 = off[s_l], o1 = off[s_l + 1]; mine = o1 > o0 && (int64_t)o1 <= cap16; }
+  if (s_l < nseg && *total <= TAB_TOTAL_MAX) {
+    const int o0 = off[s_l], o1 = off[s_l + 1];
+    mine = o0 >= 0 && o1 > o0 && (int64_t)o1 <= cap16;
+  }
   uint32_t todo = __ballot_sync(0xffffffffu, mine);
   constexpr int E = N > 1 ? 1 : 0;
   constexpr float LOG2E_HALF = 0.72134752044448170f;
@@ -320,6 +337,7 @@ struct BlkParams {
   int nwj, nwi;      // warps along j, along i (warp -> (tick range, i range, j range))
   int ncw;           // consumer warps (the producer is warp ncw)
   int64_t cap16;     // 16-byte units of table workspace (0: no tables)
+  const int64_t* tab_total;   // sum of all table sizes (device; read only if there are tables)
 };
 
 __device__ __forceinline__ uint32_t eb_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -448,6 +466,7 @@ k_effq_blk(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __rest
     };
     // raw record of one lane: words 0..6 = bbox, flag; 7..16 = p0, p1, sigma, Q'; 17, 18 = table
     // offsets of s, s + 1 (all loads of a record in flight at once)
+    const bool tab_ok = tabofs && *P.tab_total <= TAB_TOTAL_MAX;      // offsets cannot have wrapped
     auto load_rec = [&](int b0, int nbatch, int32_t (&v)[19]) {
       if (lane < nbatch) {
         const int64_t s = pair_seg[b0 + lane];
@@ -455,8 +474,8 @@ k_effq_blk(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __rest
         for (int f = 0; f < 7; ++f) v[f] = augi[f * nseg + s];
 #pragma unroll
         for (int f = 7; f < 17; ++f) v[f] = __float_as_int(augf[(f - 7) * nseg + s]);
-        v[17] = tabofs ? tabofs[s] : 0;
-        v[18] = tabofs ? tabofs[s + 1] : 0;
+        v[17] = tab_ok ? tabofs[s] : 0;
+        v[18] = tab_ok ? tabofs[s + 1] : 0;
       }
     };
     Meta m_cur = load_meta(blockIdx.x), m_nxt = load_meta((int64_t)blockIdx.x + gridDim.x);
@@ -530,7 +549,7 @@ k_effq_blk(int64_t nseg, const int64_t* __restrict__ keys, const int32_t* __rest
             rec[ER_FT + 0] = kt0 - K0; rec[ER_FT + 1] = kt1 - K0; rec[ER_FT + 2] = a0; rec[ER_FT + 3] = a1 - a0;
             rec[ER_PTOT] = ptot; rec[ER_NPASS] = npass;
             const TabGeom t = tab_geom(lox, loy, lot, hix, hiy, hit, E);
-            const bool has = o1 > o0 && (int64_t)o1 <= P.cap16;
+            const bool has = o0 >= 0 && o1 > o0 && (int64_t)o1 <= P.cap16;
             rec[ER_TOFF] = has ? o0 : -1;
             rec[ER_TRS] = t.rs;
             rec[ER_TROW + 0] = ix0 - (lox - E);
@@ -899,7 +918,7 @@ k_truth_fill(int64_t nseg, const float* __restrict__ augf, const int32_t* __rest
 
 
 
-struct EffqWork { int32_t* off; void* scan; float* tab; int64_t cap16; size_t fixed; };
+struct EffqWork { int32_t* off; void* scan; int64_t* total; float* tab; int64_t cap16; size_t fixed; };
 
 static EffqWork carve_effq(void* base, int64_t nseg, size_t work_bytes) {
   EffqWork w;
@@ -907,6 +926,7 @@ static EffqWork carve_effq(void* base, int64_t nseg, size_t work_bytes) {
   auto take = [&](size_t bytes) { void* p = b ? b + o : nullptr; o += align_up(bytes, 256); return p; };
   w.off = (int32_t*)take((size_t)(nseg + 1) * 4);
   w.scan = take(tred_scan_work_bytes(nseg + 1));
+  w.total = (int64_t*)take(sizeof(int64_t));
   w.fixed = o;
   w.tab = (float*)(b ? b + o : nullptr);
   w.cap16 = work_bytes > o ? (int64_t)((work_bytes - o) / 16) : 0;
@@ -969,13 +989,15 @@ static int effq_launch(tred_ctx* ctx, const TredGrid& g, BlkParams P, int thread
   // few blocks: the four extra launches cost more than the tables save
   const bool tables = d_work && w.cap16 >= 4096 && nseg > 0 && nblocks >= 1024;
   P.cap16 = tables ? w.cap16 : 0;
+  P.tab_total = w.total;
   if (tables) {
     TRED_CUDA(cudaMemsetAsync(w.off, 0, (size_t)(nseg + 1) * 4, st));
     k_effq_mark<<<cdiv(nblocks * 32, 256), 256, 0, st>>>(nblocks, d_blk_off, d_pair_seg, w.off);
-    k_effq_sizes<N><<<cdiv(nseg + 1, 256), 256, 0, st>>>(nseg, d_augf, d_augi, w.off);
+    TRED_CUDA(cudaMemsetAsync(w.total, 0, sizeof(int64_t), st));
+    k_effq_sizes<N><<<cdiv(nseg + 1, 256), 256, 0, st>>>(nseg, d_augf, d_augi, w.off, (unsigned long long*)w.total);
     int rc = tred_exclusive_scan_i32(w.off, w.off, nseg + 1, nullptr, w.scan, st);
     if (rc != TRED_OK) return rc;
-    k_effq_tables<N><<<cdiv(nseg, 128), 128, 0, st>>>(nseg, w.off, w.cap16, d_augf, d_augi, w.tab, g);
+    k_effq_tables<N><<<cdiv(nseg, 128), 128, 0, st>>>(nseg, w.off, w.total, w.cap16, d_augf, d_augi, w.tab, g);
     TRED_COUNT_LAUNCH(5);
   }
   const int32_t* tabofs = tables ? w.off : nullptr;
@@ -1040,6 +1062,7 @@ extern "C" int tred_truth(tred_ctx* ctx, int64_t nseg, const float* d_augf, cons
                           int32_t* d_rec_seg, int64_t* d_rec_key, float* d_rec_q, int64_t* d_nrec, void* d_work,
                           size_t work_bytes, void* stream) {
   if (!ctx || nseg < 0 || cap_rec < 0 || !d_nrec) return TRED_EINVAL;
+  TRED_CHECK_DEVICE(ctx);
   cudaStream_t st = (cudaStream_t)stream;
   if (nseg == 0) { TRED_CUDA(cudaMemsetAsync(d_nrec, 0, sizeof(int64_t), st)); return TRED_OK; }
   if (!d_augf || !d_augi || !d_work) return TRED_EINVAL;

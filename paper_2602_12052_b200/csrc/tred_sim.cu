@@ -67,12 +67,12 @@ extern "C" int tred_simulate(tred_ctx* ctx, int64_t nseg, const float* seg, int 
                              int64_t cap_tiles, int64_t* tile_keys, float* tile_data, int out_on_host,
                              int64_t npix_req, const int32_t* d_pix_ids, float* d_dense,
                              tred_sim_result* res, void* stream) {
+  if (res) memset(res, 0, sizeof(*res));                 // defined on every return, errors included
   if (!ctx || nseg < 0 || !res || cap_tiles < 0 || npix_req < 0) return TRED_EINVAL;
+  res->nseg = nseg;
   TRED_CHECK_DEVICE(ctx);
   if (nseg > 0 && !seg) return TRED_EINVAL;
   if (nseg >= (1ll << 31)) return TRED_EUNSUPPORTED;
-  memset(res, 0, sizeof(*res));
-  res->nseg = nseg;
   cudaStream_t st = (cudaStream_t)stream;
   const tred_dims& d = ctx->dims;
   const int NBt = (int)d.NB[2];

@@ -29,6 +29,24 @@ def test_reference_arm_line():
     assert d["config"]["workload"] == "cfg1_single_track" and "model" not in d["config"]
 
 
+def test_gpus_2_without_a_launcher_starts_two_ranks():
+    """`bench.py --gpus 2` run as a plain script starts its own two ranks (torch.distributed.run,
+    127.0.0.1); on the reference arm rank 0 alone works and prints, the other exits 0: still ONE line."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference",
+                          "--config", "1", "--steps", "1", "--warmup", "0", "--ref-segments", "12"],
+                         capture_output=True, text=True, timeout=900, cwd=ROOT, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1, out.stdout
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["impl"] == "reference" and d["value"] > 0
+    # a launcher's world size that contradicts --gpus is refused, not silently reported as N
+    bad = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference"],
+                         capture_output=True, text=True, timeout=120, cwd=ROOT, env=dict(env, WORLD_SIZE="1", RANK="0"))
+    assert bad.returncode == 2 and "WORLD_SIZE" in bad.stderr
+
+
 @pytest.mark.gpu
 def test_cuda_arm_line():
     d = _run(["--config", "1", "--steps", "3", "--warmup", "3", "--ref-segments", "12"])

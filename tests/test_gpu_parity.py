@@ -226,8 +226,68 @@ def test_effq_point_like_and_clipped_segments(effq_mode):
     assert np.abs(got - ref).max() <= TOL_QEFF * np.abs(ref).max()
 
 
+def _effq_with_and_without_tables(cfg, segs, min_blocks=1024):
+    """tred_effq twice on the same blocks: with its default workspace (per-segment tables built once)
+    and with none (every tile CTA builds the rows it needs)."""
+    sim = _sim(cfg)
+    augf, augi, npairs = sim.drift(_seg_tensor(segs))
+    k, blk_off, pair_seg, slab_off, nblocks = sim.blockbin(augi, int(npairs.item()))
+    nb = int(nblocks.item())
+    assert nb >= min_blocks, nb                      # below that tred_effq never builds tables
+    a = sim.effq(nb, k, blk_off, pair_seg, augf, augi)[:nb].clone()
+    b = sim.effq(nb, k, blk_off, pair_seg, augf, augi, work_bytes=0)[:nb]
+    _torch().cuda.synchronize()
+    return a, b
+
+
+def test_effq_tables_and_no_tables_give_the_same_bits():
+    """The per-segment tables are a cache of what the tile CTAs would compute: same code, same
+    bits (tred.h: 'same values, slower'), on a config-3 sample large enough for tables."""
+    cfg, segs = gen.make_segments(3, n_vertices=4)
+    a, b = _effq_with_and_without_tables(cfg, segs)
+    assert float(a.abs().max()) > 0 and bool((a == b).all())
+
+
+def test_effq_table_offsets_cannot_wrap():
+    """Table offsets are int32 sums of table sizes in 16-byte units.  40 000 unsplit segments that
+    run ~100 mm along the drift (tables of ~1-2 MB each: hundreds of ticks x hundreds of quadrature
+    points) push the sum past 2^31; a wrapped offset must never pass for a valid one (it would
+    place a table in front of the workspace).  The library then builds no tables at all, so the
+    result must equal the no-table run bit for bit; one segment with a table beyond the per-table
+    limit (200 mm) rides along."""
+    cfg = gen.make_config(3)
+    rng = np.random.default_rng(5)
+    n = 40000
+    x0 = rng.uniform(20.0, 280.0, n)                 # a 60 x 60 pixel region: ~9 000 blocks, ~1 GB of payload
+    y0 = rng.uniform(20.0, 280.0, n)
+    z0 = rng.uniform(5.0, 15.0, n)
+    dz = rng.uniform(95.0, 105.0, n)
+    dz[0] = 200.0
+    cols = dict(x0=x0, y0=y0, z0=z0, x1=x0 + rng.uniform(-1.0, 1.0, n), y1=y0 + rng.uniform(-1.0, 1.0, n),
+                z1=z0 + dz, q=np.full(n, 5.0e5), t0=np.zeros(n))
+    segs = {k: cols[k].astype(np.float32) for k in gen.SEG_FIELDS}
+    a, b = _effq_with_and_without_tables(cfg, segs)
+    assert float(a.abs().max()) > 0 and bool(_torch().isfinite(a).all()) and bool((a == b).all())
+    # the charge is all there: drift attenuation only (lifetime 2200 us, <= 75 us of drift)
+    tot = float(a.double().sum())
+    assert 0.95 * 5.0e5 * n < tot < 5.0e5 * n * (1 + 1e-6)
+
+
 # ------------------------------------------------------------------ S4 + S5
-def _wave_checks(got, ref, mode):
+def _probe(record: dict):
+    """The measured error figures DESIGN.md "Tolerances" quotes: printed (pytest -s), and appended
+    as one JSON line to the file TRED_PROBE_OUT names, if set (profiles/r3_error_probe.md gives
+    the command that wrote the committed table)."""
+    import json
+    line = json.dumps(record)
+    print("probe:", line)
+    path = os.environ.get("TRED_PROBE_OUT")
+    if path:
+        with open(path, "a") as f:
+            f.write(line + "\n")
+
+
+def _wave_checks(got, ref, mode, tag=None):
     """`mode`: the spectrum-product kernel that ran (Tred.last_mac_mode())."""
     scale = np.abs(ref).max()
     assert scale > 0
@@ -236,6 +296,15 @@ def _wave_checks(got, ref, mode):
     l1 = np.abs(ref).sum(1)
     dq = np.abs(qg - qr)
     coll = (np.abs(qr) >= 0.1 * l1) & (np.abs(qr) >= 1e-3 * np.abs(qr).max())
+    if tag is not None:
+        u = 2.0 ** -24
+        _probe(dict(tag, mac_mode=int(mode), npix=int(len(l1)), ncollecting=int(coll.sum()),
+                    wave_max_err_over_max_signal=float(np.abs(got - ref).max() / scale),
+                    dq_over_ulp_l1_collecting=float((dq[coll] / (u * l1[coll])).max()) if coll.any() else None,
+                    dq_over_ulp_l1_other=float((dq[~coll & (l1 > 0)] / (u * l1[~coll & (l1 > 0)])).max())
+                    if (~coll & (l1 > 0)).any() else None,
+                    dq_rel_collecting=float((dq[coll] / np.abs(qr)[coll]).max()) if coll.any() else None,
+                    bound_other_ulp_l1=float(tol_qpix_l1(mode) / u)))
     assert (dq[coll] <= TOL_QPIX * np.abs(qr)[coll]).all(), (dq[coll] / np.abs(qr)[coll]).max()
     assert (dq[~coll] <= tol_qpix_l1(mode) * l1[~coll]).all(), (dq[~coll] / l1[~coll]).max() * 2.0 ** 24
     # pixels the oracle leaves exactly empty stay exactly empty
@@ -320,7 +389,59 @@ def test_convolve_parity_from_oracle_charge(cfg_id, mac_mode):
     got = _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix)
     # mode 4 needs a mirror-symmetric response (this one is) and 100 phases
     assert sim.last_mac_mode() == (7 if mac_mode == 0 else mac_mode)
-    _wave_checks(got.astype(np.float64), ref, sim.last_mac_mode())
+    _wave_checks(got.astype(np.float64), ref, sim.last_mac_mode(),
+                 tag=dict(test="convolve_parity_from_oracle_charge", cfg=cfg_id, requested=mac_mode))
+
+
+def test_convolve_response_dynamic_range():
+    """What the fp16 hi / lo operands of the default product (mac_mode 7) do to a response with a
+    wide range between its offsets (include/tred.h, tred_prepare_response): the split uses one
+    power-of-two scale per frequency for all offsets, so an offset at rho times that frequency's
+    largest entry keeps 22 bits only while rho >= 2^-18; below, its lo part falls into fp16
+    subnormals and its own contribution carries a relative error of about 2^-40 / rho.  Here the
+    offsets beyond the 3 x 3 centre are scaled down by 1e-5, which with the response's own decay
+    puts them at rho = 1e-7 .. 1e-6 of the centre: a pixel that only those offsets reach (induction
+    far from all charge) must still come out within 2e-5 of ITS OWN largest sample (2^-40 / rho
+    is 1e-6 .. 1e-5), while the fp32 FMA product (mode 1) is held to 5e-6; near pixels keep the
+    usual tolerance."""
+    torch = _torch()
+    cfg = gen.make_config(1, t_origin_us=0.0)
+    rows = [(70.0, 70.0, 40.0, 70.9, 70.6, 40.8, 50000.0, 0.0)]          # one short track inside one pixel
+    segs = {k: np.array([r[i] for r in rows], np.float32) for i, k in enumerate(gen.SEG_FIELDS)}
+    H = cfg.resp_half
+    R = gen.make_response(cfg, 2011).astype(np.float64)
+    far = np.ones((2 * H + 1, 2 * H + 1))
+    far[H - 1:H + 2, H - 1:H + 2] = 0.0
+    R *= np.where(far[None, None, :, :, None] > 0, 1.0e-5, 1.0)
+    R = np.ascontiguousarray(R, dtype=np.float32)
+    aug = o.drift(cfg, segs)
+    keys = o.blocks(cfg, aug)
+    payload32 = o.effq(cfg, aug, keys).astype(np.float32)
+    # the diffused charge sits on pixels (15..16, 15..16); every `farp` pixel is >= 2 pixels away
+    # from all four along at least one axis
+    px, py = 15, 15
+    assert aug["lo"][0, 0] // cfg.sub == px and aug["hi"][0, 0] // cfg.sub == px + 1
+    assert aug["lo"][0, 1] // cfg.sub == py and aug["hi"][0, 1] // cfg.sub == py + 1
+    near = [(px, py), (px + 1, py)]
+    farp = [(px + 4, py + 3), (px - 3, py + 4), (px + 4, py - 4), (px - 4, py)]
+    pix = np.array([a * cfg.npix_y + b for a, b in near + farp])
+    order = np.argsort(pix)
+    pix = pix[order]
+    is_far = np.array([False] * len(near) + [True] * len(farp))[order]
+    ref = o.conv_direct(cfg, keys, payload32.astype(np.float64), R, pix)
+    own = np.abs(ref).max(1)
+    rho = own[is_far] / own[~is_far].max()
+    assert rho.max() < 2e-6 and rho.min() > 5e-8, rho
+    for mode, tol_far in ((1, 5e-6), (7, 2e-5)):
+        sim = _sim(cfg.with_(mac_mode=mode))
+        rhat = sim.prepare_response(torch.from_numpy(R).cuda())
+        got = _convolve_oracle_charge(sim, cfg, keys, payload32, rhat, pix).astype(np.float64)
+        assert sim.last_mac_mode() == mode
+        rel = np.abs(got - ref).max(1) / own
+        _probe(dict(test="convolve_response_dynamic_range", mac_mode=mode, rho=[float(x) for x in rho],
+                    far_err_over_own_max=float(rel[is_far].max()), near_err_over_own_max=float(rel[~is_far].max())))
+        assert rel[~is_far].max() <= TOL_WAVE
+        assert rel[is_far].max() <= tol_far, (mode, rel[is_far].max())
 
 
 @pytest.mark.parametrize("block,tr", [((4, 4, 32), 200), ((8, 8, 64), 137), ((16, 16, 128), 400),
