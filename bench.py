@@ -369,6 +369,50 @@ def next_rows_overhead(torch, m, ms_step):
     return out
 
 
+def slab_pair_statistics(torch, m):
+    """Plan statistics for the transform length (PAPER.md:L264 pads every
+    block on its own): the share of charge pixels (time slab bt, pixel) whose pixel is also
+    occupied in slab bt + 1.  Greedily pairing such neighbours into one transform of 2 Bt ticks
+    (L2 = fft length of 2 Bt + Tr - 1) instead of two of L would change the spectrum bytes and
+    product flops by the factor reported.  Integer work on the plan's keys only."""
+    sim, cfg = m["sim"], m["cfg"]
+    augf, augi, npairs = sim.drift(m["seg_d"])
+    k, blk_off, pair_seg, slab_off, nblocks = sim.blockbin(augi, int(npairs.item()))
+    nb = int(nblocks.item())
+    p = sim.convolve_plan(nb, k)
+    ncp = int(p["ncp"].item())
+    cp = p["cp_keys"][:ncp]
+    npix = cfg.npix_x * cfg.npix_y
+    has_next = torch.isin(cp + npix, cp)
+    # greedy pairing along time per pixel: runs of consecutive slabs of one pixel, floor(len / 2) pairs
+    pix, bt = cp % npix, cp // npix
+    order = torch.argsort(pix * (int(sim.dims.NB[2]) + 1) + bt)
+    ps, bs = pix[order], bt[order]
+    brk = torch.ones_like(ps, dtype=torch.bool)
+    brk[1:] = (ps[1:] != ps[:-1]) | (bs[1:] != bs[:-1] + 1)
+    run_id = torch.cumsum(brk.to(torch.int64), 0) - 1
+    run_len = torch.bincount(run_id)
+    pairs = int((run_len // 2).sum().item())
+    singles = ncp - 2 * pairs
+
+    def fft_len(n):
+        best = None
+        a = 8
+        while a < 4 * n:
+            b = a
+            while b < 4 * n:
+                if b >= n and (best is None or b < best):
+                    best = b
+                b *= 3
+            a *= 2
+        return best
+    Bt, Tr = cfg.block[2], cfg.resp_nticks
+    L1, L2 = fft_len(Bt + Tr - 1), fft_len(2 * Bt + Tr - 1)
+    return {"charge_pixels": ncp, "with_occupied_next_slab": float(has_next.float().mean().item()),
+            "greedy_pairs": pairs, "singles": singles, "L": L1, "L_two_slabs": L2,
+            "spectrum_bytes_factor_if_paired": (pairs * L2 + singles * L1) / (ncp * L1)}
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -505,6 +549,7 @@ def run_cuda(args):
         if world == 1 and not args.no_extras:
             line["cufft_s4_comparison"] = cufft_s4_comparison(torch, m)
             line["next_rows"] = next_rows_overhead(torch, m, ms_max)
+            line["s4"]["two_slab_statistics"] = slab_pair_statistics(torch, m)
         segs, R = m["segs"], m["R"]
         # release the main workload before the other configurations are timed
         m.clear(); sim = None
